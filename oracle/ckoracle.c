@@ -1,0 +1,657 @@
+/*
+ * ckoracle.c -- CPU ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * A plain, slow, double-precision restatement of what the hot path computes, written from the paper
+ * (Niemeyer & Sung, arXiv 1309.2710; cited below as P:<line of /root/reference/PAPER.md>) step by step,
+ * in the paper's order and notation.  It shares no code, header, table or constant generator with the
+ * CUDA library under paper_1309_2710_b200/csrc/ (constants that appear in both are typed twice).
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load it.
+ *
+ * Build:  gcc -O2 -ffp-contract=off -fopenmp -fPIC -shared -o libckoracle.so ckoracle.c -lm
+ * (no fast-math, no FMA contraction: what is written is what is evaluated).
+ *
+ * Readings of the paper where it is silent / ambiguous / garbled are marked Rn; the list with the
+ * justification of each is DESIGN.md section 4 (same numbering as SURVEY.md section 9).
+ *
+ * Pins (tests/test_oracle_*.py, all run without a GPU):
+ *   Table 1                  : 17+8 rooted-tree order conditions in exact rationals, row sums, R(z) incl. z^6/800
+ *   ora_rkck_step            : y'=lambda y closed form R(z), R*(z); measured order 5 / 4 on y'=-y^2
+ *   ora_rkc_coeffs/_step     : stage closed form a_j + b_j T_j(w0 + w1 z) for s = 2..200; Chebyshev bound
+ *                              |P_s(z)| <= 1 on [-beta(s), 0]; measured order 2; c_1 = c_2/T_2'(w0)
+ *   ora_spectral_radius      : linear operators with known spectrum; FD-Jacobian eigenvalues on chemistry
+ *   ora_rhs                  : A->B, A->B->C (Bateman), A+B->C+D, A+M->B+M closed forms; Arrhenius in mpmath;
+ *                              Sum Y and element mass invariants
+ *   ora_rkck/rkc drivers     : tolerance proportionality, brute-force fixed-step reference, RKCK-vs-RKC
+ *                              cross-check, linear invariants.
+ *   PARITY UNPINNED (builder's reading, nothing in the paper or the mathematics fixes them):
+ *   R4 (RKCK first trial step), R5 (end-of-interval clipping), R6/R7 (failure codes), R10 (b_1 = b_2 for
+ *   nonlinear f), R13 (controller memory dropped after a rejection), R14/R15 (initial-step weights and cap),
+ *   R16 (sigma refresh rule), R17/R18 (power-method details and its 1.2 safety factor).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* R20: physical constants (the paper gives none) */
+#define ORA_RU 8.314462618e7   /* erg / (mol K)  */
+#define ORA_RC 1.98720425864   /* cal / (mol K)  */
+
+#define ORA_OK 0
+#define ORA_EINVAL (-1)
+#define ORA_ENOMEM (-2)
+
+/* per-system status codes */
+#define ST_OK 0
+#define ST_MAXSTEPS 1
+#define ST_UNDERFLOW 2
+#define ST_NONFINITE 3
+#define ST_SIGMA 4
+
+typedef void (*ora_rhs_fn)(double t, const double *y, double *dydt, void *ctx);
+
+/* ------------------------------------------------------------------------------------------------
+ * Table 1, R1: rows 4-6 are scrambled in the extraction; these are the Cash-Karp values
+ * every legible fragment of the table agrees with.  Pinned exactly by the order-condition test.
+ * ---------------------------------------------------------------------------------------------- */
+static const double CK_A[7] = {0, 0.0, 1.0 / 5.0, 3.0 / 10.0, 3.0 / 5.0, 1.0, 7.0 / 8.0};
+static const double CK_B[7][6] = {
+    {0},
+    {0},
+    {0, 1.0 / 5.0},
+    {0, 3.0 / 40.0, 9.0 / 40.0},
+    {0, 3.0 / 10.0, -9.0 / 10.0, 6.0 / 5.0},
+    {0, -11.0 / 54.0, 5.0 / 2.0, -70.0 / 27.0, 35.0 / 27.0},
+    {0, 1631.0 / 55296.0, 175.0 / 512.0, 575.0 / 13824.0, 44275.0 / 110592.0, 253.0 / 4096.0}};
+static const double CK_C[7] = {0, 37.0 / 378.0, 0.0, 250.0 / 621.0, 125.0 / 594.0, 0.0, 512.0 / 1771.0};
+static const double CK_CS[7] = {0, 2825.0 / 27648.0, 0.0, 18575.0 / 48384.0, 13525.0 / 55296.0,
+                                277.0 / 14336.0, 1.0 / 4.0};
+
+/* test access to the table as rationals' double values: out[0..5]=a, [6..35]=b (6x5 row-major, b_ij j=1..5),
+ * [36..41]=c, [42..47]=c* */
+void ora_rkck_tableau(double *out) {
+  for (int i = 1; i <= 6; i++) out[i - 1] = CK_A[i];
+  for (int i = 1; i <= 6; i++)
+    for (int j = 1; j <= 5; j++) out[6 + (i - 1) * 5 + (j - 1)] = CK_B[i][j];
+  for (int i = 1; i <= 6; i++) out[36 + i - 1] = CK_C[i];
+  for (int i = 1; i <= 6; i++) out[42 + i - 1] = CK_CS[i];
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * One RKCK step of size h from (t, y): Eq. 7-15.  k1 = h f(t,y) is supplied by the caller
+ * (Eq. 7).  ynew = 5th-order solution (Eq. 13), delta = y_{n+1} - y*_{n+1} (Eq. 15).
+ * work: 6*n doubles.
+ * ---------------------------------------------------------------------------------------------- */
+static void rkck_attempt(ora_rhs_fn f, void *ctx, int n, double t, const double *y, const double *k1,
+                         double h, double *ynew, double *delta, double *work) {
+  double *k[7];
+  k[1] = (double *)k1;
+  for (int i = 2; i <= 6; i++) k[i] = work + (size_t)(i - 2) * n;
+  double *ytmp = work + (size_t)5 * n;
+  for (int i = 2; i <= 6; i++) { /* Eq. 8-12 */
+    for (int c = 0; c < n; c++) {
+      double s = y[c];
+      for (int j = 1; j < i; j++) s += CK_B[i][j] * k[j][c];
+      ytmp[c] = s;
+    }
+    f(t + CK_A[i] * h, ytmp, k[i], ctx);
+    for (int c = 0; c < n; c++) k[i][c] *= h;
+  }
+  for (int c = 0; c < n; c++) {
+    double s = y[c], d = 0.0;
+    for (int i = 1; i <= 6; i++) {
+      s += CK_C[i] * k[i][c];               /* Eq. 13 */
+      d += (CK_C[i] - CK_CS[i]) * k[i][c];  /* Eq. 15 */
+    }
+    ynew[c] = s;
+    delta[c] = d;
+  }
+}
+
+/* fixed-step entry for the order / closed-form tests (controller off) */
+void ora_rkck_step(ora_rhs_fn f, void *ctx, int n, double t, const double *y, double h, double *ynew,
+                   double *delta) {
+  double *work = (double *)malloc(sizeof(double) * (size_t)n * 7);
+  double *k1 = work + (size_t)6 * n;
+  f(t, y, k1, ctx);
+  for (int c = 0; c < n; c++) k1[c] *= h; /* Eq. 7 */
+  rkck_attempt(f, ctx, n, t, y, k1, h, ynew, delta, work);
+  free(work);
+}
+
+static int all_finite(const double *v, int n) {
+  for (int i = 0; i < n; i++)
+    if (!isfinite(v[i])) return 0;
+  return 1;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * RKCK driver.  Integrates y from t0 to t1 in place.
+ * stats[0]=RHS evaluations, [1]=accepted steps, [2]=rejected steps, [3]=0.  Returns a status code.
+ * ---------------------------------------------------------------------------------------------- */
+int ora_rkck_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol,
+                     double atol, int32_t *stats) {
+  const double S = 0.9;
+  const double u = 2.220446049250313e-16;     /* 2^-52 */
+  double *buf = (double *)malloc(sizeof(double) * (size_t)n * 9);
+  double *k1 = buf, *ynew = buf + n, *delta = buf + 2 * (size_t)n, *work = buf + 3 * (size_t)n;
+  int32_t nfe = 0, nacc = 0, nrej = 0;
+  int status = ST_OK;
+  double t = t0;
+  double h = t1 - t0;                         /* R4: first trial step = the whole global step */
+  int have_k1 = 0;
+  long attempts = 0;
+  int saw_nonfinite = 0;
+  while (1) {
+    int last = 0;
+    if (1.1 * h >= t1 - t) {                  /* R5: clip (with 10 % stretch) to hit t1 exactly */
+      double hn = t1 - t;
+      if (have_k1) { double r = hn / h; for (int c = 0; c < n; c++) k1[c] *= r; }
+      h = hn;
+      last = 1;
+    }
+    if (!have_k1) {
+      f(t, y, k1, ctx);                       /* Eq. 7 */
+      nfe++;
+      for (int c = 0; c < n; c++) k1[c] *= h;
+      have_k1 = 1;
+    }
+    if (++attempts > 1000000) { status = ST_MAXSTEPS; break; }           /* R7 */
+    rkck_attempt(f, ctx, n, t, y, k1, h, ynew, delta, work);
+    nfe += 5;
+    /* Eq. 16 (R2: eps -> rtol, eps*delta -> atol) and Eq. 17 (R3: errmax = max |Delta_i| / Delta0_i) */
+    double errmax = 0.0;
+    int finite = all_finite(ynew, n);
+    for (int c = 0; c < n; c++) {
+      double d0 = rtol * (fabs(y[c]) + fabs(k1[c])) + atol;
+      double e = fabs(delta[c]) / d0;
+      if (!(e <= errmax)) errmax = e;          /* NaN propagates into errmax */
+    }
+    if (finite && errmax <= 1.0) {             /* P:139 accept */
+      nacc++;
+      for (int c = 0; c < n; c++) y[c] = ynew[c];
+      have_k1 = 0;
+      if (last) { t = t1; break; }
+      t += h;
+      double fac = (errmax > 0.0) ? S * pow(errmax, -0.2) : 5.0;
+      if (fac > 5.0) fac = 5.0;                /* P:144 increases limited to five */
+      h *= fac;
+    } else {                                   /* reject */
+      nrej++;
+      double fac;
+      if (finite && isfinite(errmax)) {
+        fac = S * pow(errmax, -0.25);
+        if (fac < 0.1) fac = 0.1;              /* P:144 decreases limited to ten */
+      } else {
+        fac = 0.1;                             /* R7: non-finite -> plain rejection */
+        saw_nonfinite = 1;
+      }
+      double hn = h * fac;
+      for (int c = 0; c < n; c++) k1[c] *= fac; /* R25: k1 = hn f(t,y), rescaled not re-evaluated */
+      h = hn;
+      double tmax = fabs(t) > fabs(t1) ? fabs(t) : fabs(t1);
+      if (!(h > 10.0 * u * tmax)) {            /* R6 */
+        status = saw_nonfinite ? ST_NONFINITE : ST_UNDERFLOW;
+        break;
+      }
+    }
+  }
+  if (stats) { stats[0] = nfe; stats[1] = nacc; stats[2] = nrej; stats[3] = 0; }
+  free(buf);
+  return status;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * RKC coefficients for s >= 2 stages: Eq. 22-29.  Arrays are indexed 0..s.
+ *   R8 : w0 = 1 + eps/s^2 with eps = kappa = 2/13.
+ *   R9 : a_j = 1 - b_j T_j(w0)  (used in Eq. 23, never defined in the paper).
+ *   R10: b_0 = b_1 = b_2 (Eq. 24 prints b_1 = 1/w0, which contradicts Eq. 27's c_1 = c_2/T_2'(w0)).
+ *   R11: c_1 = mu~_1, c_j = w1 T_j''/T_j' (2 <= j <= s-1), c_s = 1.
+ * Chebyshev values by the recurrences obtained from Eq. 26 and its derivatives.
+ * ---------------------------------------------------------------------------------------------- */
+int ora_rkc_coeffs(int s, double *w0_out, double *w1_out, double *mu, double *nu, double *mut,
+                   double *gamt, double *c, double *a, double *b) {
+  if (s < 2) return ORA_EINVAL;
+  double *T = (double *)malloc(sizeof(double) * (size_t)(s + 1) * 3);
+  double *dT = T + (s + 1), *d2T = T + 2 * (s + 1);
+  const double w0 = 1.0 + (2.0 / 13.0) / ((double)s * (double)s);
+  T[0] = 1.0; T[1] = w0; dT[0] = 0.0; dT[1] = 1.0; d2T[0] = 0.0; d2T[1] = 0.0;
+  for (int j = 2; j <= s; j++) {
+    T[j] = 2.0 * w0 * T[j - 1] - T[j - 2];                          /* Eq. 26 */
+    dT[j] = 2.0 * T[j - 1] + 2.0 * w0 * dT[j - 1] - dT[j - 2];
+    d2T[j] = 4.0 * dT[j - 1] + 2.0 * w0 * d2T[j - 1] - d2T[j - 2];
+  }
+  const double w1 = dT[s] / d2T[s];                                  /* Eq. 25 */
+  for (int j = 2; j <= s; j++) b[j] = d2T[j] / (dT[j] * dT[j]);      /* Eq. 24 */
+  b[0] = b[2]; b[1] = b[2];                                          /* R10 */
+  for (int j = 0; j <= s; j++) a[j] = 1.0 - b[j] * T[j];             /* R9 */
+  mu[0] = nu[0] = mut[0] = gamt[0] = 0.0; c[0] = 0.0;
+  mu[1] = nu[1] = gamt[1] = 0.0;
+  mut[1] = b[1] * w1;                                                /* Eq. 22 */
+  c[1] = mut[1];
+  for (int j = 2; j <= s; j++) {                                     /* Eq. 23 */
+    mu[j] = 2.0 * b[j] * w0 / b[j - 1];
+    nu[j] = -b[j] / b[j - 2];
+    mut[j] = 2.0 * b[j] * w1 / b[j - 1];
+    gamt[j] = -a[j - 1] * mut[j];
+    c[j] = (j < s) ? w1 * d2T[j] / dT[j] : 1.0;                      /* Eq. 28-29 */
+  }
+  *w0_out = w0; *w1_out = w1;
+  free(T);
+  return ORA_OK;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * One RKC step with s stages: Eq. 18-21.  f0 = f(t, y).  If stages != NULL, stage vectors
+ * w_1..w_s are stored there ([s][n]) for the closed-form test.  Evaluates f at w_1..w_{s-1}: s-1 calls.
+ * ---------------------------------------------------------------------------------------------- */
+static void rkc_step(ora_rhs_fn f, void *ctx, int n, double t, const double *y, const double *f0,
+                     double h, int s, double *ynew, double *stages, double *work /* 3n */) {
+  double *wjm1 = work, *wjm2 = work + n, *fj = work + 2 * (size_t)n;
+  double *cf = (double *)malloc(sizeof(double) * 7 * (size_t)(s + 1));
+  double *mu = cf, *nu = cf + (s + 1), *mut = cf + 2 * (s + 1), *gamt = cf + 3 * (s + 1),
+         *c = cf + 4 * (s + 1), *a = cf + 5 * (s + 1), *b = cf + 6 * (s + 1);
+  double w0, w1;
+  ora_rkc_coeffs(s, &w0, &w1, mu, nu, mut, gamt, c, a, b);
+  for (int i = 0; i < n; i++) {            /* Eq. 18-19 */
+    wjm2[i] = y[i];
+    wjm1[i] = y[i] + mut[1] * h * f0[i];
+  }
+  if (stages) memcpy(stages, wjm1, sizeof(double) * n);
+  for (int j = 2; j <= s; j++) {           /* Eq. 20 */
+    f(t + c[j - 1] * h, wjm1, fj, ctx);
+    for (int i = 0; i < n; i++) {
+      double wj = (1.0 - mu[j] - nu[j]) * y[i] + mu[j] * wjm1[i] + nu[j] * wjm2[i] +
+                  mut[j] * h * fj[i] + gamt[j] * h * f0[i];
+      wjm2[i] = wjm1[i];
+      wjm1[i] = wj;
+    }
+    if (stages) memcpy(stages + (size_t)(j - 1) * n, wjm1, sizeof(double) * n);
+  }
+  for (int i = 0; i < n; i++) ynew[i] = wjm1[i]; /* Eq. 21 */
+  free(cf);
+}
+
+void ora_rkc_step(ora_rhs_fn f, void *ctx, int n, double t, const double *y, double h, int s,
+                  double *ynew, double *stages) {
+  double *work = (double *)malloc(sizeof(double) * (size_t)4 * n);
+  double *f0 = work + 3 * (size_t)n;
+  f(t, y, f0, ctx);
+  rkc_step(f, ctx, n, t, y, f0, h, s, ynew, stages, work);
+  free(work);
+}
+
+static double norm2(const double *v, int n) {
+  double s = 0.0;
+  for (int i = 0; i < n; i++) s += v[i] * v[i];
+  return sqrt(s);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Spectral radius by a nonlinear power method (P:233 names it, gives no detail): R17/R18, DESIGN.md 4.5.
+ * y, fy = f(t,y); v = previous eigenvector estimate (have_v) or scratch; on return v holds the new one.
+ * Returns 1.2 * sigma; *nfe += RHS calls; *flag = ST_SIGMA if not converged in 50 iterations.
+ * work: 2n doubles.
+ * ---------------------------------------------------------------------------------------------- */
+static double spectral_radius(ora_rhs_fn f, void *ctx, int n, double t, const double *y, const double *fy,
+                              double *v, int have_v, int32_t *nfe, int *flag, double *work) {
+  const double u = 2.220446049250313e-16;
+  const double sqrtu = 1.4901161193847656e-08; /* 2^-26 */
+  double *z = work, *g = work + n;
+  if (!have_v)
+    for (int i = 0; i < n; i++) v[i] = fy[i];
+  const double ynrm = norm2(y, n), vnrm = norm2(v, n);
+  double d;
+  if (ynrm != 0.0 && vnrm != 0.0) {
+    d = ynrm * sqrtu;
+    for (int i = 0; i < n; i++) z[i] = y[i] + v[i] * (d / vnrm);
+  } else if (ynrm != 0.0) {
+    d = ynrm * sqrtu;
+    for (int i = 0; i < n; i++) z[i] = y[i] * (1.0 + sqrtu);
+  } else if (vnrm != 0.0) {
+    d = u;
+    for (int i = 0; i < n; i++) z[i] = v[i] * (d / vnrm);
+  } else {
+    d = u;
+    for (int i = 0; i < n; i++) z[i] = d;
+  }
+  double sigma = 0.0;
+  int converged = 0;
+  for (int it = 1; it <= 50; it++) {
+    f(t, z, g, ctx);
+    (*nfe)++;
+    double dd = 0.0;
+    for (int i = 0; i < n; i++) dd += (g[i] - fy[i]) * (g[i] - fy[i]);
+    dd = sqrt(dd);
+    const double sigma_prev = sigma;
+    sigma = dd / d;
+    const double floor_ = sigma > 1e-300 ? sigma : 1e-300;
+    if (it >= 2 && fabs(sigma - sigma_prev) <= 0.01 * floor_) { converged = 1; break; }
+    if (dd != 0.0) {
+      for (int i = 0; i < n; i++) z[i] = y[i] + (g[i] - fy[i]) * (d / dd);
+    } else {
+      const int i = it % n;
+      z[i] = y[i] - (z[i] - y[i]);
+    }
+  }
+  for (int i = 0; i < n; i++) v[i] = z[i] - y[i];
+  if (!converged) *flag = ST_SIGMA;
+  return 1.2 * sigma;
+}
+
+/* test entry */
+double ora_spectral_radius(ora_rhs_fn f, void *ctx, int n, double t, const double *y, double *v,
+                           int have_v, int32_t *nfe, int32_t *flag) {
+  double *work = (double *)malloc(sizeof(double) * (size_t)n * 3);
+  double *fy = work + 2 * (size_t)n;
+  int32_t calls = 0;
+  int fl = 0;
+  f(t, y, fy, ctx);
+  double s = spectral_radius(f, ctx, n, t, y, fy, v, have_v, &calls, &fl, work);
+  if (nfe) *nfe = calls;
+  if (flag) *flag = fl;
+  free(work);
+  return s;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * RKC driver: Eq. 30-39 and P:233.  Integrates y from t0 to t1 in place.
+ * stats[0]=RHS evaluations, [1]=accepted, [2]=rejected, [3]=largest stage count used.
+ * ---------------------------------------------------------------------------------------------- */
+int ora_rkc_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol,
+                    double atol, int32_t *stats) {
+  const double u = 2.220446049250313e-16;
+  const double Dt = t1 - t0;
+  /* R12: round-off cap on the stage count, s_max = max(2, round(sqrt(rtol/(10 u)))) */
+  int s_max = (int)floor(sqrt(rtol / (10.0 * u)) + 0.5);
+  if (s_max < 2) s_max = 2;
+  const size_t nn = (size_t)n;
+  double *buf = (double *)malloc(sizeof(double) * nn * 9);
+  double *f0 = buf, *fnew = buf + nn, *ynew = buf + 2 * nn, *v = buf + 3 * nn, *pw = buf + 4 * nn,
+         *sw = buf + 6 * nn;
+  int32_t nfe = 0, nacc = 0, nrej = 0, smax_used = 0;
+  int status = ST_OK, flag = 0;
+  double t = t0;
+
+  f(t, y, f0, ctx);
+  nfe++;
+  double sigma = spectral_radius(f, ctx, n, t, y, f0, v, 0, &nfe, &flag, pw);
+  int sigma_fresh = 1, need_sigma = 0, since_sigma = 0;
+
+  /* initial step: Eq. 36-38, R14 weights atol + rtol |y_0|, R15 caps at the global step */
+  double h;
+  {
+    double h0 = (sigma > 0.0 && 1.0 / sigma < Dt) ? 1.0 / sigma : Dt;      /* Eq. 36 */
+    double *z = pw, *g = pw + nn;
+    for (int i = 0; i < n; i++) z[i] = y[i] + h0 * f0[i];
+    f(t + h0, z, g, ctx);
+    nfe++;
+    double acc = 0.0;
+    for (int i = 0; i < n; i++) {
+      double d0 = h0 * (g[i] - f0[i]);                                     /* Eq. 37 */
+      double wt = atol + rtol * fabs(y[i]);
+      acc += (d0 / wt) * (d0 / wt);
+    }
+    double est = sqrt(acc / (double)n);                                    /* Eq. 31 */
+    h = Dt;
+    if (est > 0.0) {
+      double h1 = 0.1 * h0 / sqrt(est);                                    /* Eq. 38 */
+      if (h1 < Dt) h = h1;
+    }
+  }
+
+  int have_prev = 0;           /* an accepted step precedes, with no rejection since (R13) */
+  double err_old = 0.0, h_old = 0.0;
+  long attempts = 0;
+  int saw_nonfinite = 0;
+  while (1) {
+    int last = 0;
+    if (1.1 * h >= t1 - t) { h = t1 - t; last = 1; }                       /* R5 */
+    if (need_sigma) {                                                      /* P:233, R16 */
+      sigma = spectral_radius(f, ctx, n, t, y, f0, v, 1, &nfe, &flag, pw);
+      sigma_fresh = 1; need_sigma = 0; since_sigma = 0;
+    }
+    int s = 1 + (int)floor(sqrt(1.0 + 1.54 * h * sigma));                  /* Eq. 39, R12 truncation */
+    if (s < 2) s = 2;
+    if (s > s_max) {
+      s = s_max;
+      h = ((double)s_max * (double)s_max - 1.0) / (1.54 * sigma);
+      last = 0;
+    }
+    if (s > smax_used) smax_used = s;
+    if (++attempts > 1000000) { status = ST_MAXSTEPS; break; }
+    rkc_step(f, ctx, n, t, y, f0, h, s, ynew, NULL, sw);
+    f(t + h, ynew, fnew, ctx);
+    nfe += s;
+    /* Eq. 30-32 */
+    double acc = 0.0;
+    for (int i = 0; i < n; i++) {
+      double del = 0.8 * (y[i] - ynew[i]) + 0.4 * h * (f0[i] + fnew[i]);
+      double ym = fabs(y[i]) > fabs(ynew[i]) ? fabs(y[i]) : fabs(ynew[i]);
+      double wt = atol + rtol * ym;
+      acc += (del / wt) * (del / wt);
+    }
+    double err = sqrt(acc / (double)n);
+    if (err <= 1.0) {                                                      /* accept */
+      nacc++;
+      double fac;
+      if (err > 0.0) {
+        double e3 = cbrt(err);
+        if (have_prev) fac = 0.8 * (cbrt(err_old) / e3) * (h / h_old) * (1.0 / e3);   /* Eq. 34, R13 */
+        else fac = 0.8 / e3;
+      } else fac = 10.0;                                                   /* R26 */
+      if (fac < 0.1) fac = 0.1;
+      if (fac > 10.0) fac = 10.0;                                          /* Eq. 33 */
+      for (int i = 0; i < n; i++) { y[i] = ynew[i]; f0[i] = fnew[i]; }
+      err_old = err; h_old = h; have_prev = 1;
+      sigma_fresh = 0;
+      if (++since_sigma >= 25) need_sigma = 1;
+      if (last) { t = t1; break; }
+      t += h;
+      h *= fac;
+    } else {                                                               /* reject: Eq. 35 */
+      nrej++;
+      double fac;
+      if (isfinite(err)) {
+        fac = 0.8 / cbrt(err);
+        if (fac < 0.1) fac = 0.1;
+        if (fac > 10.0) fac = 10.0;
+      } else { fac = 0.1; saw_nonfinite = 1; }
+      h *= fac;
+      have_prev = 0;
+      if (!sigma_fresh) need_sigma = 1;                                    /* R16 */
+      double tmax = fabs(t) > fabs(t1) ? fabs(t) : fabs(t1);
+      if (!(h > 10.0 * u * tmax)) { status = saw_nonfinite ? ST_NONFINITE : ST_UNDERFLOW; break; }
+    }
+  }
+  if (status == ST_OK && flag) status = flag;
+  if (stats) { stats[0] = nfe; stats[1] = nacc; stats[2] = nrej; stats[3] = smax_used; }
+  free(buf);
+  return status;
+}
+
+/* ================================================================================================
+ * Chemistry: mechanism tables and the source term, Eq. 2-6, DESIGN.md 4.3
+ * ============================================================================================== */
+typedef struct {
+  int32_t n_species, n_reactions;
+  const double *mol_weight, *nasa, *arr_A, *arr_beta, *arr_E;
+  const int32_t *reac_ptr, *reac_species, *reac_nu, *prod_ptr, *prod_species, *prod_nu;
+  int32_t n_third_body;
+  const int32_t *tb_reaction, *tb_ptr, *tb_species;
+  const double *tb_eff;
+} ora_mech_desc;
+
+typedef struct ora_mech {
+  int K, R;
+  double *W, *nasa, *A, *beta, *E;
+  int32_t *reac_ptr, *reac_sp, *reac_nu, *prod_ptr, *prod_sp, *prod_nu;
+  int32_t *tb_of; /* [R] index of the reaction's third-body row, or -1 */
+  double *alpha;  /* [R3][K] dense third-body efficiencies (1 where not listed) */
+  int R3;
+} ora_mech;
+
+static void *dup_mem(const void *src, size_t bytes) {
+  void *p = malloc(bytes ? bytes : 1);
+  if (p && bytes) memcpy(p, src, bytes);
+  return p;
+}
+
+void ora_mech_free(ora_mech *m) {
+  if (!m) return;
+  free(m->W); free(m->nasa); free(m->A); free(m->beta); free(m->E);
+  free(m->reac_ptr); free(m->reac_sp); free(m->reac_nu);
+  free(m->prod_ptr); free(m->prod_sp); free(m->prod_nu);
+  free(m->tb_of); free(m->alpha);
+  free(m);
+}
+
+int ora_mech_load(const ora_mech_desc *d, ora_mech **out) {
+  if (!d || !out || d->n_species < 1 || d->n_reactions < 0) return ORA_EINVAL;
+  const int K = d->n_species, R = d->n_reactions, R3 = d->n_third_body;
+  for (int j = 0; j < R; j++) {
+    if (d->reac_ptr[j + 1] < d->reac_ptr[j] || d->prod_ptr[j + 1] < d->prod_ptr[j]) return ORA_EINVAL;
+    for (int e = d->reac_ptr[j]; e < d->reac_ptr[j + 1]; e++)
+      if (d->reac_species[e] < 0 || d->reac_species[e] >= K || d->reac_nu[e] < 1) return ORA_EINVAL;
+    for (int e = d->prod_ptr[j]; e < d->prod_ptr[j + 1]; e++)
+      if (d->prod_species[e] < 0 || d->prod_species[e] >= K || d->prod_nu[e] < 1) return ORA_EINVAL;
+  }
+  ora_mech *m = (ora_mech *)calloc(1, sizeof(ora_mech));
+  if (!m) return ORA_ENOMEM;
+  m->K = K; m->R = R; m->R3 = R3;
+  m->W = dup_mem(d->mol_weight, sizeof(double) * K);
+  m->nasa = dup_mem(d->nasa, sizeof(double) * K * 7);
+  m->A = dup_mem(d->arr_A, sizeof(double) * R);
+  m->beta = dup_mem(d->arr_beta, sizeof(double) * R);
+  m->E = dup_mem(d->arr_E, sizeof(double) * R);
+  m->reac_ptr = dup_mem(d->reac_ptr, sizeof(int32_t) * (R + 1));
+  m->prod_ptr = dup_mem(d->prod_ptr, sizeof(int32_t) * (R + 1));
+  const int nr = R ? d->reac_ptr[R] : 0, np = R ? d->prod_ptr[R] : 0;
+  m->reac_sp = dup_mem(d->reac_species, sizeof(int32_t) * nr);
+  m->reac_nu = dup_mem(d->reac_nu, sizeof(int32_t) * nr);
+  m->prod_sp = dup_mem(d->prod_species, sizeof(int32_t) * np);
+  m->prod_nu = dup_mem(d->prod_nu, sizeof(int32_t) * np);
+  m->tb_of = (int32_t *)malloc(sizeof(int32_t) * (R ? R : 1));
+  m->alpha = (double *)malloc(sizeof(double) * (size_t)(R3 ? R3 : 1) * K);
+  for (int j = 0; j < R; j++) m->tb_of[j] = -1;
+  for (int r = 0; r < R3; r++) {
+    const int j = d->tb_reaction[r];
+    if (j < 0 || j >= R) { ora_mech_free(m); return ORA_EINVAL; }
+    m->tb_of[j] = r;
+    for (int k = 0; k < K; k++) m->alpha[(size_t)r * K + k] = 1.0;
+    for (int e = d->tb_ptr[r]; e < d->tb_ptr[r + 1]; e++) {
+      if (d->tb_species[e] < 0 || d->tb_species[e] >= K) { ora_mech_free(m); return ORA_EINVAL; }
+      m->alpha[(size_t)r * K + d->tb_species[e]] = d->tb_eff[e];
+    }
+  }
+  *out = m;
+  return ORA_OK;
+}
+
+/* f(y): y = {T, Y_1..Y_K}, constant pressure p (dyn/cm^2).  work: 2K + R doubles. */
+static void chem_rhs(const ora_mech *m, const double *y, double p, double *dydt, double *work) {
+  const int K = m->K, R = m->R;
+  const double T = y[0];
+  const double *Y = y + 1;
+  double *C = work, *wdot = work + K, *Omega = work + 2 * (size_t)K;
+  /* R9a: ideal gas at constant pressure: rho = p Wbar/(Ru T), 1/Wbar = sum Y_k/W_k; C_k = rho Y_k / W_k */
+  double Sum = 0.0;
+  for (int k = 0; k < K; k++) Sum += Y[k] / m->W[k];
+  const double rho = p / (ORA_RU * T * Sum);
+  for (int k = 0; k < K; k++) C[k] = rho * Y[k] / m->W[k];
+  for (int j = 0; j < R; j++) {
+    const double kj = m->A[j] * pow(T, m->beta[j]) * exp(-m->E[j] / (ORA_RC * T));   /* Eq. 5, literal */
+    double rate = kj;
+    if (m->tb_of[j] >= 0) {                 /* R22: [M]_j = sum_k alpha_jk C_k */
+      const double *al = m->alpha + (size_t)m->tb_of[j] * K;
+      double M = 0.0;
+      for (int k = 0; k < K; k++) M += al[k] * C[k];
+      rate *= M;
+    }
+    for (int e = m->reac_ptr[j]; e < m->reac_ptr[j + 1]; e++) /* Eq. 4, integer orders; R19 no clipping */
+      for (int q = 0; q < m->reac_nu[e]; q++) rate *= C[m->reac_sp[e]];
+    Omega[j] = rate;
+  }
+  for (int k = 0; k < K; k++) wdot[k] = 0.0;
+  for (int j = 0; j < R; j++) {             /* Eq. 3 */
+    for (int e = m->prod_ptr[j]; e < m->prod_ptr[j + 1]; e++) wdot[m->prod_sp[e]] += m->prod_nu[e] * Omega[j];
+    for (int e = m->reac_ptr[j]; e < m->reac_ptr[j + 1]; e++) wdot[m->reac_sp[e]] -= m->reac_nu[e] * Omega[j];
+  }
+  /* R8a: NASA 7-coefficient fits, one range */
+  double cp_sum = 0.0, h_sum = 0.0;
+  const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+  for (int k = 0; k < K; k++) {
+    const double *a = m->nasa + 7 * (size_t)k;
+    const double cpR = a[0] + a[1] * T + a[2] * T2 + a[3] * T3 + a[4] * T4;
+    const double hRT = a[0] + a[1] * T / 2.0 + a[2] * T2 / 3.0 + a[3] * T3 / 4.0 + a[4] * T4 / 5.0 + a[5] / T;
+    cp_sum += Y[k] * cpR / m->W[k];
+    h_sum += hRT * wdot[k];                 /* (h_k W_k)/(Ru T) * omega_k */
+  }
+  const double cp = ORA_RU * cp_sum;        /* mass-averaged c_p */
+  dydt[0] = -(ORA_RU * T * h_sum) / (rho * cp);                 /* Eq. 6 */
+  for (int k = 0; k < K; k++) dydt[1 + k] = m->W[k] * wdot[k] / rho; /* Eq. 2 */
+}
+
+void ora_rhs(const ora_mech *m, const double *y, double p, double *dydt) {
+  double *work = (double *)malloc(sizeof(double) * (2 * (size_t)m->K + (size_t)m->R + 1));
+  chem_rhs(m, y, p, dydt, work);
+  free(work);
+}
+
+typedef struct { const ora_mech *m; double p; double *work; } chem_ctx;
+
+static void chem_rhs_cb(double t, const double *y, double *dydt, void *ctx) {
+  (void)t;                                   /* autonomous */
+  chem_ctx *c = (chem_ctx *)ctx;
+  chem_rhs(c->m, y, c->p, dydt, c->work);
+}
+
+/* Batch entry mirroring the product's integrate(): states are HOST, SoA [(K+1)][ld], updated in place.
+ * method 0 = RKCK, 1 = RKC.  status [N] and stats [4][N] may be NULL.  nthreads <= 0 -> OpenMP default. */
+int ora_integrate(const ora_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                  int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                  int32_t *status, int32_t *stats, int32_t nthreads) {
+  if (!m || !states || N < 0 || ld < N || (method != 0 && method != 1) || !(dt > 0.0) || !(rtol > 0.0) ||
+      !(atol >= 0.0))
+    return ORA_EINVAL;
+  const int n = m->K + 1;
+#ifdef _OPENMP
+  if (nthreads <= 0) nthreads = omp_get_max_threads();
+#else
+  nthreads = 1;
+#endif
+#pragma omp parallel num_threads(nthreads)
+  {
+    double *y = (double *)malloc(sizeof(double) * (size_t)n);
+    double *work = (double *)malloc(sizeof(double) * (2 * (size_t)m->K + (size_t)m->R + 1));
+    chem_ctx ctx;
+    ctx.m = m;
+    ctx.work = work;
+#pragma omp for schedule(dynamic, 16)
+    for (int64_t i = 0; i < N; i++) {
+      for (int c = 0; c < n; c++) y[c] = states[(size_t)c * ld + i];
+      ctx.p = pressure ? pressure[i] : p_uniform;
+      int32_t st[4];
+      int code = (method == 0) ? ora_rkck_generic(chem_rhs_cb, &ctx, n, y, t, t + dt, rtol, atol, st)
+                               : ora_rkc_generic(chem_rhs_cb, &ctx, n, y, t, t + dt, rtol, atol, st);
+      for (int c = 0; c < n; c++) states[(size_t)c * ld + i] = y[c];
+      if (status) status[i] = code;
+      if (stats)
+        for (int q = 0; q < 4; q++) stats[(size_t)q * N + i] = st[q];
+    }
+    free(y);
+    free(work);
+  }
+  return ORA_OK;
+}
+
+int ora_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
