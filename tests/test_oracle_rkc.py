@@ -1,0 +1,188 @@
+"""Pins for the oracle's RKC (section 2.4).  No GPU.
+
+The coefficient generator and the stage recursion are pinned by the closed-form stage polynomial
+a_j + b_j T_j(w0 + w1 z) with Chebyshev values from cosh/sinh formulas evaluated in mpmath (an
+independent route: the oracle uses three-term recurrences), the stability claim by the Chebyshev
+bound, the order by a measured slope, the power method by operators with known spectrum.
+"""
+import mpmath as mp
+import numpy as np
+import pytest
+
+import oracle
+
+mp.mp.dps = 40
+
+
+def _cheb(j, w0):
+    """T_j, T_j', T_j'' at w0 > 1 via theta = arcosh w0 (closed forms, not the recurrence)."""
+    th = mp.acosh(w0)
+    T = mp.cosh(j * th)
+    dT = j * mp.sinh(j * th) / mp.sinh(th)
+    d2T = (j * j * T - w0 * dT) / (w0 * w0 - 1)
+    return T, dT, d2T
+
+
+def _closed_form_coeffs(s):
+    w0 = 1 + mp.mpf(2) / 13 / (s * s)
+    Ts, dTs, d2Ts = _cheb(s, w0)
+    w1 = dTs / d2Ts
+    b = [None] * (s + 1)
+    for j in range(2, s + 1):
+        T, dT, d2T = _cheb(j, w0)
+        b[j] = d2T / dT ** 2
+    b[0] = b[1] = b[2]
+    a = [1 - b[j] * _cheb(j, w0)[0] for j in range(s + 1)]
+    return w0, w1, a, b
+
+
+@pytest.mark.parametrize("s", [2, 3, 4, 5, 7, 10, 20, 50, 101, 200])
+def test_stage_polynomials_closed_form(s):
+    """f = lambda y: w_j / y_n = a_j + b_j T_j(w0 + w1 z) for every stage j >= 2 (Eq. 18-25)."""
+    w0, w1, a, b = _closed_form_coeffs(s)
+    co = oracle.rkc_coeffs(s)
+    assert abs(co["w0"] - float(w0)) < 1e-15 and abs(co["w1"] / float(w1) - 1) < 1e-11
+    beta = float((1 + w0) / w1)
+    for z in (-0.9 * beta, -0.37 * beta, -1.0, -1e-2):
+        lam, h = z / 0.5, 0.5
+        ynew, stages = oracle.rkc_step(lambda t, y: lam * y, 0.0, [1.5], h, s, want_stages=True)
+        for j in range(2, s + 1):
+            x = w0 + w1 * z
+            Tj = mp.cos(j * mp.acos(x)) if abs(x) <= 1 else mp.cosh(j * mp.acosh(x))
+            expect = float(a[j] + b[j] * Tj)
+            assert abs(stages[j - 1, 0] / 1.5 - expect) < 2e-10 * max(1.0, s / 10), (s, j, z)
+        assert ynew[0] == stages[s - 1, 0]
+        # first stage: w_1 = y (1 + b_1 w1 z)  (Eq. 19, 22 with R10 b_1 = b_2)
+        assert abs(stages[0, 0] / 1.5 - float(1 + b[1] * w1 * z)) < 2e-11
+
+
+@pytest.mark.parametrize("s", list(range(2, 41)) + [64, 100, 150, 200])
+def test_chebyshev_stability_bound_and_eq39(s):
+    """|P_s(z)| <= 1 on [-beta(s), 0), > 1 at 1.5 beta (damping makes the growth past beta slow for small s); beta(s) >= (s^2-1)/1.54 so Eq. 39 with
+    truncation keeps dt*sigma inside the stability interval."""
+    co = oracle.rkc_coeffs(s)
+    w0, w1 = co["w0"], co["w1"]
+    a_s, b_s = co["a"][s], co["b"][s]
+    beta = (1 + w0) / w1
+    z = -np.linspace(1e-3 * beta, beta, 20001)
+    P = a_s + b_s * np.cos(s * np.arccos(np.clip(w0 + w1 * z, -1, 1)))
+    inside = np.abs(w0 + w1 * z) <= 1
+    P = np.where(inside, P, a_s + b_s * np.cosh(s * np.arccosh(np.maximum(np.abs(w0 + w1 * z), 1))))
+    assert np.max(np.abs(P)) <= 1.0 + 1e-12
+    assert np.max(np.abs(P[z < -0.05 * beta])) <= a_s + b_s + 1e-12 <= 0.996
+    xb = w0 + w1 * (-1.5 * beta)
+    assert abs(a_s + b_s * (-1) ** s * np.cosh(s * np.arccosh(-xb))) > 1.0
+    assert beta >= (s * s - 1) / 1.54
+    assert abs(beta / ((2.0 / 3.0) * (s * s - 1) * (1 - 2.0 / 15.0 * 2.0 / 13.0)) - 1) < 0.15
+
+
+@pytest.mark.parametrize("s", [2, 3, 5, 20, 80])
+def test_consistency_order2_and_c_identities(s):
+    """P_s(z) = 1 + z + z^2/2 + O(z^3); c_1 = c_2/T_2'(w0) (Eq. 27, which fixes R10); c_j ~ (j^2-1)/(s^2-1)."""
+    co = oracle.rkc_coeffs(s)
+    w0, w1 = co["w0"], co["w1"]
+    errs = []
+    for z in (-1e-2, -5e-3):
+        ynew = oracle.rkc_step(lambda t, y: z * y, 0.0, [1.0], 1.0, s)
+        errs.append((ynew[0] - (1 + z + z * z / 2)) / z ** 3)
+    lead = {2: -1 / 6 + 1 / 6}.get(s)  # P_2 has no z^3 term: (P - 1 - z - z^2/2)/z^3 -> 0
+    if s == 2:
+        assert abs(errs[1]) < 1e-3
+    else:
+        assert abs(errs[0] - errs[1]) < 2e-3 and 0.0 < errs[1] < 1 / 6
+    c = co["c"]
+    if s >= 3:
+        assert abs(c[1] - c[2] / (4 * w0)) < 1e-15          # T_2'(w0) = 4 w0
+    else:
+        assert abs(c[1] - (w1 / w0) / (4 * w0)) < 1e-15      # c_2 formula value w1 T_2''/T_2' = w1/w0
+    assert c[s] == 1.0
+    for j in range(2, s):
+        assert abs(c[j] - (j * j - 1) / (s * s - 1)) < 0.03
+    # mu + nu + (1 - mu - nu) = 1 trivially; check gamt = -a_{j-1} mut (Eq. 23) with R9's a_j
+    for j in range(2, s + 1):
+        assert co["gamt"][j] == -co["a"][j - 1] * co["mut"][j]
+
+
+@pytest.mark.parametrize("s", [2, 5, 20])
+def test_measured_order_2_nonautonomous(s):
+    """y' = lambda (y - cos t) - sin t, y = cos t: global error slope 2 (uses the stage times c_j)."""
+    lam = -5.0
+    f = lambda t, y: lam * (y - np.cos(t)) - np.sin(t)
+    errs = []
+    for n in (20, 40, 80, 160):
+        h = 1.0 / n
+        y = np.array([1.0])
+        for i in range(n):
+            y = oracle.rkc_step(f, i * h, y, h, s)
+        errs.append(abs(y[0] - np.cos(1.0)))
+    slopes = [np.log2(errs[i] / errs[i + 1]) for i in range(3)]
+    assert all(1.85 < q < 2.15 for q in slopes), (slopes, errs)
+
+
+def test_power_method_known_spectrum():
+    """f(y) = A y + c, A symmetric with known eigenvalues: returned value / rho(A) in [1.2*0.99, 1.2*1.0001] (R17/R18)."""
+    rng = np.random.default_rng(5)
+    for n, top in ((4, 1e3), (10, 1e6), (14, 3e7)):
+        Q, _ = np.linalg.qr(rng.standard_normal((n, n)))
+        lam = -np.concatenate([[top], rng.uniform(0.0, 0.5 * top, n - 1)])
+        A = (Q * lam) @ Q.T
+        c = rng.standard_normal(n)
+        y0 = rng.uniform(0.5, 2.0, n)
+        sig, v, nfe, flag = oracle.spectral_radius(lambda t, y: A @ y + c, 0.0, y0)
+        assert flag == 0 and nfe >= 2                      # at least two iterations (f(y) not counted)
+        assert 1.2 * 0.985 <= sig / top <= 1.2 * 1.0001, sig / top
+        # warm start from the saved vector converges in the minimum two iterations, same value
+        sig2, _, nfe2, flag2 = oracle.spectral_radius(lambda t, y: A @ y + c, 0.0, y0, v=v)
+        assert flag2 == 0 and nfe2 == 2 and abs(sig2 / sig - 1) < 0.02
+
+
+def test_power_method_degenerate_inputs():
+    """f = 0 everywhere: sigma = 0, converged; y = 0 and v = 0 branch does not divide by zero."""
+    sig, v, nfe, flag = oracle.spectral_radius(lambda t, y: 0.0 * y, 0.0, [0.0, 0.0, 0.0])
+    assert sig == 0.0 and flag == 0 and np.all(np.isfinite(v))
+    sig, v, nfe, flag = oracle.spectral_radius(lambda t, y: -3.0 * y, 0.0, [0.0, 0.0])
+    assert abs(sig / 3.0 - 1.2) < 1e-6 and flag == 0
+
+
+def test_driver_linear_accuracy_and_stage_growth():
+    """Stiff linear problem y' = A y: result within ~tolerance-scaled error of expm; stage count grows with
+    dt*sigma as Eq. 39 says; evaluations = accepted/rejected bookkeeping is consistent."""
+    lam = np.array([-1.0, -50.0, -2.0e4])
+    f = lambda t, y: lam * y
+    for rtol, bound in ((1e-3, 2e-2), (1e-5, 5e-4)):
+        y, status, st = oracle.rkc_generic(f, [1.0, 1.0, 1.0], 0.0, 1.0, rtol, 1e-10)
+        assert status == 0
+        assert np.max(np.abs(y - np.exp(lam))) < bound
+        assert st[3] >= 10                                  # needs many stages: dt*sigma >> 1 late in the interval
+        assert st[0] > st[1] + st[2]
+    # nonstiff: s stays 2 and the number of evaluations is 2 per attempt + start-up
+    y, status, st = oracle.rkc_generic(lambda t, y: -y, [1.0], 0.0, 1.0, 1e-6, 1e-12)
+    assert status == 0 and st[3] == 2
+    assert abs(y[0] - np.exp(-1.0)) < 2e-5
+
+
+def test_driver_step_count_matches_estimator_model():
+    """y' = -y with s = 2: Eq. 30 gives est = 0.2 |z|^3 |y| / (rtol |y|); with the controller's target
+    0.8^3 the step count over [0,1] is about (0.2/(0.512 rtol))^(1/3).  A dropped or mis-signed term in
+    Eq. 30 or a wrong exponent in Eq. 33-35 changes this by large factors."""
+    for rtol in (1e-6, 1e-8):
+        y, status, st = oracle.rkc_generic(lambda t, y: -y, [1.0], 0.0, 1.0, rtol, 1e-300)
+        predicted = (0.2 / (0.512 * rtol)) ** (1.0 / 3.0)
+        assert status == 0 and st[2] <= 2
+        assert 0.85 * predicted < st[1] < 1.35 * predicted, (st, predicted)
+
+
+def test_driver_tolerance_proportionality():
+    f = lambda t, y: np.array([y[1], -y[0]])
+    errs = []
+    for tol in (1e-4, 1e-6, 1e-8):
+        y, status, st = oracle.rkc_generic(f, [1.0, 0.0], 0.0, 3.0, tol, tol * 1e-3)
+        assert status == 0
+        errs.append(np.hypot(y[0] - np.cos(3.0), y[1] + np.sin(3.0)))
+    slope = np.log10(errs[0] / errs[-1]) / 4.0
+    assert 0.55 < slope < 1.2, (errs, slope)               # global error ~ tol^(2/3) .. tol for a 2nd-order pair
+
+
+def test_driver_nonfinite_fails_cleanly():
+    y, status, st = oracle.rkc_generic(lambda t, y: np.array([np.nan]), [1.0], 0.0, 1.0, 1e-6, 1e-12)
+    assert status in (3, 4) and y[0] == 1.0 and st[1] == 0
