@@ -1,0 +1,150 @@
+/*
+ * ckb.h -- C ABI of the batched chemical-kinetics integrator for B200 (sm_100a, FP64).
+ *
+ * The library advances N independent constant-pressure chemistry ODE systems
+ *     y = {T, Y_1 .. Y_K}
+ * over one global flow step dt by adaptive explicit integration, statelessly ("take as input
+ * initial conditions and a global time step, performing internal sub-stepping as necessary"):
+ *     method 0 : RKCK, 5th-order Runge-Kutta-Cash-Karp with embedded 4th-order error estimate
+ *                (Eq. 7-17, Table 1)
+ *     method 1 : RKC, stabilised 2nd-order Runge-Kutta-Chebyshev (Eq. 18-39) with the
+ *                nonlinear power-method spectral-radius estimate and per-step stage count
+ * Source term f(y): Eq. 2-6: Arrhenius rate coefficients (Eq. 5), third-body concentrations
+ * (P:80), mass-action rates of progress (Eq. 4), net production rates (Eq. 3), NASA-polynomial cp / h
+ * for the temperature equation (Eq. 6).  Readings of the paper where it is silent: DESIGN.md section 4.
+ *
+ * Every step of that path runs in hand-written CUDA kernels; there is no CPU fallback.  All entry
+ * points return CKB_OK (0) or a negative error code; ckb_strerror() gives the text.
+ *
+ * Units (cgs): mol, cm, s, K; activation energy in cal/mol; molecular weight in g/mol; pressure in
+ * dyn/cm^2.
+ */
+#ifndef CKB_H_
+#define CKB_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CKB_OK 0
+#define CKB_EINVAL (-1)       /* null pointer, bad shape, inconsistent CSR, index out of range       */
+#define CKB_ENOMEM (-2)       /* host or device allocation failed                                    */
+#define CKB_ECUDA (-3)        /* a CUDA runtime call failed; text via ckb_last_cuda_error()          */
+#define CKB_EUNSUPPORTED (-4) /* mechanism outside the packed format's limits (see ckb_mech_load)    */
+
+#define CKB_METHOD_RKCK 0
+#define CKB_METHOD_RKC 1
+
+/* variant: how ODE systems are mapped onto lanes */
+#define CKB_VARIANT_AUTO 0    /* thread-per-ODE for K+1 <= 16, warp-per-ODE above                     */
+#define CKB_VARIANT_THREAD 1  /* one thread integrates one system (the paper's mapping)        */
+#define CKB_VARIANT_WARP 2    /* one warp integrates one system; species and reactions over lanes     */
+#define CKB_VARIANT_SUB8 3    /* 8 lanes per system (4 systems per warp)                              */
+#define CKB_VARIANT_SUB16 4   /* 16 lanes per system (2 systems per warp)                             */
+
+/* per-system status codes written to status[] */
+#define CKB_ST_OK 0
+#define CKB_ST_MAXSTEPS 1     /* more than 10^6 step attempts                                         */
+#define CKB_ST_UNDERFLOW 2    /* step size fell below 10 u max(|t|,|t+dt|)                            */
+#define CKB_ST_NONFINITE 3    /* as 2, after a non-finite trial state                                 */
+#define CKB_ST_SIGMA 4        /* RKC: power method did not converge in 50 iterations (result kept)    */
+
+/*
+ * Mechanism description: plain HOST arrays, caller-owned, copied during ckb_mech_load.
+ * Irreversible reactions only (every reversible reaction is entered as two irreversible ones).
+ */
+typedef struct {
+  int32_t n_species;           /* K, 1..254                                                         */
+  int32_t n_reactions;         /* R irreversible reactions                                          */
+  const double *mol_weight;    /* [K]    W_k, g/mol                                                 */
+  const double *nasa;          /* [K][7] a1..a7 of one temperature range (a7 unused on this path)   */
+  const double *arr_A;         /* [R]    pre-exponential A_j (Eq. 5), cgs, > 0                      */
+  const double *arr_beta;      /* [R]    temperature exponent                                       */
+  const double *arr_E;         /* [R]    activation energy, cal/mol                                 */
+  const int32_t *reac_ptr;     /* [R+1]  CSR over reactant entries                                  */
+  const int32_t *reac_species; /* [nnz]  species index 0..K-1                                       */
+  const int32_t *reac_nu;      /* [nnz]  nu'_kj  >= 1 (integer reaction order = stoichiometry)      */
+  const int32_t *prod_ptr;     /* [R+1]  CSR over product entries                                   */
+  const int32_t *prod_species; /* [nnz]                                                             */
+  const int32_t *prod_nu;      /* [nnz]  nu''_kj >= 1                                               */
+  int32_t n_third_body;        /* R3 reactions that carry a third body +M                    */
+  const int32_t *tb_reaction;  /* [R3]   reaction index                                             */
+  const int32_t *tb_ptr;       /* [R3+1] CSR over listed (non-unity) efficiencies                   */
+  const int32_t *tb_species;   /* [nnz]                                                             */
+  const double *tb_eff;        /* [nnz]  alpha_jk; every species not listed has alpha = 1           */
+} ckb_mech_desc;
+
+typedef struct ckb_mech ckb_mech; /* opaque; owns the packed tables in device memory */
+
+/*
+ * ckb_mech_load: validate `d`, pack it into the device tables of DESIGN.md section 6.1 (forward /
+ * reverse reactions over the same species are fused into one slot; species-major gather lists for
+ * Eq. 3; third-body efficiency sets), upload them to the current CUDA device, and return a handle in
+ * *out (library-owned; release with ckb_mech_free).  Synchronous.
+ * Limits (CKB_EUNSUPPORTED): K <= 254; at most 3 molecules (sum of nu) on either side of a reaction;
+ * at most 65534 fused reaction slots; at most 65534 distinct third-body efficiency sets.
+ */
+int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out);
+void ckb_mech_free(ckb_mech *m);
+
+/* number of species / reactions / fused reaction slots / algorithmic flops per f(y) */
+int ckb_mech_info(const ckb_mech *m, int32_t *n_species, int32_t *n_reactions, int32_t *n_slots,
+                  double *flops_per_rhs);
+
+/*
+ * ckb_integrate: advance every system i in [0, N) from t to t+dt, in place.
+ *   states   DEVICE  SoA, row-major [(K+1)][ld]: row 0 = T (K), rows 1..K = mass fractions Y_k;
+ *                    element (c, i) at states[c*ld + i]; ld >= N.  Caller-owned (e.g. a torch tensor).
+ *   pressure DEVICE  [N] dyn/cm^2, or NULL to use p_uniform for every system (constant over the call).
+ *   t, dt            f is autonomous; t only anchors the sub-step clock.  dt > 0.
+ *   rtol, atol       tolerances: RKCK Eq. 16 with eps = rtol, eps*delta = atol; RKC Eq. 32.
+ *   method, variant  CKB_METHOD_*, CKB_VARIANT_*.
+ *   status   DEVICE  [N] int32 or NULL: CKB_ST_* per system.  A failed system holds its last accepted state.
+ *   stats    DEVICE  [4][N] int32 or NULL: f(y) evaluations, accepted steps, rejected steps, largest
+ *                    RKC stage count (0 for RKCK).
+ *   stream           cudaStream_t as void* (NULL = legacy default stream).
+ * Asynchronous on `stream`: never synchronises, allocates nothing.  Stateless between calls.
+ * N == 0 is a no-op.  Errors: CKB_EINVAL for bad arguments, CKB_EUNSUPPORTED if the variant cannot hold
+ * the mechanism (thread-per-ODE needs K+1 <= 16; lane-distributed variants need K+1 <= 4*lanes...),
+ * CKB_ECUDA if the launch failed.
+ */
+int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, double p_uniform,
+                  int64_t N, int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                  int32_t variant, int32_t *status, int32_t *stats, void *stream);
+
+/*
+ * ckb_integrate_host: the same call with HOST buffers (states, pressure, status, stats as above but in
+ * host memory, pinned or pageable).  Copies host->device, integrates, copies device->host on `stream`
+ * and synchronises it before returning -- the per-global-step protocol the paper timed.  Uses
+ * a grow-only device workspace owned by the handle (not thread-safe per handle).
+ */
+int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                       int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                       int32_t variant, int32_t *status, int32_t *stats, void *stream);
+
+/*
+ * ckb_rhs: evaluate the source term f(y) (Eq. 2-6) once for each of N systems, without integrating;
+ * dydt DEVICE [(K+1)][ld] receives (dT/dt, dY_k/dt).  Same layout and mapping variants as
+ * ckb_integrate.  Used by the parity tests of the source term and by the roofline measurement.
+ * `repeat` >= 1 evaluates f that many times per system inside the kernel (timing aid; result unchanged).
+ */
+int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, double p_uniform, int64_t N,
+            int64_t ld, double *dydt, int32_t variant, int32_t repeat, void *stream);
+
+/*
+ * ckb_fp64_probe: roofline denominator.  Runs a register-resident kernel of independent DFMA chains on
+ * every SM (iters FMAs per chain) on `stream`, times it with CUDA events and returns the achieved
+ * FP64 rate in FLOP/s (2 per FMA) in *flops_per_s.  kind 0 = DFMA chains; kind 1 = exp(double) calls
+ * (returns exp evaluations per second).  Synchronises `stream`.
+ */
+int ckb_fp64_probe(int32_t kind, int64_t iters, double *per_second, void *stream);
+
+const char *ckb_strerror(int code);
+const char *ckb_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CKB_H_ */

@@ -1,0 +1,211 @@
+"""Thin ctypes binding over the C ABI of include/ckb.h (libckb.so).  Argument marshalling only: every
+step of the path (source term, RKCK, RKC, spectral radius, controllers) runs in the CUDA kernels.
+
+PyTorch is used for device memory and streams only.  There is no CPU fallback: if libckb.so is missing
+the import of the entry points fails loudly (build it with ``python -m paper_1309_2710_b200.build``).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libckb.so")
+
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
+METHODS = {"rkck": 0, "rkc": 1}
+VARIANTS = {"auto": 0, "thread": 1, "warp": 2, "sub8": 3, "sub16": 4}
+ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
+
+# every symbol include/ckb.h declares
+EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "ckb_integrate_host",
+           "ckb_rhs", "ckb_fp64_probe", "ckb_strerror", "ckb_last_cuda_error")
+
+
+class CkbError(RuntimeError):
+    def __init__(self, code, where):
+        L = lib()
+        msg = L.ckb_strerror(code).decode()
+        if code == ECUDA:
+            msg += ": " + L.ckb_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} ({code})")
+        self.code = code
+
+
+class _Desc(C.Structure):
+    _fields_ = [
+        ("n_species", C.c_int32), ("n_reactions", C.c_int32),
+        ("mol_weight", C.c_void_p), ("nasa", C.c_void_p), ("arr_A", C.c_void_p),
+        ("arr_beta", C.c_void_p), ("arr_E", C.c_void_p),
+        ("reac_ptr", C.c_void_p), ("reac_species", C.c_void_p), ("reac_nu", C.c_void_p),
+        ("prod_ptr", C.c_void_p), ("prod_species", C.c_void_p), ("prod_nu", C.c_void_p),
+        ("n_third_body", C.c_int32),
+        ("tb_reaction", C.c_void_p), ("tb_ptr", C.c_void_p), ("tb_species", C.c_void_p),
+        ("tb_eff", C.c_void_p),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    """Load libckb.so and declare the prototypes of include/ckb.h."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build the CUDA library with "
+                          "`python -m paper_1309_2710_b200.build` (there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    L.ckb_mech_load.argtypes = [C.POINTER(_Desc), C.POINTER(vp)]
+    L.ckb_mech_load.restype = C.c_int
+    L.ckb_mech_free.argtypes = [vp]
+    L.ckb_mech_free.restype = None
+    L.ckb_mech_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
+    L.ckb_mech_info.restype = C.c_int
+    integ = [vp, vp, vp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, i32, vp, vp, vp]
+    L.ckb_integrate.argtypes = integ
+    L.ckb_integrate.restype = C.c_int
+    L.ckb_integrate_host.argtypes = integ
+    L.ckb_integrate_host.restype = C.c_int
+    L.ckb_rhs.argtypes = [vp, vp, vp, dbl, i64, i64, vp, i32, i32, vp]
+    L.ckb_rhs.restype = C.c_int
+    L.ckb_fp64_probe.argtypes = [i32, i64, C.POINTER(dbl), vp]
+    L.ckb_fp64_probe.restype = C.c_int
+    L.ckb_strerror.argtypes = [C.c_int]
+    L.ckb_strerror.restype = C.c_char_p
+    L.ckb_last_cuda_error.argtypes = []
+    L.ckb_last_cuda_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc, where):
+    if rc != OK:
+        raise CkbError(rc, where)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dev_ptr(t, dtype, where):
+    import torch
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{where}: expected a contiguous CUDA tensor of {dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+class Mech:
+    """ckb_mech handle.  `mech` is any object that carries the arrays of ckb_mech_desc as attributes."""
+
+    def __init__(self, mech):
+        keep = dict(
+            mol_weight=_f64(mech.mol_weight), nasa=_f64(mech.nasa), arr_A=_f64(mech.arr_A),
+            arr_beta=_f64(mech.arr_beta), arr_E=_f64(mech.arr_E),
+            reac_ptr=_i32(mech.reac_ptr), reac_species=_i32(mech.reac_species), reac_nu=_i32(mech.reac_nu),
+            prod_ptr=_i32(mech.prod_ptr), prod_species=_i32(mech.prod_species), prod_nu=_i32(mech.prod_nu),
+            tb_reaction=_i32(mech.tb_reaction), tb_ptr=_i32(mech.tb_ptr), tb_species=_i32(mech.tb_species),
+            tb_eff=_f64(mech.tb_eff))
+        d = _Desc()
+        d.n_species = int(keep["mol_weight"].shape[0])
+        d.n_reactions = int(keep["arr_A"].shape[0])
+        d.n_third_body = int(keep["tb_reaction"].shape[0])
+        for k, v in keep.items():
+            setattr(d, k, v.ctypes.data)
+        self._h = C.c_void_p()
+        _check(lib().ckb_mech_load(C.byref(d), C.byref(self._h)), "ckb_mech_load")
+        ks, rs, ns, fl = C.c_int32(), C.c_int32(), C.c_int32(), C.c_double()
+        _check(lib().ckb_mech_info(self._h, C.byref(ks), C.byref(rs), C.byref(ns), C.byref(fl)), "ckb_mech_info")
+        self.K, self.R, self.n_slots, self.flops_per_rhs = ks.value, rs.value, ns.value, fl.value
+
+    def close(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.ckb_mech_free(self._h)
+            self._h = None
+
+    __del__ = close
+
+
+def mech_load(mech) -> Mech:
+    return Mech(mech)
+
+
+def integrate(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None, pressure=None,
+              variant="auto", status=None, stats=None, stream=None):
+    """ckb_integrate: advance states (CUDA float64 tensor [(K+1)][ld], in place) over one global step dt.
+
+    p: uniform pressure (dyn/cm^2) or pressure: CUDA tensor [N].  status: int32 CUDA [N]; stats: int32 CUDA [4][N].
+    Asynchronous on the current (or given) torch stream.
+    """
+    import torch
+    if states.dim() != 2 or states.shape[0] != m.K + 1:
+        raise ValueError("states must be [(K+1)][ld]")
+    ld = int(states.shape[1])
+    N = ld if N is None else int(N)
+    rc = lib().ckb_integrate(
+        m._h, _dev_ptr(states, torch.float64, "states"), _dev_ptr(pressure, torch.float64, "pressure"),
+        float(0.0 if p is None else p), N, ld, float(t), float(dt), float(rtol), float(atol),
+        int(METHODS.get(method, method)), int(VARIANTS.get(variant, variant)),
+        _dev_ptr(status, torch.int32, "status"), _dev_ptr(stats, torch.int32, "stats"), _stream_ptr(stream))
+    _check(rc, "ckb_integrate")
+    return states
+
+
+def integrate_host(m: Mech, states, dt, rtol, atol, method, *, t=0.0, p=None, pressure=None, variant="auto",
+                   status=None, stats=None, stream=None):
+    """ckb_integrate_host: the same call on HOST buffers (numpy float64 [(K+1)][N] C-contiguous, or a pinned
+    CPU torch tensor), host<->device copies inside the call; returns after the stream has been synchronised."""
+    def hp(a, dtype):
+        if a is None:
+            return None
+        if hasattr(a, "data_ptr"):
+            return C.c_void_p(a.data_ptr())
+        assert a.dtype == dtype and a.flags["C_CONTIGUOUS"]
+        return C.c_void_p(a.ctypes.data)
+    n, N = int(states.shape[0]), int(states.shape[1])
+    if n != m.K + 1:
+        raise ValueError("states must be [(K+1)][N]")
+    rc = lib().ckb_integrate_host(
+        m._h, hp(states, np.float64), hp(pressure, np.float64), float(0.0 if p is None else p), N, N, float(t),
+        float(dt), float(rtol), float(atol), int(METHODS.get(method, method)), int(VARIANTS.get(variant, variant)),
+        hp(status, np.int32), hp(stats, np.int32), _stream_ptr(stream))
+    _check(rc, "ckb_integrate_host")
+    return states
+
+
+def rhs(m: Mech, states, *, p=None, pressure=None, variant="auto", repeat=1, out=None, N=None, stream=None):
+    """ckb_rhs: f(y) for every system; returns dydt [(K+1)][ld] (CUDA float64)."""
+    import torch
+    ld = int(states.shape[1])
+    N = ld if N is None else int(N)
+    if out is None:
+        out = torch.empty_like(states)
+    rc = lib().ckb_rhs(m._h, _dev_ptr(states, torch.float64, "states"), _dev_ptr(pressure, torch.float64, "pressure"),
+                       float(0.0 if p is None else p), N, ld, _dev_ptr(out, torch.float64, "out"),
+                       int(VARIANTS.get(variant, variant)), int(repeat), _stream_ptr(stream))
+    _check(rc, "ckb_rhs")
+    return out
+
+
+def fp64_probe(kind="dfma", iters=1 << 16, stream=None) -> float:
+    """ckb_fp64_probe: measured FP64 FLOP/s (kind='dfma') or exp(double)/s (kind='exp') of this device."""
+    v = C.c_double()
+    _check(lib().ckb_fp64_probe({"dfma": 0, "exp": 1}[kind], int(iters), C.byref(v), _stream_ptr(stream)),
+           "ckb_fp64_probe")
+    return v.value

@@ -1,0 +1,80 @@
+"""Build libckb.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+    python -m paper_1309_2710_b200.build [--force] [--verbose]
+
+One object per kernel instantiation (csrc/ckb_inst.cu compiled with -DCKB_L/-DCKB_NV, the list is read
+from CKB_FOR_THREAD / CKB_FOR_GROUP in csrc/ckb_host.h), compiled in parallel, then linked together
+with the API and probe objects.  nvcc cross-compiles without a GPU.
+"""
+from __future__ import annotations
+
+import hashlib
+import os
+import re
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
+LIB = os.path.join(HERE, "libckb.so")
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", *ARCH]
+
+
+def instantiations():
+    txt = open(os.path.join(CSRC, "ckb_host.h")).read()
+    out = []
+    for name in ("CKB_FOR_THREAD", "CKB_FOR_GROUP"):
+        line = re.search(r"#define %s\(X\)(.*)" % name, txt).group(1)
+        out += [(int(a), int(b)) for a, b in re.findall(r"X\((\d+),\s*(\d+)\)", line)]
+    return out
+
+
+def _digest(extra: str) -> str:
+    h = hashlib.sha256(extra.encode())
+    for root in (CSRC, os.path.join(HERE, "..", "include")):
+        for fn in sorted(os.listdir(root)):
+            if fn.endswith((".cu", ".cuh", ".h")):
+                h.update(fn.encode())
+                h.update(open(os.path.join(root, fn), "rb").read())
+    return h.hexdigest()
+
+
+def _run(cmd, verbose):
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("build failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    if verbose:
+        sys.stderr.write(r.stdout + r.stderr)
+
+
+def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> str:
+    os.makedirs(OBJ, exist_ok=True)
+    flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else [])
+    stamp = os.path.join(OBJ, "stamp")
+    digest = _digest(" ".join(flags))
+    if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
+        return LIB
+    jobs = []
+    for src in ("ckb_api.cu", "ckb_probe.cu"):
+        obj = os.path.join(OBJ, src.replace(".cu", ".o"))
+        jobs.append((obj, [NVCC, *flags, "-c", os.path.join(CSRC, src), "-o", obj]))
+    for (L, NV) in instantiations():
+        obj = os.path.join(OBJ, f"ckb_inst_L{L}_NV{NV}.o")
+        jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", "-c",
+                           os.path.join(CSRC, "ckb_inst.cu"), "-o", obj]))
+    with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
+        list(ex.map(lambda j: _run(j[1], verbose or ptxas_v), jobs))
+    tmp = LIB + f".tmp{os.getpid()}"
+    _run([NVCC, "-shared", *ARCH, "-o", tmp, *[j[0] for j in jobs]], verbose)
+    os.replace(tmp, LIB)
+    with open(stamp, "w") as fh:
+        fh.write(digest)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, ptxas_v="--ptxas-v" in sys.argv))

@@ -1,0 +1,59 @@
+/*
+ * ckb_host.h -- host-side types shared by ckb_api.cu (C ABI, packing, dispatch) and ckb_inst.cu (one
+ * object per (lanes-per-system, slots-per-lane) instantiation of the kernels).
+ */
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/ckb.h"
+#include "ckb_tables.h"
+
+namespace ckb_host {
+int cuda_fail(cudaError_t e, const char *what);
+}
+#define CK(call)                                                  \
+  do {                                                            \
+    cudaError_t e_ = (call);                                      \
+    if (e_ != cudaSuccess) return ckb_host::cuda_fail(e_, #call); \
+  } while (0)
+
+struct ckb_mech {
+  ckb::DevMech dm{};
+  std::vector<unsigned long long> blob; /* host copy of the packed tables */
+  unsigned long long *d_blob = nullptr;
+  int R = 0;
+  double flops_per_rhs = 0.0;
+  /* grow-only device workspace of ckb_integrate_host */
+  double *ws_states = nullptr, *ws_pressure = nullptr;
+  int32_t *ws_status = nullptr, *ws_stats = nullptr;
+  size_t ws_states_cap = 0, ws_n_cap = 0;
+};
+
+
+namespace ckb_host {
+
+struct IntegrateArgs {
+  double *states; const double *pressure; double p_uniform; long long N, ld;
+  double t, dt, rtol, atol; int *status, *stats; cudaStream_t stream;
+};
+struct RhsArgs {
+  const double *states; const double *pressure; double p_uniform; long long N, ld; double *dydt; int repeat;
+  cudaStream_t stream;
+};
+
+/* the instantiation list: (lanes per system L, register slots per lane NV); a system needs K+1 <= L*NV */
+#define CKB_FOR_THREAD(X) X(1, 4) X(1, 10) X(1, 14) X(1, 16)
+#define CKB_FOR_GROUP(X) X(8, 7) X(8, 14) X(16, 4) X(16, 7) X(32, 1) X(32, 2) X(32, 4)
+
+#define CKB_DECL(L_, NV_)                                                                         \
+  int integrate_L##L_##_NV##NV_(const ckb_mech *m, int method, const IntegrateArgs &a);           \
+  int rhs_L##L_##_NV##NV_(const ckb_mech *m, const RhsArgs &a);
+CKB_FOR_THREAD(CKB_DECL)
+CKB_FOR_GROUP(CKB_DECL)
+#undef CKB_DECL
+
+}  // namespace ckb_host

@@ -1,0 +1,86 @@
+/*
+ * ckb_inst.cu -- one object per kernel instantiation: compile with -DCKB_L=<lanes per system>
+ * -DCKB_NV=<register slots per lane>.  L = 1 takes the packed mechanism as a kernel parameter
+ * (ParamTab), L > 1 reads it from the device blob (GlobalTab).
+ */
+#include <cstring>
+
+#include "ckb_device.cuh"
+#include "ckb_host.h"
+
+#ifndef CKB_L
+#error "compile with -DCKB_L=.. -DCKB_NV=.."
+#endif
+
+#define CKB_CAT_(a, b, c, d) a##b##c##d
+#define CKB_CAT(a, b, c, d) CKB_CAT_(a, b, c, d)
+
+namespace ckb_host {
+
+namespace {
+
+constexpr int L = CKB_L, NV = CKB_NV;
+#if CKB_L == 1
+typedef ckb::ParamTab Tab;
+#else
+typedef ckb::GlobalTab Tab;
+#endif
+
+size_t smem_bytes(const ckb_mech *m) {
+  const int G = 32 / L;
+  return (size_t)(m->dm.K + 1 + m->dm.NTB + 1 + m->dm.NS) * G * (CKB_BLOCK / 32) * sizeof(double);
+}
+
+template <class KERN>
+int prep(KERN kern, size_t smem) {
+  if (smem > 227 * 1024) return CKB_EUNSUPPORTED;
+  if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  return CKB_OK;
+}
+
+void make_tab(const ckb_mech *m, ckb::ParamTab &t) { std::memcpy(t.w, m->blob.data(), m->blob.size() * 8); }
+void make_tab(const ckb_mech *m, ckb::GlobalTab &t) { t.p = m->d_blob; }
+
+long long n_blocks(long long N) {
+  const long long per_block = (long long)(CKB_BLOCK / 32) * (32 / L);
+  return (N + per_block - 1) / per_block;
+}
+
+template <int METHOD>
+int launch(const ckb_mech *m, const IntegrateArgs &a) {
+  auto kern = ckb::integrate_kernel<L, NV, Tab, METHOD>;
+  const size_t smem = smem_bytes(m);
+  int rc = prep(kern, smem);
+  if (rc) return rc;
+  const long long blocks = n_blocks(a.N);
+  if (blocks > 2147483647LL) return CKB_EINVAL;
+  Tab tab;
+  make_tab(m, tab);
+  kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(m->dm, tab, a.states, a.pressure, a.p_uniform, a.N, a.ld,
+                                                       a.t, a.dt, a.rtol, a.atol, a.status, a.stats);
+  CK(cudaGetLastError());
+  return CKB_OK;
+}
+
+}  // namespace
+
+int CKB_CAT(integrate_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, int method, const IntegrateArgs &a) {
+  return method == 0 ? launch<0>(m, a) : launch<1>(m, a);
+}
+
+int CKB_CAT(rhs_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const RhsArgs &a) {
+  auto kern = ckb::rhs_kernel<L, NV, Tab>;
+  const size_t smem = smem_bytes(m);
+  int rc = prep(kern, smem);
+  if (rc) return rc;
+  const long long blocks = n_blocks(a.N);
+  if (blocks > 2147483647LL) return CKB_EINVAL;
+  Tab tab;
+  make_tab(m, tab);
+  kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(m->dm, tab, a.states, a.pressure, a.p_uniform, a.N, a.ld,
+                                                       a.dydt, a.repeat);
+  CK(cudaGetLastError());
+  return CKB_OK;
+}
+
+}  // namespace ckb_host

@@ -1,0 +1,92 @@
+"""The C-ABI library builds, loads and exports every symbol include/ckb.h declares; argument checks that
+need no GPU.  (No compute calls here: those are the -m gpu parity tests.)"""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1309_2710_b200 import binding, build, synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    build.build()
+    return binding.lib()
+
+
+def test_header_symbols_exported(L):
+    hdr = open(os.path.join(ROOT, "include", "ckb.h")).read()
+    declared = set(re.findall(r"\b(ckb_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert getattr(L, name) is not None
+
+
+def test_strerror(L):
+    assert L.ckb_strerror(0) == b"ok"
+    for code in (-1, -2, -3, -4):
+        assert len(L.ckb_strerror(code)) > 3
+    assert b"unknown" in L.ckb_strerror(-99)
+
+
+def test_instantiation_list_consistent():
+    inst = build.instantiations()
+    assert (1, 10) in inst and (1, 14) in inst and (32, 2) in inst and (32, 4) in inst
+    api = open(os.path.join(ROOT, "paper_1309_2710_b200", "csrc", "ckb_api.cu")).read()
+    for L_, name in ((1, "nv1"), (8, "nv8"), (16, "nv16"), (32, "nv32")):
+        lst = re.search(r"static const int %s\[\] = \{([^}]*)\}" % name, api).group(1)
+        assert [int(x) for x in lst.split(",")] == [nv for (l, nv) in inst if l == L_]
+
+
+def _load(mech):
+    d = binding._Desc()
+    keep = {}
+    for k in ("mol_weight", "nasa", "arr_A", "arr_beta", "arr_E", "tb_eff"):
+        keep[k] = np.ascontiguousarray(getattr(mech, k), dtype=np.float64)
+    for k in ("reac_ptr", "reac_species", "reac_nu", "prod_ptr", "prod_species", "prod_nu", "tb_reaction",
+              "tb_ptr", "tb_species"):
+        keep[k] = np.ascontiguousarray(getattr(mech, k), dtype=np.int32)
+    d.n_species, d.n_reactions, d.n_third_body = len(keep["mol_weight"]), len(keep["arr_A"]), len(keep["tb_reaction"])
+    for k, v in keep.items():
+        setattr(d, k, v.ctypes.data)
+    h = C.c_void_p()
+    rc = binding.lib().ckb_mech_load(C.byref(d), C.byref(h))
+    return rc, h, keep
+
+
+def test_mech_load_rejects_bad_input(L):
+    """Validation happens before any CUDA call, so these return codes are the same with or without a GPU."""
+    assert L.ckb_mech_load(None, None) == binding.EINVAL
+    m = synth.toy_mechanism(2, [({0: 1}, {1: 1}, 1.0, 0.0, 0.0)])
+    m.reac_species = np.array([5], dtype=np.int32)             # species index out of range
+    assert _load(m)[0] == binding.EINVAL
+    m = synth.toy_mechanism(2, [({0: 1}, {1: 1}, -1.0, 0.0, 0.0)])   # negative A
+    assert _load(m)[0] == binding.EINVAL
+    m = synth.toy_mechanism(2, [({0: 4}, {1: 4}, 1.0, 0.0, 0.0)])    # 4 molecules on a side
+    assert _load(m)[0] == binding.EUNSUPPORTED
+    m = synth.toy_mechanism(2, [({0: 1}, {1: 1}, 1.0, 0.0, 0.0)], W=[1.0, -2.0])
+    assert _load(m)[0] == binding.EINVAL
+    m = synth.toy_mechanism(2, [({0: 1}, {1: 1}, 1.0, 0.0, 0.0)], third_body={3: {0: 2.0}})  # bad reaction index
+    assert _load(m)[0] == binding.EINVAL
+
+
+def test_integrate_argument_errors_without_handle(L):
+    assert L.ckb_integrate(None, None, None, 1e6, 0, 0, 0.0, 1e-6, 1e-8, 1e-12, 0, 0, None, None, None) == binding.EINVAL
+    assert L.ckb_rhs(None, None, None, 1e6, 0, 0, None, 0, 1, None) == binding.EINVAL
+    v = C.c_double()
+    assert L.ckb_fp64_probe(7, 10, C.byref(v), None) == binding.EINVAL
+
+
+def test_product_path_does_not_import_oracle():
+    """The binding, the generator and bench's product arm never touch oracle/ (no CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_1309_2710_b200")
+    for fn in os.listdir(pkg):
+        if fn.endswith(".py"):
+            src = open(os.path.join(pkg, fn)).read()
+            assert not re.search(r"^\s*(import|from)\s+oracle", src, re.M), fn
+    for fn in os.listdir(os.path.join(pkg, "csrc")):
+        assert "oracle" not in open(os.path.join(pkg, "csrc", fn)).read().replace("shared with oracle/", ""), fn

@@ -1,0 +1,187 @@
+"""GPU-vs-oracle parity through the C ABI.
+
+Bar (BASELINE.json north_star): per-component max relative error <= 1e-6 on Y_k > 1e-12 and <= 1e-8 on T,
+at rtol = 1e-8, atol = 1e-12.  The integrators are adaptive, so parity is decision-for-decision: the bound
+is asserted on every system whose controller took the same decisions as the oracle's (identical stats:
+f(y) evaluations, accepted, rejected, largest stage count).  A system whose decision flipped on a
+round-off-sized difference (expected O(1e-8) per decision) must be rare and must still agree with the
+oracle to the integrator's own tolerance.
+"""
+import numpy as np
+import pytest
+
+from paper_1309_2710_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+RTOL, ATOL = 1e-8, 1e-12
+TOL_Y, TOL_T, Y_CUT = 1e-6, 1e-8, 1e-12
+
+
+def _run_gpu(mech, states, p, dt, method, variant="auto", ld=None, pressure=None):
+    import torch
+    from paper_1309_2710_b200 import binding
+    m = binding.mech_load(mech)
+    n, N = states.shape
+    ld = N if ld is None else ld
+    buf = torch.full((n, ld), float("nan"), dtype=torch.float64, device="cuda")
+    buf[:, :N] = torch.from_numpy(states).cuda()
+    status = torch.full((N,), -7, dtype=torch.int32, device="cuda")
+    stats = torch.full((4, N), -7, dtype=torch.int32, device="cuda")
+    pr = None if pressure is None else torch.from_numpy(pressure).cuda()
+    binding.integrate(m, buf, dt, RTOL, ATOL, method, N=N, p=p, pressure=pr, variant=variant,
+                      status=status, stats=stats)
+    torch.cuda.synchronize()
+    out = buf.cpu().numpy()
+    if ld > N:
+        assert np.isnan(out[:, N:]).all()          # padding columns untouched
+    m.close()
+    return out[:, :N].copy(), status.cpu().numpy(), stats.cpu().numpy()
+
+
+def _compare(gpu, ora, max_flip_frac=2e-3):
+    (yg, sg, tg), (yo, so, to) = gpu, ora
+    N = yg.shape[1]
+    assert np.isfinite(yg).all()
+    same = (tg == to).all(axis=0) & (sg == so)
+    relT = np.abs(yg[0] - yo[0]) / np.abs(yo[0])
+    Yg, Yo = yg[1:], yo[1:]
+    big = Yo > Y_CUT
+    relY = np.where(big, np.abs(Yg - Yo) / np.where(big, Yo, 1.0), 0.0).max(axis=0)
+    assert relT[same].max(initial=0.0) <= TOL_T, f"T parity {relT[same].max():.3e}"
+    assert relY[same].max(initial=0.0) <= TOL_Y, f"Y parity {relY[same].max():.3e}"
+    n_flip = int((~same).sum())
+    assert n_flip <= max(2, int(max_flip_frac * N)), f"{n_flip} of {N} systems took different decisions"
+    if n_flip:
+        # a flipped system is still a valid integration: agrees to the integrator's own accuracy
+        assert relT[~same].max() <= 1e-6
+        absY = np.abs(Yg - Yo)[:, ~same]
+        assert (absY <= 1e-5 * np.abs(Yo[:, ~same]) + 1e-9).all()
+    return dict(n=N, flipped=n_flip, relT=float(relT[same].max(initial=0.0)), relY=float(relY[same].max(initial=0.0)))
+
+
+def _oracle(mech, states, p, dt, method, pressure=None):
+    import oracle
+    om = oracle.OracleMech(mech)
+    return om.integrate(states, p, dt, RTOL, ATOL, method, pressure=pressure)
+
+
+CASES = [
+    # cfg, N, dt, variant
+    (0, 1024, 1e-6, "auto"),
+    (1, 1500, 1e-6, "thread"),
+    (2, 1024, 1e-6, "auto"),
+    (2, 300, 1e-6, "warp"),
+    (2, 300, 1e-6, "sub8"),
+    (3, 256, 1e-6, "auto"),
+    (3, 130, 1e-6, "sub8"),
+    (3, 130, 1e-6, "sub16"),
+    (4, 96, 1e-6, "warp"),
+    (4, 48, 1e-5, "warp"),
+    (4, 40, 1e-6, "sub8"),
+]
+
+
+@pytest.mark.parametrize("cfg,N,dt,variant", CASES)
+def test_parity_configs(cfg, N, dt, variant):
+    spec = synth.CONFIGS[cfg]
+    mech = synth.make_mechanism(cfg)
+    states, p = synth.make_states(cfg, N)
+    ora = _oracle(mech, states, p, dt, spec.method)
+    gpu = _run_gpu(mech, states, p, dt, spec.method, variant=variant, ld=N + 37)   # ragged row stride
+    rep = _compare(gpu, ora)
+    print(f"cfg{cfg} {spec.method} {variant} N={N} dt={dt}: {rep}")
+    assert (ora[1] == 0).all()
+
+
+@pytest.mark.parametrize("cfg,method", [(0, "rkc"), (2, "rkck")])
+def test_parity_other_method(cfg, method):
+    """Both integrators on both small mechanisms (RKC on the nonstiff one, RKCK on the stiff one)."""
+    mech = synth.make_mechanism(cfg)
+    states, p = synth.make_states(cfg, 512)
+    _compare(_run_gpu(mech, states, p, 1e-6, method), _oracle(mech, states, p, 1e-6, method))
+
+
+def test_per_system_pressure_and_similar_ordering():
+    mech = synth.make_mechanism(2)
+    states, p = synth.make_states(2, 400, ordering="similar")
+    pressure = p * np.linspace(0.5, 2.0, 400)
+    gpu = _run_gpu(mech, states, 0.0, 1e-6, "rkc", pressure=pressure)
+    ora = _oracle(mech, states, p, 1e-6, "rkc", pressure=pressure)
+    _compare(gpu, ora)
+
+
+def test_source_term_parity():
+    """ckb_rhs against the oracle's f(y): every variant, every mechanism."""
+    import torch
+    import oracle
+    from paper_1309_2710_b200 import binding
+    for cfg, variants in ((0, ("thread", "warp", "sub8")), (2, ("thread", "sub16")), (3, ("warp", "sub8", "sub16")),
+                          (4, ("warp", "sub8"))):
+        mech = synth.make_mechanism(cfg)
+        om = oracle.OracleMech(mech)
+        states, p = synth.make_states(cfg, 70)
+        ref = np.stack([om.rhs(states[:, i].copy(), p) for i in range(70)], axis=1)
+        m = binding.mech_load(mech)
+        st = torch.from_numpy(states).cuda()
+        for v in variants:
+            out = binding.rhs(m, st, p=p, variant=v).cpu().numpy()
+            scale = np.abs(ref).max(axis=1, keepdims=True)
+            assert (np.abs(out - ref) <= 1e-11 * scale + 1e-13 * np.abs(ref)).all(), (cfg, v)
+        m.close()
+
+
+def test_empty_and_single():
+    import torch
+    from paper_1309_2710_b200 import binding
+    mech = synth.make_mechanism(0)
+    m = binding.mech_load(mech)
+    empty = torch.empty((10, 0), dtype=torch.float64, device="cuda")
+    binding.integrate(m, empty, 1e-6, RTOL, ATOL, "rkck", p=synth.P_ATM)
+    m.close()
+    states, p = synth.make_states(0, 1)
+    for method in ("rkck", "rkc"):
+        _compare(_run_gpu(mech, states, p, 1e-6, method), _oracle(mech, states, p, 1e-6, method))
+
+
+def test_toy_mechanisms_closed_form():
+    """A -> B with equal W and identical thermo: Y_A(t) = Y_A0 exp(-A t), through the CUDA path."""
+    mech = synth.toy_mechanism(2, [({0: 1}, {1: 1}, 5e5, 0.0, 0.0)])
+    N = 33
+    states = np.zeros((3, N))
+    states[0] = np.linspace(900, 1800, N)
+    states[1] = np.linspace(0.1, 1.0, N)
+    states[2] = 1.0 - states[1]
+    for method in ("rkck", "rkc"):
+        for variant in ("thread", "warp"):
+            y, st, _ = _run_gpu(mech, states, synth.P_ATM, 1e-6, method, variant=variant)
+            assert (st == 0).all()
+            assert np.allclose(y[1], states[1] * np.exp(-5e5 * 1e-6), rtol=2e-7, atol=0)
+            assert np.allclose(y[0], states[0], rtol=1e-12)
+            assert np.allclose(y[1] + y[2], 1.0, rtol=0, atol=1e-14)
+
+
+def test_host_entry_matches_device_entry():
+    from paper_1309_2710_b200 import binding
+    mech = synth.make_mechanism(2)
+    states, p = synth.make_states(2, 257)
+    dev, sd, td = _run_gpu(mech, states, p, 1e-6, "rkc")
+    m = binding.mech_load(mech)
+    host = states.copy()
+    status = np.full(257, -1, dtype=np.int32)
+    stats = np.full((4, 257), -1, dtype=np.int32)
+    binding.integrate_host(m, host, 1e-6, RTOL, ATOL, "rkc", p=p, status=status, stats=stats)
+    m.close()
+    assert np.array_equal(host, dev) and np.array_equal(status, sd) and np.array_equal(stats, td)
+
+
+def test_linear_invariants_on_gpu():
+    """Sum Y and element mass fractions are conserved by the CUDA path (Runge-Kutta methods keep linear invariants)."""
+    for cfg, method in ((1, "rkck"), (3, "rkc")):
+        mech = synth.make_mechanism(cfg)
+        states, p = synth.make_states(cfg, 200)
+        y, st, _ = _run_gpu(mech, states, p, 1e-6, method)
+        aw = np.array([synth.ATOMIC_WEIGHT[e] for e in mech.elements])
+        Z = lambda s: (mech.elem_counts * aw).T @ (s[1:] / mech.mol_weight[:, None])
+        assert np.abs(y[1:].sum(0) - 1.0).max() < 1e-12
+        assert np.abs(Z(y) - Z(states)).max() < 1e-12
