@@ -1,0 +1,351 @@
+#!/usr/bin/env python
+"""bench.py -- ODE systems integrated per second for one global step dt (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C] [--n N] [--no-extra]
+
+A "step" is one pass of the whole hot path over one batch: ckb_integrate() advances all N systems of the
+workload from their (seeded, synthetic) initial states over one global step dt -- load state, adaptive
+sub-stepping (RKCK or RKC with its spectral-radius estimate), source term f(y) fused in, store state.
+Headline workload = BASELINE.json configs[1] (9/38 synthetic mechanism, RKCK, N = 2^19, dt = 1e-6 s,
+rtol 1e-8, atol 1e-12); the other configs are measured too and reported under "configs" (configs[3] at
+N = 2^17 is the one north_star's roofline target is stated on).
+
+Timing: every step restarts from the same initial states (device-to-device copy, not timed), L2 is flushed
+(256 MiB write, not timed), then CUDA events on the launching stream bracket the ckb_integrate launch;
+`value` = N * K / sum of the K event durations (max over ranks).  `e2e` is the same step through
+ckb_integrate_host with pinned HOST buffers (H2D + kernel + D2H inside the timed region).
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1309_2710_b200 import synth  # noqa: E402
+
+RTOL, ATOL = 1e-8, 1e-12
+METRIC = "ODE systems integrated/sec per global dt"
+UNIT = "ODEs/s"
+# nominal FP64 FMA peak of a B200: 148 SMs x 64 FP64 FMA lanes/clk x 2 flop x 1.965 GHz
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+HEADLINE_N = {0: 1024, 1: 2 ** 19, 2: 2 ** 18, 3: 2 ** 17, 4: 2 ** 16}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--n", type=int, default=0, help="override the batch size N")
+    ap.add_argument("--dt", type=float, default=0.0)
+    ap.add_argument("--variant", default="auto")
+    ap.add_argument("--ordering", default="shuffled", choices=["shuffled", "similar"])
+    ap.add_argument("--no-extra", action="store_true", help="skip the other configs, e2e and cpu_baseline")
+    ap.add_argument("--sweep", action="store_true", help="also sweep N over the config's N_list")
+    return ap.parse_args()
+
+
+def workload(cfg, n_override=0, dt=0.0):
+    spec = synth.CONFIGS[cfg]
+    N = n_override or HEADLINE_N[cfg]
+    return spec, N, (dt or spec.dt[0])
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self._stop = [], set(), threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:  # pragma: no cover
+            self.nv = None
+            self.max = None
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:  # pragma: no cover
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.nv:
+            self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self.nv:
+            self.t.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+class GpuCase:
+    """One (config, N, dt, variant) workload resident on the GPU."""
+
+    def __init__(self, cfg, N, dt, variant="auto", ordering="shuffled", device=0):
+        import torch
+        from paper_1309_2710_b200 import binding
+        self.torch, self.binding = torch, binding
+        self.spec = synth.CONFIGS[cfg]
+        self.cfg, self.N, self.dt, self.variant = cfg, N, dt, variant
+        self.mech = synth.make_mechanism(cfg)
+        self.m = binding.mech_load(self.mech)
+        st, self.p = synth.make_states(cfg, N, ordering=ordering)
+        self.host0 = st
+        self.states0 = torch.from_numpy(st).cuda()
+        self.states = torch.empty_like(self.states0)
+        self.status = torch.zeros((N,), dtype=torch.int32, device="cuda")
+        self.stats = torch.zeros((4, N), dtype=torch.int32, device="cuda")
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def step(self, want_stats=False):
+        self.binding.integrate(self.m, self.states, self.dt, RTOL, ATOL, self.spec.method, p=self.p,
+                               variant=self.variant, status=self.status if want_stats else None,
+                               stats=self.stats if want_stats else None)
+
+    def timed_steps(self, K, W):
+        """Returns the K per-step kernel durations in ms (CUDA events on the launching stream)."""
+        torch = self.torch
+        for _ in range(W):
+            self.states.copy_(self.states0)
+            self.step()
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        for a, b in ev:
+            self.states.copy_(self.states0)
+            self.flush.fill_(1)
+            a.record()
+            self.step()
+            b.record()
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    def work(self):
+        """Per-step work counters (same every step: same inputs): one untimed step with stats on."""
+        torch = self.torch
+        self.states.copy_(self.states0)
+        self.step(want_stats=True)
+        torch.cuda.synchronize()
+        st = self.stats.cpu().numpy().astype(np.int64)
+        status = self.status.cpu().numpy()
+        d = st[0].reshape(-1, 32) if self.N % 32 == 0 else None
+        out = {"rhs_calls": int(st[0].sum()), "rhs_per_ode_mean": float(st[0].mean()), "rhs_per_ode_max": int(st[0].max()),
+               "accepted_mean": float(st[1].mean()), "rejected_mean": float(st[2].mean()),
+               "stages_max": int(st[3].max()), "status_nonzero": int((status != 0).sum()),
+               "status_sigma": int((status == 4).sum())}
+        if d is not None:   # Eq. 40: D = sum d_i / (32 max d_i) per 32 consecutive systems
+            out["divergence_D_mean"] = float((d.sum(1) / (32.0 * d.max(1))).mean())
+        return out
+
+    def e2e(self, K, W):
+        """ckb_integrate_host on pinned host buffers: H2D + kernel + D2H inside the timed region."""
+        torch = self.torch
+        n = self.mech.n_species + 1
+        host = torch.empty((n, self.N), dtype=torch.float64).pin_memory()
+        status = torch.zeros((self.N,), dtype=torch.int32).pin_memory()
+        src = torch.from_numpy(self.host0)
+        times = []
+        for i in range(W + K):
+            host.copy_(src)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            self.binding.integrate_host(self.m, host, self.dt, RTOL, ATOL, self.spec.method, p=self.p,
+                                        variant=self.variant, status=status)
+            t1 = time.perf_counter()
+            if i >= W:
+                times.append(t1 - t0)
+        return times, n * self.N * 8, n * self.N * 8 + 4 * self.N
+
+    def close(self):
+        self.m.close()
+
+
+def roofline(case, ms, work, peak_tflops, peak_src):
+    flops = case.m.flops_per_rhs * work["rhs_calls"]
+    ach = flops / (ms * 1e-3) / 1e12
+    return {"bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s", "frac": ach / peak_tflops,
+            "traffic": None, "peak_source": peak_src, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
+            "flops_per_rhs": case.m.flops_per_rhs, "rhs_calls_per_launch": work["rhs_calls"],
+            "kernel_ms": ms, "hbm_algorithmic_GBps": 2 * 8 * (case.mech.n_species + 1) * case.N / (ms * 1e-3) / 1e9}
+
+
+def oracle_time(cfg, N, dt, budget_s=15.0, nthreads=0):
+    """The oracle as it stands on a bounded sample (first n systems of the same workload)."""
+    import oracle
+    spec = synth.CONFIGS[cfg]
+    mech = synth.make_mechanism(cfg)
+    om = oracle.OracleMech(mech)
+    states, p = synth.make_states(cfg, N)
+    probe = min(N, 256)
+    t0 = time.perf_counter()
+    om.integrate(states[:, :probe], p, dt, RTOL, ATOL, spec.method, nthreads=nthreads)
+    t_probe = time.perf_counter() - t0
+    n = int(min(N, max(probe, probe * budget_s / max(t_probe, 1e-6))))
+    t0 = time.perf_counter()
+    om.integrate(states[:, :n], p, dt, RTOL, ATOL, spec.method, nthreads=nthreads)
+    t = time.perf_counter() - t0
+    cores = oracle.num_threads() if nthreads <= 0 else nthreads
+    return n / t, n, cores, t
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, bounded sample per step (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    spec, N, dt = workload(args.config, args.n, args.dt)
+    budget = max(2.0, min(15.0, 120.0 / max(1, args.steps + args.warmup)))
+    rates, n_used, cores = [], 0, 0
+    for i in range(args.warmup + args.steps):
+        r, n_used, cores, _ = oracle_time(args.config, N, dt, budget_s=budget)
+        if i >= args.warmup:
+            rates.append(r)
+    value = float(len(rates) / sum(1.0 / r for r in rates))
+    sample = f"first {n_used} of {N} systems of the workload per step, OpenMP over systems"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * N / value, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {spec.name} species/reactions, {spec.method.upper()}, "
+                               f"N={N}, dt={dt:g} s, rtol={RTOL:g}, atol={ATOL:g}", "N": N, "sample_n": n_used},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    spec, N, dt = workload(args.config, args.n, args.dt)
+    K, W = args.steps, max(args.warmup, 3)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    from paper_1309_2710_b200 import binding
+    peak_flops = binding.fp64_probe("dfma", 1 << 15)
+    exp_rate = binding.fp64_probe("exp", 1 << 12)
+    # every rank integrates its own N systems (independent problems, no data-path collective): weak scaling
+    case = GpuCase(args.config, N, dt, args.variant, args.ordering, local)
+    work = case.work()
+    barrier()
+    with ClockSampler(local) as clk:
+        ms = case.timed_steps(K, W)
+    barrier()
+    total_ms = float(sum(ms))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = N * world * K / (total_ms * 1e-3)
+    ms_step = total_ms / K
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {spec.name} species/reactions, {spec.method.upper()}, "
+                               f"N={N} per GPU, dt={dt:g} s, rtol={RTOL:g}, atol={ATOL:g}",
+                   "N_per_gpu": N, "variant": args.variant, "ordering": args.ordering,
+                   "l2": "flushed between timed steps (256 MiB write, untimed)",
+                   "restart": "every step restarts from the same initial states (device copy, untimed)"},
+        "clocks": clk.summary(),
+        "gpu_launches": K,
+        "work_per_step": work,
+        "roofline": roofline(case, float(np.mean(ms)), work, peak_flops / 1e12,
+                             "measured: ckb_fp64_probe DFMA chains on this GPU (MEASURED_PEAKS.json has no FP64 figure)"),
+        "exp_per_s": {"achieved": 2.0 * case.m.n_slots * work["rhs_calls"] / (np.mean(ms) * 1e-3), "peak_measured": exp_rate},
+        "ms_min_max": [float(min(ms)), float(max(ms))],
+    }
+    if rank == 0 and not args.no_extra:
+        tt, h2d, d2h = case.e2e(min(K, 5), 2)
+        e = N / float(np.mean(tt))
+        out["e2e"] = {"value": e * world, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                      "note": "ckb_integrate_host on pinned host buffers; measured on rank 0, scaled by n_gpus"}
+    if rank == 0 and not args.no_extra and world == 1:
+        r, n_used, cores, t = oracle_time(args.config, N, dt, budget_s=12.0)
+        out["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": f"first {n_used} of {N} systems of the workload, {t:.1f} s, OpenMP over systems"}
+        r1, n1, _, t1 = oracle_time(args.config, N, dt, budget_s=6.0, nthreads=1)
+        out["cpu_baseline"]["single_core"] = {"value": r1, "sample_n": n1, "seconds": t1}
+        extra = {}
+        others = [c for c in (2, 3, 4) if c != args.config] + ([1] if args.config != 1 else [])
+        for c in others:
+            s2, N2, dt2 = workload(c)
+            for var in (("auto",) if c != 3 else ("warp", "sub16", "sub8")):
+                try:
+                    cs = GpuCase(c, N2, dt2, var)
+                    wk = cs.work()
+                    m2 = cs.timed_steps(3, 3)
+                    extra[f"cfg{c}_{s2.method}_{var}_N{N2}"] = {
+                        "odes_per_s": N2 / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)), "work": wk,
+                        "roofline": roofline(cs, float(np.mean(m2)), wk, peak_flops / 1e12, "measured DFMA probe")}
+                    cs.close()
+                    del cs
+                except Exception as ex:  # pragma: no cover
+                    extra[f"cfg{c}_{var}"] = {"error": str(ex)}
+        out["configs"] = extra
+    if args.sweep and rank == 0 and world == 1:
+        sw = {}
+        for n in spec.N_list:
+            cs = GpuCase(args.config, n, dt, args.variant, args.ordering)
+            m2 = cs.timed_steps(5, 3)
+            sw[str(n)] = {"odes_per_s": n / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2))}
+            cs.close()
+        out["sweep"] = sw
+    if "e2e" not in out:
+        out["e2e"] = None
+    case.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
