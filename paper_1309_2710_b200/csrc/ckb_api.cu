@@ -308,8 +308,10 @@ int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out) {
   }
   cudaError_t e = cudaMalloc((void **)&m->d_blob, m->blob.size() * 8 + 8);
   if (e == cudaSuccess) e = cudaMemcpy(m->d_blob, m->blob.data(), m->blob.size() * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMalloc((void **)&m->d_counters, CKB_COUNTER_RING * 8);
   if (e != cudaSuccess) {
     if (m->d_blob) cudaFree(m->d_blob);
+    if (m->d_counters) cudaFree(m->d_counters);
     delete m;
     return ckb_host::cuda_fail(e, "ckb_mech_load upload");
   }
@@ -320,6 +322,7 @@ int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out) {
 void ckb_mech_free(ckb_mech *m) {
   if (!m) return;
   if (m->d_blob) cudaFree(m->d_blob);
+  if (m->d_counters) cudaFree(m->d_counters);
   if (m->ws_states) cudaFree(m->ws_states);
   if (m->ws_pressure) cudaFree(m->ws_pressure);
   if (m->ws_status) cudaFree(m->ws_status);

@@ -37,7 +37,6 @@ struct Sys {
   int g;                /* lane within the group */
   int src0;             /* warp lane that holds component 0 (T) */
   double p;             /* pressure, dyn/cm^2 (R24: constant over the call) */
-  int nfe;
 
   __device__ __forceinline__ Sys(const DevMech &m_, const TAB &tab_) : m(m_), tab(tab_) {}
   __device__ __forceinline__ unsigned long long tw(int i) const { return tab.ld(i); }
@@ -64,7 +63,6 @@ struct Sys {
 
   /* f(y): Eq. 2-6.  y, f: component (g + L*i) in slot i. */
   __device__ __forceinline__ void rhs(const double (&y)[NV], double (&f)[NV]) {
-    nfe++;
     const int K = m.K;
     const double T = bcast0(y[0]);
     const double invT = 1.0 / T;
@@ -163,33 +161,44 @@ struct Sys {
 #define CKB_U 2.220446049250313e-16      /* 2^-52 */
 #define CKB_SQRTU 1.4901161193847656e-08 /* 2^-26 */
 
-/* ------------------------------------------------------------------------------------------------
- * RKCK driver: Eq. 7-17, Table 1; DESIGN.md 4.2 (R1-R7, R25).
- * ---------------------------------------------------------------------------------------------- */
-template <class S>
-__device__ __forceinline__ int rkck_driver(S &sys, double (&y)[S::NV], double t0, double t1, double rtol,
-                                           double atol, int (&st)[4]) {
-  constexpr int NV = S::NV;
-  /* Table 1 (R1: Cash-Karp values) */
-  constexpr double B21 = 1.0 / 5.0;
-  constexpr double B31 = 3.0 / 40.0, B32 = 9.0 / 40.0;
-  constexpr double B41 = 3.0 / 10.0, B42 = -9.0 / 10.0, B43 = 6.0 / 5.0;
-  constexpr double B51 = -11.0 / 54.0, B52 = 5.0 / 2.0, B53 = -70.0 / 27.0, B54 = 35.0 / 27.0;
-  constexpr double B61 = 1631.0 / 55296.0, B62 = 175.0 / 512.0, B63 = 575.0 / 13824.0,
-                   B64 = 44275.0 / 110592.0, B65 = 253.0 / 4096.0;
-  constexpr double C1 = 37.0 / 378.0, C3 = 250.0 / 621.0, C4 = 125.0 / 594.0, C6 = 512.0 / 1771.0;
-  constexpr double D1 = C1 - 2825.0 / 27648.0, D3 = C3 - 18575.0 / 48384.0, D4 = C4 - 13525.0 / 55296.0,
-                   D5 = -277.0 / 14336.0, D6 = C6 - 1.0 / 4.0;
-  constexpr double SAFETY = 0.9;
+/* ================================================================================================
+ * Integrators as state machines with ONE call site of f(y).
+ *
+ * Each integrator object holds the whole per-system controller state in registers.  The kernel loop is
+ *     while (work) { f = rhs(integ.w);  done = integ.advance(f); }
+ * so that (a) the source term -- > 90 % of the instructions -- is inlined once, and (b) in the
+ * thread-per-ODE mapping all lanes of a warp evaluate f(y) together whatever sub-step, stage or
+ * power-method iteration each of them is in: divergence is confined to the short vector updates
+ * between two evaluations (the paper's divergence sources, made harmless).
+ * The arithmetic and the order of the controller decisions follow DESIGN.md section 4 step by step.
+ * ============================================================================================== */
 
-  double k1[NV], k2[NV], k3[NV], k4[NV], k5[NV], k6[NV], yt[NV];
-  int nacc = 0, nrej = 0, status = ST_OK;
-  double t = t0, h = t1 - t0; /* R4: first trial step = the whole global step */
-  bool have_k1 = false, saw_nonfinite = false;
-  int attempts = 0;
-  while (true) {
-    bool last = false;
-    if (1.1 * h >= t1 - t) { /* R5 */
+/* RKCK: Eq. 7-17, Table 1; R1-R7, R25. */
+template <class S>
+struct Rkck {
+  static constexpr int NV = S::NV;
+  /* Table 1 (R1: Cash-Karp values) */
+  static constexpr double B21 = 1.0 / 5.0;
+  static constexpr double B31 = 3.0 / 40.0, B32 = 9.0 / 40.0;
+  static constexpr double B41 = 3.0 / 10.0, B42 = -9.0 / 10.0, B43 = 6.0 / 5.0;
+  static constexpr double B51 = -11.0 / 54.0, B52 = 5.0 / 2.0, B53 = -70.0 / 27.0, B54 = 35.0 / 27.0;
+  static constexpr double B61 = 1631.0 / 55296.0, B62 = 175.0 / 512.0, B63 = 575.0 / 13824.0,
+                          B64 = 44275.0 / 110592.0, B65 = 253.0 / 4096.0;
+  static constexpr double C1 = 37.0 / 378.0, C3 = 250.0 / 621.0, C4 = 125.0 / 594.0, C6 = 512.0 / 1771.0;
+  static constexpr double D1 = C1 - 2825.0 / 27648.0, D3 = C3 - 18575.0 / 48384.0,
+                          D4 = C4 - 13525.0 / 55296.0, D5 = -277.0 / 14336.0, D6 = C6 - 1.0 / 4.0;
+  static constexpr double SAFETY = 0.9;
+
+  double w[NV];                 /* the next argument of f */
+  double y[NV], k1[NV], k2[NV], k3[NV], k4[NV], k5[NV];
+  double t, h, t1, rtol, atol;
+  int stage, nfe, nacc, nrej, attempts, status;
+  bool last, saw_nonfinite;
+
+  /* R5 clip, then either evaluate k1 (stage 1) or go on with the stages (k1 kept and rescaled, R25) */
+  __device__ __forceinline__ void begin_attempt(bool have_k1) {
+    last = false;
+    if (1.1 * h >= t1 - t) {
       const double hn = t1 - t;
       if (have_k1) {
         const double r = hn / h;
@@ -199,52 +208,89 @@ __device__ __forceinline__ int rkck_driver(S &sys, double (&y)[S::NV], double t0
       h = hn;
       last = true;
     }
-    if (!have_k1) { /* Eq. 7 */
-      sys.rhs(y, k1);
+    if (!have_k1) {
+      stage = 1;
 #pragma unroll
-      for (int i = 0; i < NV; i++) k1[i] *= h;
-      have_k1 = true;
+      for (int i = 0; i < NV; i++) w[i] = y[i];
+    } else {
+      start_stages();
     }
+  }
+  __device__ __forceinline__ void start_stages() {
     if (++attempts > 1000000) { /* R7 */
       status = ST_MAXSTEPS;
-      break;
+      stage = 0;
+      return;
     }
-    /* Eq. 8-12 */
+    stage = 2;
 #pragma unroll
-    for (int i = 0; i < NV; i++) yt[i] = fma(B21, k1[i], y[i]);
-    sys.rhs(yt, k2);
+    for (int i = 0; i < NV; i++) w[i] = fma(B21, k1[i], y[i]);
+  }
+
+  __device__ __forceinline__ void start(const double (&y0)[NV], double t0_, double t1_, double rtol_, double atol_,
+                                        int /*n*/) {
 #pragma unroll
-    for (int i = 0; i < NV; i++) {
-      k2[i] *= h;
-      yt[i] = fma(B32, k2[i], fma(B31, k1[i], y[i]));
+    for (int i = 0; i < NV; i++) y[i] = y0[i];
+    t = t0_; t1 = t1_; rtol = rtol_; atol = atol_;
+    h = t1_ - t0_; /* R4 */
+    nfe = nacc = nrej = attempts = 0;
+    status = ST_OK;
+    saw_nonfinite = false;
+    begin_attempt(false);
+  }
+
+  /* consume f = f(w); returns true when the system has reached t1 (or failed) */
+  __device__ __forceinline__ bool advance(const S &sys, const double (&f)[NV]) {
+    nfe++;
+    switch (stage) {
+      case 1: /* Eq. 7 */
+#pragma unroll
+        for (int i = 0; i < NV; i++) k1[i] = h * f[i];
+        start_stages();
+        return stage == 0;
+      case 2:
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+          k2[i] = h * f[i];
+          w[i] = fma(B32, k2[i], fma(B31, k1[i], y[i]));
+        }
+        stage = 3;
+        return false;
+      case 3:
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+          k3[i] = h * f[i];
+          w[i] = fma(B43, k3[i], fma(B42, k2[i], fma(B41, k1[i], y[i])));
+        }
+        stage = 4;
+        return false;
+      case 4:
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+          k4[i] = h * f[i];
+          w[i] = fma(B54, k4[i], fma(B53, k3[i], fma(B52, k2[i], fma(B51, k1[i], y[i]))));
+        }
+        stage = 5;
+        return false;
+      case 5:
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+          k5[i] = h * f[i];
+          w[i] = fma(B65, k5[i], fma(B64, k4[i], fma(B63, k3[i], fma(B62, k2[i], fma(B61, k1[i], y[i])))));
+        }
+        stage = 6;
+        return false;
+      default:
+        break;
     }
-    sys.rhs(yt, k3);
-#pragma unroll
-    for (int i = 0; i < NV; i++) {
-      k3[i] *= h;
-      yt[i] = fma(B43, k3[i], fma(B42, k2[i], fma(B41, k1[i], y[i])));
-    }
-    sys.rhs(yt, k4);
-#pragma unroll
-    for (int i = 0; i < NV; i++) {
-      k4[i] *= h;
-      yt[i] = fma(B54, k4[i], fma(B53, k3[i], fma(B52, k2[i], fma(B51, k1[i], y[i]))));
-    }
-    sys.rhs(yt, k5);
-#pragma unroll
-    for (int i = 0; i < NV; i++) {
-      k5[i] *= h;
-      yt[i] = fma(B65, k5[i], fma(B64, k4[i], fma(B63, k3[i], fma(B62, k2[i], fma(B61, k1[i], y[i])))));
-    }
-    sys.rhs(yt, k6);
-    /* Eq. 13, 15, 16 (R2), 17 (R3) */
+    /* stage 6: Eq. 13, 15, 16 (R2), 17 (R3) */
     double errmax = 0.0;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      k6[i] *= h;
-      const double yn = fma(C6, k6[i], fma(C4, k4[i], fma(C3, k3[i], fma(C1, k1[i], y[i]))));
-      const double dl = fma(D6, k6[i], fma(D5, k5[i], fma(D4, k4[i], fma(D3, k3[i], D1 * k1[i]))));
-      yt[i] = yn;
+      const double k6 = h * f[i];
+      const double yn = fma(C6, k6, fma(C4, k4[i], fma(C3, k3[i], fma(C1, k1[i], y[i]))));
+      const double dl = fma(D6, k6, fma(D5, k5[i], fma(D4, k4[i], fma(D3, k3[i], D1 * k1[i]))));
+      w[i] = yn;
       if (sys.valid(i)) {
         const double d0 = fma(rtol, fabs(y[i]) + fabs(k1[i]), atol);
         double e = fabs(dl) / d0;
@@ -256,176 +302,130 @@ __device__ __forceinline__ int rkck_driver(S &sys, double (&y)[S::NV], double t0
     if (errmax <= 1.0) { /* P:139 accept */
       nacc++;
 #pragma unroll
-      for (int i = 0; i < NV; i++) y[i] = yt[i];
-      have_k1 = false;
-      if (last) break;
+      for (int i = 0; i < NV; i++) y[i] = w[i];
+      if (last) return true;
       t += h;
       double fac = (errmax > 0.0) ? SAFETY * pow(errmax, -0.2) : 5.0;
       if (fac > 5.0) fac = 5.0;
       h *= fac;
-    } else {
-      nrej++;
-      double fac;
-      if (isfinite(errmax)) {
-        fac = SAFETY * pow(errmax, -0.25);
-        if (fac < 0.1) fac = 0.1;
-      } else {
-        fac = 0.1;
-        saw_nonfinite = true;
-      }
-#pragma unroll
-      for (int i = 0; i < NV; i++) k1[i] *= fac; /* R25 */
-      h *= fac;
-      const double tmax = fmax(fabs(t), fabs(t1));
-      if (!(h > 10.0 * CKB_U * tmax)) { /* R6 */
-        status = saw_nonfinite ? ST_NONFINITE : ST_UNDERFLOW;
-        break;
-      }
+      begin_attempt(false);
+      return false;
     }
+    nrej++;
+    double fac;
+    if (isfinite(errmax)) {
+      fac = SAFETY * pow(errmax, -0.25);
+      if (fac < 0.1) fac = 0.1;
+    } else {
+      fac = 0.1;
+      saw_nonfinite = true;
+    }
+#pragma unroll
+    for (int i = 0; i < NV; i++) k1[i] *= fac; /* R25 */
+    h *= fac;
+    const double tmax = fmax(fabs(t), fabs(t1));
+    if (!(h > 10.0 * CKB_U * tmax)) { /* R6 */
+      status = saw_nonfinite ? ST_NONFINITE : ST_UNDERFLOW;
+      return true;
+    }
+    begin_attempt(true);
+    return stage == 0;
   }
-  st[0] = sys.nfe;
-  st[1] = nacc;
-  st[2] = nrej;
-  st[3] = 0;
-  return status;
-}
 
-/* ------------------------------------------------------------------------------------------------
- * Spectral radius by the nonlinear power method (R17/R18).
- * y, fy = f(y); v = previous eigenvector estimate (have_v) -- on return the new one.  z, gq: scratch.
- * ---------------------------------------------------------------------------------------------- */
+  __device__ __forceinline__ void result(int (&st)[4]) const {
+    st[0] = nfe; st[1] = nacc; st[2] = nrej; st[3] = 0;
+  }
+};
+
+/* RKC: Eq. 18-39 and P:233; R8-R18, R26.  Spectral radius by the nonlinear power method (R17/R18). */
 template <class S>
-__device__ __forceinline__ double spectral_radius(S &sys, const double (&y)[S::NV], const double (&fy)[S::NV],
-                                                  double (&v)[S::NV], bool have_v, int &flag,
-                                                  double (&z)[S::NV], double (&gq)[S::NV]) {
-  constexpr int NV = S::NV;
-  if (!have_v) {
-#pragma unroll
-    for (int i = 0; i < NV; i++) v[i] = fy[i];
-  }
-  double a = 0.0, b = 0.0;
-#pragma unroll
-  for (int i = 0; i < NV; i++) {
-    a = fma(y[i], y[i], a);
-    b = fma(v[i], v[i], b);
-  }
-  const double ynrm = sqrt(sys.gsum(a)), vnrm = sqrt(sys.gsum(b));
-  double d;
-  if (ynrm != 0.0 && vnrm != 0.0) {
-    d = ynrm * CKB_SQRTU;
-    const double r = d / vnrm;
-#pragma unroll
-    for (int i = 0; i < NV; i++) z[i] = fma(v[i], r, y[i]);
-  } else if (ynrm != 0.0) {
-    d = ynrm * CKB_SQRTU;
-#pragma unroll
-    for (int i = 0; i < NV; i++) z[i] = y[i] * (1.0 + CKB_SQRTU);
-  } else if (vnrm != 0.0) {
-    d = CKB_U;
-    const double r = d / vnrm;
-#pragma unroll
-    for (int i = 0; i < NV; i++) z[i] = v[i] * r;
-  } else {
-    d = CKB_U;
-#pragma unroll
-    for (int i = 0; i < NV; i++) z[i] = sys.valid(i) ? d : 0.0;
-  }
-  double sigma = 0.0;
-  bool converged = false;
-  for (int it = 1; it <= 50; it++) {
-    sys.rhs(z, gq);
-    double dd = 0.0;
+struct Rkc {
+  static constexpr int NV = S::NV;
+  enum { S_F0 = 1, S_PM = 2, S_H0 = 3, S_STAGE = 4, S_FINAL = 5 };
+
+  double w[NV];                                   /* the next argument of f: y, z (power method), w_{j-1} */
+  double y[NV], f0[NV], wjm2[NV], v[NV];
+  double t, h, t1, Dt, rtol, atol, nd;
+  double sigma, err_old, h_old;
+  double pm_d, pm_sigma;                          /* power method: displacement size, last estimate */
+  double w0, w1, Tm1, Tm2, dm1, dm2, em1, em2, bjm1, bjm2, ajm1; /* Eq. 22-26 recurrences */
+  int state, j, s, s_max, pm_it;
+  int nfe, nacc, nrej, smax_used, attempts, since_sigma, status, flag;
+  bool last, have_prev, saw_nonfinite, sigma_fresh, need_sigma, pm_initial;
+
+  __device__ __forceinline__ void start(const double (&y0)[NV], double t0_, double t1_, double rtol_, double atol_,
+                                        int n) {
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      const double e = gq[i] - fy[i];
-      dd = fma(e, e, dd);
+      y[i] = y0[i];
+      w[i] = y0[i];
     }
-    dd = sqrt(sys.gsum(dd));
-    const double sigma_prev = sigma;
-    sigma = dd / d;
-    const double fl = sigma > 1e-300 ? sigma : 1e-300;
-    if (it >= 2 && fabs(sigma - sigma_prev) <= 0.01 * fl) {
-      converged = true;
-      break;
-    }
-    if (dd != 0.0) {
-      const double r = d / dd;
-#pragma unroll
-      for (int i = 0; i < NV; i++) z[i] = fma(gq[i] - fy[i], r, y[i]);
-    } else {
-      const int ci = it % sys.m.n;
-#pragma unroll
-      for (int i = 0; i < NV; i++)
-        if (sys.g + S::L * i == ci) z[i] = y[i] - (z[i] - y[i]);
-    }
+    t = t0_; t1 = t1_; Dt = t1_ - t0_; rtol = rtol_; atol = atol_; nd = (double)n;
+    s_max = (int)floor(sqrt(rtol_ / (10.0 * CKB_U)) + 0.5); /* R12 */
+    if (s_max < 2) s_max = 2;
+    nfe = nacc = nrej = smax_used = attempts = since_sigma = 0;
+    status = ST_OK; flag = 0;
+    have_prev = saw_nonfinite = need_sigma = false;
+    sigma_fresh = true;
+    err_old = h_old = 0.0;
+    state = S_F0;
   }
+
+  /* power method set-up: place z at distance d from y along v (R17 step 2) */
+  __device__ __forceinline__ void pm_begin(const S &sys, bool have_v, bool initial) {
+    if (!have_v) {
 #pragma unroll
-  for (int i = 0; i < NV; i++) v[i] = z[i] - y[i];
-  if (!converged) flag = ST_SIGMA;
-  return 1.2 * sigma; /* R18 */
-}
-
-/* ------------------------------------------------------------------------------------------------
- * RKC driver: Eq. 18-39 and P:233; DESIGN.md 4.4 (R8-R18, R26).
- * ---------------------------------------------------------------------------------------------- */
-template <class S>
-__device__ __forceinline__ int rkc_driver(S &sys, double (&y)[S::NV], double t0, double t1, double rtol,
-                                          double atol, int (&st)[4]) {
-  constexpr int NV = S::NV;
-  const double Dt = t1 - t0;
-  const double nd = (double)sys.m.n;
-  int s_max = (int)floor(sqrt(rtol / (10.0 * CKB_U)) + 0.5); /* R12 */
-  if (s_max < 2) s_max = 2;
-  double f0[NV], fj[NV], wjm1[NV], wjm2[NV], v[NV];
-  int nacc = 0, nrej = 0, smax_used = 0, status = ST_OK, flag = 0;
-  double t = t0;
-
-  sys.rhs(y, f0);
-  double sigma = spectral_radius(sys, y, f0, v, false, flag, wjm1, fj);
-  bool sigma_fresh = true, need_sigma = false;
-  int since_sigma = 0;
-
-  /* initial step: Eq. 36-38 (R14, R15) */
-  double h;
-  {
-    const double h0 = (sigma > 0.0 && 1.0 / sigma < Dt) ? 1.0 / sigma : Dt;
-#pragma unroll
-    for (int i = 0; i < NV; i++) wjm1[i] = fma(h0, f0[i], y[i]);
-    sys.rhs(wjm1, fj);
-    double acc = 0.0;
+      for (int i = 0; i < NV; i++) v[i] = f0[i];
+    }
+    double a = 0.0, b = 0.0;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      if (sys.valid(i)) {
-        const double d0 = h0 * (fj[i] - f0[i]);
-        const double wt = fma(rtol, fabs(y[i]), atol);
-        const double q = d0 / wt;
-        acc = fma(q, q, acc);
-      }
+      a = fma(y[i], y[i], a);
+      b = fma(v[i], v[i], b);
     }
-    const double est = sqrt(sys.gsum(acc) / nd);
-    h = Dt;
-    if (est > 0.0) {
-      const double h1 = 0.1 * h0 / sqrt(est);
-      if (h1 < Dt) h = h1;
+    const double ynrm = sqrt(sys.gsum(a)), vnrm = sqrt(sys.gsum(b));
+    if (ynrm != 0.0 && vnrm != 0.0) {
+      pm_d = ynrm * CKB_SQRTU;
+      const double r = pm_d / vnrm;
+#pragma unroll
+      for (int i = 0; i < NV; i++) w[i] = fma(v[i], r, y[i]);
+    } else if (ynrm != 0.0) {
+      pm_d = ynrm * CKB_SQRTU;
+#pragma unroll
+      for (int i = 0; i < NV; i++) w[i] = y[i] * (1.0 + CKB_SQRTU);
+    } else if (vnrm != 0.0) {
+      pm_d = CKB_U;
+      const double r = pm_d / vnrm;
+#pragma unroll
+      for (int i = 0; i < NV; i++) w[i] = v[i] * r;
+    } else {
+      pm_d = CKB_U;
+#pragma unroll
+      for (int i = 0; i < NV; i++) w[i] = sys.valid(i) ? pm_d : 0.0;
     }
+    pm_sigma = 0.0;
+    pm_it = 1;
+    pm_initial = initial;
+    state = S_PM;
   }
 
-  bool have_prev = false, saw_nonfinite = false;
-  double err_old = 0.0, h_old = 0.0;
-  int attempts = 0;
-  while (true) {
-    bool last = false;
-    if (1.1 * h >= t1 - t) { /* R5 */
+  /* R5 clip, R16 refresh check (the clip is not redone after a refresh) */
+  __device__ __forceinline__ bool begin_step(const S &sys) {
+    last = false;
+    if (1.1 * h >= t1 - t) {
       h = t1 - t;
       last = true;
     }
-    if (need_sigma) { /* P:233, R16 */
-      sigma = spectral_radius(sys, y, f0, v, true, flag, wjm1, fj);
-      sigma_fresh = true;
-      need_sigma = false;
-      since_sigma = 0;
+    if (need_sigma) {
+      pm_begin(sys, true, false);
+      return false;
     }
-    int s = 1 + (int)floor(sqrt(fma(1.54 * h, sigma, 1.0))); /* Eq. 39, R12 */
+    return take_step();
+  }
+
+  /* Eq. 39 (R12), coefficients for j = 1, 2 (Eq. 22-26, R8-R10), first stage Eq. 19; true = failed */
+  __device__ __forceinline__ bool take_step() {
+    s = 1 + (int)floor(sqrt(fma(1.54 * h, sigma, 1.0)));
     if (s < 2) s = 2;
     if (s > s_max) {
       s = s_max;
@@ -435,75 +435,157 @@ __device__ __forceinline__ int rkc_driver(S &sys, double (&y)[S::NV], double t0,
     if (s > smax_used) smax_used = s;
     if (++attempts > 1000000) {
       status = ST_MAXSTEPS;
-      break;
+      return true;
     }
-    /* coefficients, Eq. 22-26: w0 (R8), then w1 = T_s'(w0)/T_s''(w0) by a scalar pre-pass */
-    const double w0 = 1.0 + (2.0 / 13.0) / ((double)s * (double)s);
-    double w1;
+    w0 = 1.0 + (2.0 / 13.0) / ((double)s * (double)s);
     {
-      double Tm2 = 1.0, Tm1 = w0, dm2 = 0.0, dm1 = 1.0, em2 = 0.0, em1 = 0.0;
-      for (int j = 2; j <= s; j++) {
+      double a2 = 1.0, a1 = w0, b2 = 0.0, b1 = 1.0, c2 = 0.0, c1 = 0.0;
+      for (int q = 2; q <= s; q++) { /* T_s'(w0), T_s''(w0) */
+        const double Tq = 2.0 * w0 * a1 - a2;
+        const double dq = 2.0 * a1 + 2.0 * w0 * b1 - b2;
+        const double eq = 4.0 * b1 + 2.0 * w0 * c1 - c2;
+        a2 = a1; a1 = Tq; b2 = b1; b1 = dq; c2 = c1; c1 = eq;
+      }
+      w1 = b1 / c1; /* Eq. 25 */
+    }
+    Tm2 = 1.0; Tm1 = w0; dm2 = 0.0; dm1 = 1.0; em2 = 0.0; em1 = 0.0;
+    const double d2 = 2.0 * Tm1 + 2.0 * w0 * dm1 - dm2, e2 = 4.0 * dm1;
+    const double b2 = e2 / (d2 * d2);
+    bjm2 = b2; bjm1 = b2;      /* R10: b_0 = b_1 = b_2 */
+    ajm1 = 1.0 - bjm1 * w0;    /* R9 */
+    const double mh = bjm1 * w1 * h; /* Eq. 22 */
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
+      wjm2[i] = y[i];
+      w[i] = fma(mh, f0[i], y[i]); /* Eq. 19 */
+    }
+    j = 2;
+    state = S_STAGE;
+    return false;
+  }
+
+  __device__ __forceinline__ bool advance(const S &sys, const double (&f)[NV]) {
+    nfe++;
+    switch (state) {
+      case S_F0: {
+#pragma unroll
+        for (int i = 0; i < NV; i++) f0[i] = f[i];
+        pm_begin(sys, false, true);
+        return false;
+      }
+      case S_PM: { /* R17 step 3-5 */
+        double dd = 0.0;
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+          const double e = f[i] - f0[i];
+          dd = fma(e, e, dd);
+        }
+        dd = sqrt(sys.gsum(dd));
+        const double sigma_prev = pm_sigma;
+        pm_sigma = dd / pm_d;
+        const double fl = pm_sigma > 1e-300 ? pm_sigma : 1e-300;
+        const bool conv = pm_it >= 2 && fabs(pm_sigma - sigma_prev) <= 0.01 * fl;
+        if (!conv && pm_it < 50) {
+          if (dd != 0.0) {
+            const double r = pm_d / dd;
+#pragma unroll
+            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0[i], r, y[i]);
+          } else {
+            const int ci = pm_it % (int)nd;
+#pragma unroll
+            for (int i = 0; i < NV; i++)
+              if (sys.g + S::L * i == ci) w[i] = y[i] - (w[i] - y[i]);
+          }
+          pm_it++;
+          return false;
+        }
+        if (!conv) {
+          flag = ST_SIGMA;
+          /* R17: z is updated once more after the 50th evaluation before v is saved */
+          if (dd != 0.0) {
+            const double r = pm_d / dd;
+#pragma unroll
+            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0[i], r, y[i]);
+          } else {
+            const int ci = pm_it % (int)nd;
+#pragma unroll
+            for (int i = 0; i < NV; i++)
+              if (sys.g + S::L * i == ci) w[i] = y[i] - (w[i] - y[i]);
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < NV; i++) v[i] = w[i] - y[i];
+        sigma = 1.2 * pm_sigma; /* R18 */
+        sigma_fresh = true;
+        need_sigma = false;
+        since_sigma = 0;
+        if (!pm_initial) return take_step();
+        /* initial step, Eq. 36-37 (R14, R15): probe f(y + h0 f0) */
+        h_old = (sigma > 0.0 && 1.0 / sigma < Dt) ? 1.0 / sigma : Dt; /* h0, parked in h_old */
+#pragma unroll
+        for (int i = 0; i < NV; i++) w[i] = fma(h_old, f0[i], y[i]);
+        state = S_H0;
+        return false;
+      }
+      case S_H0: { /* Eq. 37-38 */
+        const double h0 = h_old;
+        double acc = 0.0;
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+          if (sys.valid(i)) {
+            const double d0 = h0 * (f[i] - f0[i]);
+            const double wt = fma(rtol, fabs(y[i]), atol);
+            const double q = d0 / wt;
+            acc = fma(q, q, acc);
+          }
+        }
+        const double est = sqrt(sys.gsum(acc) / nd);
+        h = Dt;
+        if (est > 0.0) {
+          const double h1 = 0.1 * h0 / sqrt(est);
+          if (h1 < Dt) h = h1;
+        }
+        h_old = 0.0;
+        return begin_step(sys);
+      }
+      case S_STAGE: { /* Eq. 20, 23-24, 26 */
         const double Tj = 2.0 * w0 * Tm1 - Tm2;
         const double dj = 2.0 * Tm1 + 2.0 * w0 * dm1 - dm2;
         const double ej = 4.0 * dm1 + 2.0 * w0 * em1 - em2;
-        Tm2 = Tm1; Tm1 = Tj; dm2 = dm1; dm1 = dj; em2 = em1; em1 = ej;
-      }
-      w1 = dm1 / em1;
-    }
-    /* Eq. 18-21 */
-    {
-      /* j = 2 values: T_2 = 2 w0^2 - 1, T_2' = 4 w0, T_2'' = 4 */
-      double Tm2 = 1.0, Tm1 = w0, dm2 = 0.0, dm1 = 1.0, em2 = 0.0, em1 = 0.0;
-      const double T2 = 2.0 * w0 * Tm1 - Tm2, d2 = 2.0 * Tm1 + 2.0 * w0 * dm1 - dm2, e2 = 4.0 * dm1;
-      const double b2 = e2 / (d2 * d2);
-      double bjm2 = b2, bjm1 = b2;           /* R10: b_0 = b_1 = b_2 */
-      double ajm1 = 1.0 - bjm1 * w0;         /* R9: a_1 = 1 - b_1 T_1(w0) */
-      const double mut1 = bjm1 * w1;         /* Eq. 22 */
-#pragma unroll
-      for (int i = 0; i < NV; i++) {
-        wjm2[i] = y[i];
-        wjm1[i] = fma(mut1 * h, f0[i], y[i]); /* Eq. 19 */
-      }
-      for (int j = 2; j <= s; j++) {
-        double Tj, dj, ej;
-        if (j == 2) { Tj = T2; dj = d2; ej = e2; }
-        else {
-          Tj = 2.0 * w0 * Tm1 - Tm2;
-          dj = 2.0 * Tm1 + 2.0 * w0 * dm1 - dm2;
-          ej = 4.0 * dm1 + 2.0 * w0 * em1 - em2;
-        }
-        const double bj = ej / (dj * dj);                 /* Eq. 24 */
-        const double mu = 2.0 * bj * w0 / bjm1;           /* Eq. 23 */
+        const double bj = ej / (dj * dj);
+        const double mu = 2.0 * bj * w0 / bjm1;
         const double nu = -bj / bjm2;
         const double mut = 2.0 * bj * w1 / bjm1;
         const double gamt = -ajm1 * mut;
-        sys.rhs(wjm1, fj);
         const double c0 = 1.0 - mu - nu, mh = mut * h, gh = gamt * h;
 #pragma unroll
-        for (int i = 0; i < NV; i++) {                    /* Eq. 20 */
-          const double wj = fma(gh, f0[i], fma(mh, fj[i], fma(nu, wjm2[i], fma(mu, wjm1[i], c0 * y[i]))));
-          wjm2[i] = wjm1[i];
-          wjm1[i] = wj;
+        for (int i = 0; i < NV; i++) {
+          const double wj = fma(gh, f0[i], fma(mh, f[i], fma(nu, wjm2[i], fma(mu, w[i], c0 * y[i]))));
+          wjm2[i] = w[i];
+          w[i] = wj;
         }
         ajm1 = 1.0 - bj * Tj;
         bjm2 = bjm1; bjm1 = bj;
         Tm2 = Tm1; Tm1 = Tj; dm2 = dm1; dm1 = dj; em2 = em1; em1 = ej;
+        if (++j > s) state = S_FINAL;
+        return false;
       }
+      default:
+        break;
     }
-    sys.rhs(wjm1, fj); /* f(y_{n+1}) */
-    /* Eq. 30-32 */
+    /* S_FINAL: f = f(y_{n+1}), y_{n+1} = w.  Eq. 30-35 */
     double acc = 0.0;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       if (sys.valid(i)) {
-        const double del = fma(0.8, y[i] - wjm1[i], 0.4 * h * (f0[i] + fj[i]));
-        const double wt = fma(rtol, fmax(fabs(y[i]), fabs(wjm1[i])), atol);
+        const double del = fma(0.8, y[i] - w[i], 0.4 * h * (f0[i] + f[i]));
+        const double wt = fma(rtol, fmax(fabs(y[i]), fabs(w[i])), atol);
         const double q = del / wt;
         acc = fma(q, q, acc);
       }
     }
     const double err = sqrt(sys.gsum(acc) / nd);
-    if (err <= 1.0) { /* accept */
+    if (err <= 1.0) {
       nacc++;
       double fac;
       if (err > 0.0) {
@@ -514,115 +596,146 @@ __device__ __forceinline__ int rkc_driver(S &sys, double (&y)[S::NV], double t0,
       fac = fmin(10.0, fmax(0.1, fac)); /* Eq. 33 */
 #pragma unroll
       for (int i = 0; i < NV; i++) {
-        y[i] = wjm1[i];
-        f0[i] = fj[i];
+        y[i] = w[i];
+        f0[i] = f[i];
       }
       err_old = err;
       h_old = h;
       have_prev = true;
       sigma_fresh = false;
       if (++since_sigma >= 25) need_sigma = true;
-      if (last) break;
+      if (last) return true;
       t += h;
       h *= fac;
-    } else { /* reject: Eq. 35 */
-      nrej++;
-      double fac;
-      if (isfinite(err)) fac = fmin(10.0, fmax(0.1, 0.8 / cbrt(err)));
-      else {
-        fac = 0.1;
-        saw_nonfinite = true;
-      }
-      h *= fac;
-      have_prev = false;
-      if (!sigma_fresh) need_sigma = true; /* R16 */
-      const double tmax = fmax(fabs(t), fabs(t1));
-      if (!(h > 10.0 * CKB_U * tmax)) {
-        status = saw_nonfinite ? ST_NONFINITE : ST_UNDERFLOW;
-        break;
-      }
+      return begin_step(sys);
     }
+    nrej++;
+    double fac;
+    if (isfinite(err)) fac = fmin(10.0, fmax(0.1, 0.8 / cbrt(err))); /* Eq. 35 */
+    else {
+      fac = 0.1;
+      saw_nonfinite = true;
+    }
+    h *= fac;
+    have_prev = false;
+    if (!sigma_fresh) need_sigma = true; /* R16 */
+    const double tmax = fmax(fabs(t), fabs(t1));
+    if (!(h > 10.0 * CKB_U * tmax)) {
+      status = saw_nonfinite ? ST_NONFINITE : ST_UNDERFLOW;
+      return true;
+    }
+    return begin_step(sys);
   }
-  if (status == ST_OK && flag) status = flag;
-  st[0] = sys.nfe;
-  st[1] = nacc;
-  st[2] = nrej;
-  st[3] = smax_used;
-  return status;
-}
+
+  __device__ __forceinline__ void result(int (&st)[4]) {
+    if (status == ST_OK && flag) status = flag;
+    st[0] = nfe; st[1] = nacc; st[2] = nrej; st[3] = smax_used;
+  }
+};
 
 /* ------------------------------------------------------------------------------------------------
- * Kernels.  Block = CKB_BLOCK threads; a warp holds G = 32/L systems.
+ * Kernels.  Block = CKB_BLOCK threads; a warp holds G = 32/L systems at a time.
  * Shared memory per warp: (K+1 + NTB+1 + NS) * G doubles.
+ *
+ * integrate_kernel is persistent: the grid is sized to the resident capacity of the GPU (a multiple of the
+ * SM count) and every group of L lanes pulls system indices -- first its own global group index, then
+ * from an atomic counter -- until the batch is exhausted.  In the thread-per-ODE mapping this is "lane
+ * refill": a lane whose system has finished fetches the next one while its warp neighbours are still
+ * sub-stepping, so finished lanes never idle behind a slow neighbour (divergence control).
  * ---------------------------------------------------------------------------------------------- */
 #define CKB_BLOCK 128
 
 template <class S>
-__device__ __forceinline__ bool sys_setup(S &sys, const DevMech &m, double *smem, long long N, long long &ode) {
+__device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem) {
   constexpr int L = S::L, G = S::G;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int grp = lane / L;
   sys.g = lane % L;
   sys.src0 = grp * L;
   sys.mask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (grp * L));
-  ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + warp) * G + grp;
   const int per_warp = (m.K + 1 + m.NTB + 1 + m.NS) * G;
   double *base = smem + (size_t)warp * per_warp + grp;
   sys.sC = base;
   sys.sM = base + (m.K + 1) * G;
   sys.sQ = base + (m.K + 1 + m.NTB + 1) * G;
-  sys.nfe = 0;
-  if (ode >= N) return false;
   if (sys.g == 0) {
     sys.sC[m.K * G] = 1.0;   /* "absent molecule" concentration */
     sys.sM[m.NTB * G] = 1.0; /* "no third body" */
   }
   sys.gsync();
-  return true;
 }
+
+template <class S, int METHOD>
+struct IntegratorOf { typedef Rkck<S> type; };
+template <class S>
+struct IntegratorOf<S, 1> { typedef Rkc<S> type; };
 
 template <int L, int NV, class TAB, int METHOD>
 __global__ void __launch_bounds__(CKB_BLOCK)
-integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, double *__restrict__ states, const double *__restrict__ pressure,
-                 double p_uniform, long long N, long long ld, double t0, double dt, double rtol, double atol,
-                 int *__restrict__ status, int *__restrict__ stats) {
+integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, double *__restrict__ states,
+                 const double *__restrict__ pressure, double p_uniform, long long N, long long ld, double t0,
+                 double dt, double rtol, double atol, int *__restrict__ status, int *__restrict__ stats,
+                 unsigned long long *__restrict__ counter) {
   extern __shared__ double smem[];
-  Sys<L, NV, TAB> sys(m, tab);
-  long long ode;
-  if (!sys_setup(sys, m, smem, N, ode)) return;
-  sys.p = pressure ? pressure[ode] : p_uniform;
-  double y[NV];
+  typedef Sys<L, NV, TAB> S;
+  S sys(m, tab);
+  sys_setup(sys, m, smem);
+  constexpr int G = S::G;
+  const long long n_groups = (long long)gridDim.x * (CKB_BLOCK / 32) * G;
+  long long ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L;
+  typename IntegratorOf<S, METHOD>::type integ;
+  bool need_load = true;
+  double f[NV];
+  while (true) {
+    if (need_load) {
+      if (ode >= N) break;
+      sys.p = pressure ? pressure[ode] : p_uniform;
+      double y0[NV];
 #pragma unroll
-  for (int i = 0; i < NV; i++) {
-    const int c = sys.g + L * i;
-    y[i] = (c < m.n) ? states[(size_t)c * ld + ode] : 0.0;
-  }
-  int st[4];
-  int code;
-  if (METHOD == 0) code = rkck_driver(sys, y, t0, t0 + dt, rtol, atol, st);
-  else code = rkc_driver(sys, y, t0, t0 + dt, rtol, atol, st);
+      for (int i = 0; i < NV; i++) {
+        const int c = sys.g + L * i;
+        y0[i] = (c < m.n) ? states[(size_t)c * ld + ode] : 0.0;
+      }
+      integ.start(y0, t0, t0 + dt, rtol, atol, m.n);
+      need_load = false;
+    }
+    sys.rhs(integ.w, f);
+    if (integ.advance(sys, f)) {
+      int st[4];
+      integ.result(st);
 #pragma unroll
-  for (int i = 0; i < NV; i++) {
-    const int c = sys.g + L * i;
-    if (c < m.n) states[(size_t)c * ld + ode] = y[i];
-  }
-  if (sys.g == 0) {
-    if (status) status[ode] = code;
-    if (stats) {
+      for (int i = 0; i < NV; i++) {
+        const int c = sys.g + L * i;
+        if (c < m.n) states[(size_t)c * ld + ode] = integ.y[i];
+      }
+      if (sys.g == 0) {
+        if (status) status[ode] = integ.status;
+        if (stats) {
 #pragma unroll
-      for (int q = 0; q < 4; q++) stats[(size_t)q * N + ode] = st[q];
+          for (int q = 0; q < 4; q++) stats[(size_t)q * N + ode] = st[q];
+        }
+      }
+      /* next system: lane refill (L = 1) / group refill */
+      unsigned long long nx = 0;
+      if (sys.g == 0) nx = atomicAdd(counter, 1ull);
+      if (L > 1) nx = __shfl_sync(sys.mask, nx, sys.src0);
+      ode = n_groups + (long long)nx;
+      need_load = true;
     }
   }
 }
 
 template <int L, int NV, class TAB>
 __global__ void __launch_bounds__(CKB_BLOCK)
-rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, const double *__restrict__ states, const double *__restrict__ pressure,
-           double p_uniform, long long N, long long ld, double *__restrict__ dydt, int repeat) {
+rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, const double *__restrict__ states,
+           const double *__restrict__ pressure, double p_uniform, long long N, long long ld,
+           double *__restrict__ dydt, int repeat) {
   extern __shared__ double smem[];
-  Sys<L, NV, TAB> sys(m, tab);
-  long long ode;
-  if (!sys_setup(sys, m, smem, N, ode)) return;
+  typedef Sys<L, NV, TAB> S;
+  S sys(m, tab);
+  sys_setup(sys, m, smem);
+  const long long ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * S::G + (threadIdx.x & 31) / L;
+  if (ode >= N) return;
   sys.p = pressure ? pressure[ode] : p_uniform;
   double y[NV], f[NV];
 #pragma unroll

@@ -5,6 +5,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdint>
 #include <string>
 #include <vector>
@@ -31,8 +32,13 @@ struct ckb_mech {
   double *ws_states = nullptr, *ws_pressure = nullptr;
   int32_t *ws_status = nullptr, *ws_stats = nullptr;
   size_t ws_states_cap = 0, ws_n_cap = 0;
+  /* work-queue counters of the persistent kernels: a ring, one slot per launch in flight */
+  unsigned long long *d_counters = nullptr;
+  mutable std::atomic<unsigned> next_counter{0};
 };
 
+
+#define CKB_COUNTER_RING 256
 
 namespace ckb_host {
 

@@ -52,12 +52,25 @@ int launch(const ckb_mech *m, const IntegrateArgs &a) {
   const size_t smem = smem_bytes(m);
   int rc = prep(kern, smem);
   if (rc) return rc;
-  const long long blocks = n_blocks(a.N);
-  if (blocks > 2147483647LL) return CKB_EINVAL;
+  /* persistent grid: resident capacity of the device (a multiple of the SM count), capped by the batch */
+  static int resident = 0, resident_smem = -1; /* per instantiation */
+  if (resident == 0 || resident_smem != (int)smem) {
+    int dev = 0, sms = 0, per_sm = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, CKB_BLOCK, smem));
+    if (per_sm < 1) return CKB_EUNSUPPORTED;
+    resident = sms * per_sm;
+    resident_smem = (int)smem;
+  }
+  long long blocks = n_blocks(a.N);
+  if (blocks > resident) blocks = resident;
+  unsigned long long *counter = m->d_counters + (m->next_counter.fetch_add(1) % CKB_COUNTER_RING);
+  CK(cudaMemsetAsync(counter, 0, 8, a.stream));
   Tab tab;
   make_tab(m, tab);
   kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(m->dm, tab, a.states, a.pressure, a.p_uniform, a.N, a.ld,
-                                                       a.t, a.dt, a.rtol, a.atol, a.status, a.stats);
+                                                       a.t, a.dt, a.rtol, a.atol, a.status, a.stats, counter);
   CK(cudaGetLastError());
   return CKB_OK;
 }
