@@ -2,15 +2,16 @@
  * ckb_device.cuh -- device code of the batched chemistry integrator (sm_100a, FP64).
  *
  * One templated "system" type maps an ODE system onto L lanes (L = 1: thread-per-ODE, the paper's
- * mapping P:255; L = 32: warp-per-ODE; L = 8/16: sub-warp).  Component c of y = {T, Y_1..Y_K}
- * lives in lane (c mod L), register slot (c div L); every stage vector of the integrators is a
- * register array double[NV] with static indexing only.  The runtime-indexed quantities of the source
- * term (concentrations C_k, third-body concentrations [M], net rates of progress q_s) live in shared
- * memory, interleaved so that thread-per-ODE access is bank-conflict free.
+ * mapping P:255; L = 32: warp-per-ODE; L = 8/16: sub-warp).  Component c of the (renumbered, see
+ * ckb_tables.h) unknowns {T, Y_1..Y_K} lives in lane (c mod L), register slot (c div L); every
+ * stage vector of the integrators is a register array double[NV] with static indexing only.  The
+ * runtime-indexed quantities of the source term (concentrations C_c, third-body concentrations [M], net
+ * rates of progress q_s) live in shared memory, interleaved so that thread-per-ODE access is
+ * bank-conflict free.
  *
  * Source term: Eq. 2-6.  Integrators: RKCK Eq. 7-17, RKC Eq. 18-39.
  * The readings of the paper where it is silent (R-numbers) are listed in DESIGN.md section 4.
- * Nothing here is shared with oracle/ (constants that appear in both are typed twice).
+ * Nothing here is shared with the CPU checker (constants that appear in both are typed twice).
  */
 #pragma once
 #include <math.h>
@@ -23,24 +24,53 @@ namespace ckb {
 /* R20: physical constants */
 #define CKB_RU 8.314462618e7 /* erg/(mol K) */
 
+/* exp(x) for the Arrhenius coefficients (Eq. 5): x = k ln2 + r, |r| <= ln2/2; e^r = 1 + r + r^2 q(r) with
+ * q of degree 9 fitted at Chebyshev nodes (truncation 1.7e-17 relative); 2^k by exponent arithmetic with k
+ * clamped to the normal range, so x << -708 gives ~1e-308 (not 0, not NaN) and the code has no branch.
+ * The coefficients sit in the constant bank so that every DFMA takes its addend as a c[][] operand. */
+static __constant__ double c_expq[10] = {
+    0.5000000000000001,    0.16666666666666669,   0.041666666666623824,  0.008333333333330039,
+    0.0013888888917367081, 0.00019841269863171557, 2.4801521057868204e-05, 2.7557268276905696e-06,
+    2.7620201591031547e-07, 2.5100472505694996e-08};
+
+__device__ __forceinline__ double ckb_exp(double x) {
+  const double t = fma(x, 1.4426950408889634, 6755399441055744.0); /* 1.5 * 2^52: round to nearest integer */
+  const double kd = t - 6755399441055744.0;
+  double r = fma(kd, -0.6931471805599453, x);
+  r = fma(kd, -2.3190468138462996e-17, r);
+  double p = c_expq[9];
+#pragma unroll
+  for (int i = 8; i >= 0; i--) p = fma(p, r, c_expq[i]);
+  p = fma(p, r, 1.0);
+  p = fma(p, r, 1.0);
+  int k = __double2loint(t);
+  k = max(-1022, min(1023, k));
+  return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
 /* ------------------------------------------------------------------------------------------------
- * Sys<L, NV, CT>: one ODE system on L lanes with NV register slots per lane; tables in constant
- * memory (CT) or global/L1.
+ * Sys<L, NV, TAB>: one ODE system on L lanes with NV register slots per lane; tables from the kernel
+ * parameter bank (ParamTab) or global/L1 (GlobalTab).
  * ---------------------------------------------------------------------------------------------- */
 template <int L_, int NV_, class TAB>
 struct Sys {
   static constexpr int L = L_, NV = NV_, G = 32 / L_;
   const DevMech &m;
   const TAB &tab;
-  double *sC, *sM, *sQ; /* this group's shared arrays, element idx at [idx*G] */
-  unsigned mask;        /* lanes of this group */
-  int g;                /* lane within the group */
-  int src0;             /* warp lane that holds component 0 (T) */
-  double p;             /* pressure, dyn/cm^2 (R24: constant over the call) */
+  double *sR;      /* this system's shared region (ckb_tables.h), element e at sR[e*G] */
+  double *sQ;      /* = sR + (n + NTB + 1) * G */
+  unsigned mask;   /* lanes of this group */
+  int g;           /* lane within the group */
+  int src0;        /* warp lane that holds component 0 (T) */
+  double pR, Rp;   /* p / Ru and Ru / p (R24: pressure constant over the call) */
 
   __device__ __forceinline__ Sys(const DevMech &m_, const TAB &tab_) : m(m_), tab(tab_) {}
   __device__ __forceinline__ unsigned long long tw(int i) const { return tab.ld(i); }
   __device__ __forceinline__ double td(int i) const { return __longlong_as_double((long long)tab.ld(i)); }
+  __device__ __forceinline__ void set_pressure(double p) {
+    pR = p / CKB_RU;
+    Rp = CKB_RU / p;
+  }
 
   __device__ __forceinline__ void gsync() const {
     if (L > 1) __syncwarp(mask);
@@ -63,91 +93,86 @@ struct Sys {
 
   /* f(y): Eq. 2-6.  y, f: component (g + L*i) in slot i. */
   __device__ __forceinline__ void rhs(const double (&y)[NV], double (&f)[NV]) {
-    const int K = m.K;
+    const int n = m.n;
     const double T = bcast0(y[0]);
     const double invT = 1.0 / T;
     const double lnT = log(T);
     double s1 = 0.0, s2 = 0.0;
     double hrt[NV], yw[NV];
+    /* species table rows of T and of padding components are all zero: no branch needed */
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      const int c = g + L * i, k = c - 1;
-      hrt[i] = 0.0;
-      yw[i] = 0.0;
-      if (c >= 1 && c <= K) {
-        /* R8a: cp_k/R = a1 + a2 T + ... + a5 T^4;  h_k/(RT) = a1 + a2 T/2 + ... + a5 T^4/5 + a6/T */
-        double cp = td(m.o_cp + 4 * K + k);
-        double h = td(m.o_h + 4 * K + k);
+      const int b = m.o_sp + i * CKB_SP_WORDS * L + g;
+      /* R8a: cp_k/R = a1 + a2 T + ... + a5 T^4;  h_k/(RT) = a1 + a2 T/2 + ... + a5 T^4/5 + a6/T */
+      double cp = td(b + (CKB_SP_CP + 4) * L);
+      double h = td(b + (CKB_SP_H + 4) * L);
 #pragma unroll
-        for (int q = 3; q >= 0; q--) {
-          cp = fma(cp, T, td(m.o_cp + q * K + k));
-          h = fma(h, T, td(m.o_h + q * K + k));
-        }
-        h = fma(td(m.o_h + 5 * K + k), invT, h);
-        const double v = y[i] * td(m.o_invW + k); /* Y_k / W_k */
-        yw[i] = v;
-        hrt[i] = h;
-        s1 += v;
-        s2 = fma(v, cp, s2);
+      for (int q = 3; q >= 0; q--) {
+        cp = fma(cp, T, td(b + (CKB_SP_CP + q) * L));
+        h = fma(h, T, td(b + (CKB_SP_H + q) * L));
       }
+      h = fma(td(b + (CKB_SP_H + 5) * L), invT, h);
+      const double v = y[i] * td(b + CKB_SP_INVW * L); /* Y_k / W_k */
+      yw[i] = v;
+      hrt[i] = h;
+      s1 += v;
+      s2 = fma(v, cp, s2);
     }
     s1 = gsum(s1);
     s2 = gsum(s2);
     /* R9a: ideal gas at constant pressure: rho = p / (Ru T sum_k Y_k/W_k), C_k = rho Y_k / W_k */
-    const double ctot = p / (CKB_RU * T);
-    const double rho = ctot / s1;
+    const double ctot = pR * invT;
+    const double rho = ctot * (1.0 / s1);
+    const double invrho = s1 * T * Rp;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       const int c = g + L * i;
-      if (c >= 1 && c <= K) sC[(c - 1) * G] = rho * yw[i];
+      if (c >= 1 && c < n) sR[c * G] = rho * yw[i];
     }
     gsync();
     /* R22: [M] = sum_k alpha_k C_k = C_tot + sum_listed (alpha_k - 1) C_k, one value per efficiency set */
-    for (int t = g; t < m.NTB; t += L) {
-      const int e0 = (int)tw(m.o_tbptr + t), e1 = (int)tw(m.o_tbptr + t + 1);
+    for (int r = 0; r < m.NTBR; r++) {
       double M = ctot;
-      for (int e = e0; e < e1; e++)
-        M = fma(td(m.o_tbam1 + e), sC[(int)tw(m.o_tbsp + e) * G], M);
-      sM[t * G] = M;
+      int b = m.o_tb + r * m.TBE * 2 * L + g;
+      for (int e = 0; e < m.TBE; e++, b += 2 * L) M = fma(td(b), sR[(int)tw(b + L)], M);
+      const int t = r * L + g;
+      if (t < m.NTB) sR[(n + t) * G] = M;
     }
     gsync();
-    /* Eq. 4-5: q_s = [M] (k_f prod C_reactants - k_r prod C_products); absent molecules point at C = 1 */
-#pragma unroll 2
-    for (int s = g; s < m.NS; s += L) {
-      const unsigned long long w = tw(m.o_idx + s);
-      const double xf = fma(td(m.o_bf + s), lnT, td(m.o_lnAf + s)) -
-                        td(m.o_thf + s) * invT;
-      const double xr = fma(td(m.o_br + s), lnT, td(m.o_lnAr + s)) -
-                        td(m.o_thr + s) * invT;
-      const unsigned lo = (unsigned)w, hi = (unsigned)(w >> 32);
-      const double pf = sC[(lo & 255u) * G] * sC[((lo >> 8) & 255u) * G] * sC[((lo >> 16) & 255u) * G];
-      const double pr = sC[(lo >> 24) * G] * sC[(hi & 255u) * G] * sC[((hi >> 8) & 255u) * G];
-      const double kf = exp(xf), kr = exp(xr);
-      sQ[s * G] = (kf * pf - kr * pr) * sM[(hi >> 16) * G];
+    /* Eq. 4-5: q_s = [M] (k_f prod C_reactants - k_r prod C_products); absent molecules point at C_0 = 1 */
+    {
+      int b = m.o_sl + g;
+      double *q = sQ + g * G;
+      for (int r = 0; r < m.NSR; r++, b += CKB_SL_WORDS * L, q += L * G) {
+        const double xf = fma(-td(b + CKB_SL_THF * L), invT, fma(td(b + CKB_SL_BF * L), lnT, td(b + CKB_SL_LNAF * L)));
+        const double xr = fma(-td(b + CKB_SL_THR * L), invT, fma(td(b + CKB_SL_BR * L), lnT, td(b + CKB_SL_LNAR * L)));
+        const unsigned long long wa = tw(b + CKB_SL_IDXA * L), wb = tw(b + CKB_SL_IDXB * L);
+        const unsigned alo = (unsigned)wa, ahi = (unsigned)(wa >> 32), blo = (unsigned)wb, bhi = (unsigned)(wb >> 32);
+        const double pf = sR[alo & 0xFFFFu] * sR[alo >> 16] * sR[ahi & 0xFFFFu];
+        const double pr = sR[blo & 0xFFFFu] * sR[blo >> 16] * sR[bhi & 0xFFFFu];
+        const double kf = ckb_exp(xf), kr = ckb_exp(xr);
+        *q = (kf * pf - kr * pr) * sR[ahi >> 16];
+      }
     }
     gsync();
-    /* Eq. 3: omega_k = sum_s (nu''_ks - nu'_ks) q_s (gather);  Eq. 2: dY_k/dt = W_k omega_k / rho */
-    const double invrho = 1.0 / rho;
+    /* Eq. 3: omega_c = sum_s (nu''_cs - nu'_cs) q_s (gather);  Eq. 2: dY_k/dt = W_k omega_k / rho */
     double s3 = 0.0;
+    int gp = m.o_gat + g;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      const int c = g + L * i, k = c - 1;
-      f[i] = 0.0;
-      if (c >= 1 && c <= K) {
-        const int e0 = (int)tw(m.o_gptr + k), e1 = (int)tw(m.o_gptr + k + 1);
-        double acc = 0.0;
-        for (int e = e0; e < e1; e++) {
-          const unsigned long long w = tw(m.o_gat + e);
-          const double coef = __longlong_as_double((long long)(w & ~0xFFFFull));
-          acc = fma(coef, sQ[(int)(w & 0xFFFFull) * G], acc);
-        }
-        f[i] = td(m.o_W + k) * acc * invrho;
-        s3 = fma(hrt[i], acc, s3);
+      const int len = (int)tw(m.o_glen + i);
+      double acc = 0.0;
+      for (int t = 0; t < len; t++, gp += L) {
+        const unsigned long long w = tw(gp);
+        const double coef = __longlong_as_double((long long)(w & ~0xFFFFull));
+        acc = fma(coef, sQ[(unsigned)w & 0xFFFFu], acc);
       }
+      f[i] = td(m.o_sp + i * CKB_SP_WORDS * L + g + CKB_SP_W * L) * acc * invrho;
+      s3 = fma(hrt[i], acc, s3);
     }
     s3 = gsum(s3);
     /* Eq. 6: dT/dt = -(Ru T sum_k (h_k/RT) omega_k) / (rho cp), cp = Ru sum_k Y_k (cp_k/R) / W_k */
-    if (g == 0) f[0] = -(T * s3) / (rho * s2);
+    if (g == 0) f[0] = -(T * s3 * invrho) / s2;
   }
 };
 
@@ -337,6 +362,34 @@ struct Rkck {
   }
 };
 
+/* RKC coefficients of stage j (2 <= j <= s) of an s-stage step, Eq. 22-26 with R8-R10, computed from scratch
+ * (O(s) scalar work; used only above the precomputed table, s > s_tab, where f(y) costs far more). */
+static __device__ __noinline__ void rkc_coefficients(int s, int j, double &mut1, double &mu, double &nu, double &mut,
+                                              double &gamt) {
+  const double w0 = 1.0 + (2.0 / 13.0) / ((double)s * (double)s);
+  double Tm2 = 1.0, Tm1 = w0, dm2 = 0.0, dm1 = 1.0, em2 = 0.0, em1 = 0.0;
+  double b2 = 0.0, bj = 0.0, bjm1 = 0.0, bjm2 = 0.0, Tjm1 = w0;
+  for (int q = 2; q <= s; q++) {
+    const double Tq = 2.0 * w0 * Tm1 - Tm2;
+    const double dq = 2.0 * Tm1 + 2.0 * w0 * dm1 - dm2;
+    const double eq = 4.0 * dm1 + 2.0 * w0 * em1 - em2;
+    if (q == 2) b2 = eq / (dq * dq);
+    if (q == j - 2) bjm2 = eq / (dq * dq);
+    if (q == j - 1) { bjm1 = eq / (dq * dq); Tjm1 = Tq; }
+    if (q == j) bj = eq / (dq * dq);
+    Tm2 = Tm1; Tm1 = Tq; dm2 = dm1; dm1 = dq; em2 = em1; em1 = eq;
+  }
+  const double w1 = dm1 / em1; /* Eq. 25 */
+  if (j - 2 < 2) bjm2 = b2;    /* R10: b_0 = b_1 = b_2 */
+  if (j - 1 < 2) { bjm1 = b2; Tjm1 = w0; }
+  const double ajm1 = 1.0 - bjm1 * Tjm1; /* R9 */
+  mut1 = b2 * w1;
+  mu = 2.0 * bj * w0 / bjm1;
+  nu = -bj / bjm2;
+  mut = 2.0 * bj * w1 / bjm1;
+  gamt = -ajm1 * mut;
+}
+
 /* RKC: Eq. 18-39 and P:233; R8-R18, R26.  Spectral radius by the nonlinear power method (R17/R18). */
 template <class S>
 struct Rkc {
@@ -348,8 +401,7 @@ struct Rkc {
   double t, h, t1, Dt, rtol, atol, nd;
   double sigma, err_old, h_old;
   double pm_d, pm_sigma;                          /* power method: displacement size, last estimate */
-  double w0, w1, Tm1, Tm2, dm1, dm2, em1, em2, bjm1, bjm2, ajm1; /* Eq. 22-26 recurrences */
-  int state, j, s, s_max, pm_it;
+  int state, j, s, s_max, pm_it, cbase;           /* cbase: this step's rows of the coefficient table */
   int nfe, nacc, nrej, smax_used, attempts, since_sigma, status, flag;
   bool last, have_prev, saw_nonfinite, sigma_fresh, need_sigma, pm_initial;
 
@@ -420,11 +472,11 @@ struct Rkc {
       pm_begin(sys, true, false);
       return false;
     }
-    return take_step();
+    return take_step(sys);
   }
 
   /* Eq. 39 (R12), coefficients for j = 1, 2 (Eq. 22-26, R8-R10), first stage Eq. 19; true = failed */
-  __device__ __forceinline__ bool take_step() {
+  __device__ __forceinline__ bool take_step(const S &sys) {
     s = 1 + (int)floor(sqrt(fma(1.54 * h, sigma, 1.0)));
     if (s < 2) s = 2;
     if (s > s_max) {
@@ -437,23 +489,16 @@ struct Rkc {
       status = ST_MAXSTEPS;
       return true;
     }
-    w0 = 1.0 + (2.0 / 13.0) / ((double)s * (double)s);
-    {
-      double a2 = 1.0, a1 = w0, b2 = 0.0, b1 = 1.0, c2 = 0.0, c1 = 0.0;
-      for (int q = 2; q <= s; q++) { /* T_s'(w0), T_s''(w0) */
-        const double Tq = 2.0 * w0 * a1 - a2;
-        const double dq = 2.0 * a1 + 2.0 * w0 * b1 - b2;
-        const double eq = 4.0 * b1 + 2.0 * w0 * c1 - c2;
-        a2 = a1; a1 = Tq; b2 = b1; b1 = dq; c2 = c1; c1 = eq;
-      }
-      w1 = b1 / c1; /* Eq. 25 */
+    double mut1; /* Eq. 22 */
+    if (s <= sys.m.s_tab) {
+      mut1 = sys.td(sys.m.o_rkc + (s - 2));
+      cbase = sys.m.o_rkcs + 4 * ((s - 2) * (s - 1) / 2);
+    } else {
+      double mu, nu, mut, gamt;
+      rkc_coefficients(s, 2, mut1, mu, nu, mut, gamt);
+      cbase = -1;
     }
-    Tm2 = 1.0; Tm1 = w0; dm2 = 0.0; dm1 = 1.0; em2 = 0.0; em1 = 0.0;
-    const double d2 = 2.0 * Tm1 + 2.0 * w0 * dm1 - dm2, e2 = 4.0 * dm1;
-    const double b2 = e2 / (d2 * d2);
-    bjm2 = b2; bjm1 = b2;      /* R10: b_0 = b_1 = b_2 */
-    ajm1 = 1.0 - bjm1 * w0;    /* R9 */
-    const double mh = bjm1 * w1 * h; /* Eq. 22 */
+    const double mh = mut1 * h;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       wjm2[i] = y[i];
@@ -519,7 +564,7 @@ struct Rkc {
         sigma_fresh = true;
         need_sigma = false;
         since_sigma = 0;
-        if (!pm_initial) return take_step();
+        if (!pm_initial) return take_step(sys);
         /* initial step, Eq. 36-37 (R14, R15): probe f(y + h0 f0) */
         h_old = (sigma > 0.0 && 1.0 / sigma < Dt) ? 1.0 / sigma : Dt; /* h0, parked in h_old */
 #pragma unroll
@@ -549,14 +594,14 @@ struct Rkc {
         return begin_step(sys);
       }
       case S_STAGE: { /* Eq. 20, 23-24, 26 */
-        const double Tj = 2.0 * w0 * Tm1 - Tm2;
-        const double dj = 2.0 * Tm1 + 2.0 * w0 * dm1 - dm2;
-        const double ej = 4.0 * dm1 + 2.0 * w0 * em1 - em2;
-        const double bj = ej / (dj * dj);
-        const double mu = 2.0 * bj * w0 / bjm1;
-        const double nu = -bj / bjm2;
-        const double mut = 2.0 * bj * w1 / bjm1;
-        const double gamt = -ajm1 * mut;
+        double mu, nu, mut, gamt;
+        if (cbase >= 0) {
+          const int b = cbase + 4 * (j - 2);
+          mu = sys.td(b); nu = sys.td(b + 1); mut = sys.td(b + 2); gamt = sys.td(b + 3);
+        } else {
+          double mut1;
+          rkc_coefficients(s, j, mut1, mu, nu, mut, gamt);
+        }
         const double c0 = 1.0 - mu - nu, mh = mut * h, gh = gamt * h;
 #pragma unroll
         for (int i = 0; i < NV; i++) {
@@ -564,9 +609,6 @@ struct Rkc {
           wjm2[i] = w[i];
           w[i] = wj;
         }
-        ajm1 = 1.0 - bj * Tj;
-        bjm2 = bjm1; bjm1 = bj;
-        Tm2 = Tm1; Tm1 = Tj; dm2 = dm1; dm1 = dj; em2 = em1; em1 = ej;
         if (++j > s) state = S_FINAL;
         return false;
       }
@@ -635,7 +677,7 @@ struct Rkc {
 
 /* ------------------------------------------------------------------------------------------------
  * Kernels.  Block = CKB_BLOCK threads; a warp holds G = 32/L systems at a time.
- * Shared memory per warp: (K+1 + NTB+1 + NS) * G doubles.
+ * Shared memory per warp: region_doubles(m) * G doubles (ckb_tables.h).
  *
  * integrate_kernel is persistent: the grid is sized to the resident capacity of the GPU (a multiple of the
  * SM count) and every group of L lanes pulls system indices -- first its own global group index, then
@@ -653,14 +695,12 @@ __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem
   sys.g = lane % L;
   sys.src0 = grp * L;
   sys.mask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (grp * L));
-  const int per_warp = (m.K + 1 + m.NTB + 1 + m.NS) * G;
-  double *base = smem + (size_t)warp * per_warp + grp;
-  sys.sC = base;
-  sys.sM = base + (m.K + 1) * G;
-  sys.sQ = base + (m.K + 1 + m.NTB + 1) * G;
+  const int per_warp = region_doubles(m) * G;
+  sys.sR = smem + (size_t)warp * per_warp + grp;
+  sys.sQ = sys.sR + (m.n + m.NTB + 1) * G;
   if (sys.g == 0) {
-    sys.sC[m.K * G] = 1.0;   /* "absent molecule" concentration */
-    sys.sM[m.NTB * G] = 1.0; /* "no third body" */
+    sys.sR[0] = 1.0;                   /* "absent molecule" concentration */
+    sys.sR[(m.n + m.NTB) * G] = 1.0;   /* "no third body" */
   }
   sys.gsync();
 }
@@ -689,12 +729,12 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
   while (true) {
     if (need_load) {
       if (ode >= N) break;
-      sys.p = pressure ? pressure[ode] : p_uniform;
+      sys.set_pressure(pressure ? pressure[ode] : p_uniform);
       double y0[NV];
 #pragma unroll
       for (int i = 0; i < NV; i++) {
         const int c = sys.g + L * i;
-        y0[i] = (c < m.n) ? states[(size_t)c * ld + ode] : 0.0;
+        y0[i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode] : 0.0;
       }
       integ.start(y0, t0, t0 + dt, rtol, atol, m.n);
       need_load = false;
@@ -706,7 +746,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
 #pragma unroll
       for (int i = 0; i < NV; i++) {
         const int c = sys.g + L * i;
-        if (c < m.n) states[(size_t)c * ld + ode] = integ.y[i];
+        if (c < m.n) states[(size_t)sys.tw(m.o_perm + c) * ld + ode] = integ.y[i];
       }
       if (sys.g == 0) {
         if (status) status[ode] = integ.status;
@@ -736,12 +776,12 @@ rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, c
   sys_setup(sys, m, smem);
   const long long ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * S::G + (threadIdx.x & 31) / L;
   if (ode >= N) return;
-  sys.p = pressure ? pressure[ode] : p_uniform;
+  sys.set_pressure(pressure ? pressure[ode] : p_uniform);
   double y[NV], f[NV];
 #pragma unroll
   for (int i = 0; i < NV; i++) {
     const int c = sys.g + L * i;
-    y[i] = (c < m.n) ? states[(size_t)c * ld + ode] : 0.0;
+    y[i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode] : 0.0;
   }
   for (int r = 0; r < repeat; r++) {
     sys.rhs(y, f);
@@ -754,7 +794,7 @@ rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, c
 #pragma unroll
   for (int i = 0; i < NV; i++) {
     const int c = sys.g + L * i;
-    if (c < m.n) dydt[(size_t)c * ld + ode] = f[i];
+    if (c < m.n) dydt[(size_t)sys.tw(m.o_perm + c) * ld + ode] = f[i];
   }
 }
 

@@ -22,11 +22,25 @@ int cuda_fail(cudaError_t e, const char *what);
     if (e_ != cudaSuccess) return ckb_host::cuda_fail(e_, #call); \
   } while (0)
 
-struct ckb_mech {
+struct ckb_mech;
+namespace ckb_host {
+/* one packing of the mechanism per lanes-per-system value L (ckb_tables.h) */
+struct Packed {
   ckb::DevMech dm{};
   std::vector<unsigned long long> blob; /* host copy of the packed tables */
   unsigned long long *d_blob = nullptr;
-  int R = 0;
+  int rc = CKB_EUNSUPPORTED;            /* CKB_OK when this packing exists */
+};
+struct Parsed;
+int parse_mechanism(const ckb_mech_desc *d, Parsed &P);
+int pack_for(const Parsed &P, int L, Packed &out);
+int load_packings(const ckb_mech_desc *d, ckb_mech *m);
+inline int pack_index(int L) { return L == 1 ? 0 : L == 8 ? 1 : L == 16 ? 2 : 3; }
+}  // namespace ckb_host
+
+struct ckb_mech {
+  ckb_host::Packed pk[4]; /* L = 1, 8, 16, 32 */
+  int K = 0, R = 0, NS = 0;
   double flops_per_rhs = 0.0;
   /* grow-only device workspace of ckb_integrate_host */
   double *ws_states = nullptr, *ws_pressure = nullptr;
@@ -54,6 +68,17 @@ struct RhsArgs {
 /* the instantiation list: (lanes per system L, register slots per lane NV); a system needs K+1 <= L*NV */
 #define CKB_FOR_THREAD(X) X(1, 4) X(1, 10) X(1, 14) X(1, 16)
 #define CKB_FOR_GROUP(X) X(8, 7) X(8, 14) X(16, 4) X(16, 7) X(32, 1) X(32, 2) X(32, 4)
+
+/* smallest instantiated NV that holds n unknowns on L lanes, or -1 */
+inline int pick_nv(int L, int n) {
+  int best = -1;
+#define X(L_, NV_) \
+  if (L == L_ && n <= L_ * NV_ && (best < 0 || NV_ < best)) best = NV_;
+  CKB_FOR_THREAD(X)
+  CKB_FOR_GROUP(X)
+#undef X
+  return best;
+}
 
 #define CKB_DECL(L_, NV_)                                                                         \
   int integrate_L##L_##_NV##NV_(const ckb_mech *m, int method, const IntegrateArgs &a);           \

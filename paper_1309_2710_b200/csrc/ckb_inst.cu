@@ -26,28 +26,30 @@ typedef ckb::ParamTab Tab;
 typedef ckb::GlobalTab Tab;
 #endif
 
-size_t smem_bytes(const ckb_mech *m) {
-  const int G = 32 / L;
-  return (size_t)(m->dm.K + 1 + m->dm.NTB + 1 + m->dm.NS) * G * (CKB_BLOCK / 32) * sizeof(double);
+static const Packed &pack_of(const ckb_mech *m) { return m->pk[pack_index(L)]; }
+
+static size_t smem_bytes(const ckb_mech *m) {
+  const ckb::DevMech &dm = pack_of(m).dm;
+  return (size_t)ckb::region_doubles(dm) * (32 / L) * (CKB_BLOCK / 32) * sizeof(double);
 }
 
 template <class KERN>
-int prep(KERN kern, size_t smem) {
+static int prep(KERN kern, size_t smem) {
   if (smem > 227 * 1024) return CKB_EUNSUPPORTED;
   if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   return CKB_OK;
 }
 
-void make_tab(const ckb_mech *m, ckb::ParamTab &t) { std::memcpy(t.w, m->blob.data(), m->blob.size() * 8); }
-void make_tab(const ckb_mech *m, ckb::GlobalTab &t) { t.p = m->d_blob; }
+static void make_tab(const ckb_mech *m, ckb::ParamTab &t) { std::memcpy(t.w, pack_of(m).blob.data(), pack_of(m).blob.size() * 8); }
+static void make_tab(const ckb_mech *m, ckb::GlobalTab &t) { t.p = pack_of(m).d_blob; }
 
-long long n_blocks(long long N) {
+static long long n_blocks(long long N) {
   const long long per_block = (long long)(CKB_BLOCK / 32) * (32 / L);
   return (N + per_block - 1) / per_block;
 }
 
 template <int METHOD>
-int launch(const ckb_mech *m, const IntegrateArgs &a) {
+static int launch(const ckb_mech *m, const IntegrateArgs &a) {
   auto kern = ckb::integrate_kernel<L, NV, Tab, METHOD>;
   const size_t smem = smem_bytes(m);
   int rc = prep(kern, smem);
@@ -69,7 +71,7 @@ int launch(const ckb_mech *m, const IntegrateArgs &a) {
   CK(cudaMemsetAsync(counter, 0, 8, a.stream));
   Tab tab;
   make_tab(m, tab);
-  kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(m->dm, tab, a.states, a.pressure, a.p_uniform, a.N, a.ld,
+  kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(pack_of(m).dm, tab, a.states, a.pressure, a.p_uniform, a.N, a.ld,
                                                        a.t, a.dt, a.rtol, a.atol, a.status, a.stats, counter);
   CK(cudaGetLastError());
   return CKB_OK;
@@ -90,7 +92,7 @@ int CKB_CAT(rhs_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const RhsArgs &a) {
   if (blocks > 2147483647LL) return CKB_EINVAL;
   Tab tab;
   make_tab(m, tab);
-  kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(m->dm, tab, a.states, a.pressure, a.p_uniform, a.N, a.ld,
+  kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(pack_of(m).dm, tab, a.states, a.pressure, a.p_uniform, a.N, a.ld,
                                                        a.dydt, a.repeat);
   CK(cudaGetLastError());
   return CKB_OK;

@@ -1,9 +1,22 @@
 /*
  * ckb_tables.h -- layout of the packed mechanism, seen by the packer and the kernels.
+ *
+ * The mechanism is packed once per lanes-per-system value L (1, 8, 16, 32) because every table is
+ * "blocked SoA with block L": entry x of item (r*L + g) sits at word (r*X + x)*L + g, so that the L lanes
+ * of a group read X consecutive runs of L words with ONE address register and immediate offsets -- fully
+ * coalesced for L = 32, a broadcast for L = 1 (kernel-parameter / constant bank).
+ *
+ * Components are renumbered: c = 0 is T, c = 1..K are the species sorted by the length of their gather
+ * row (longest first), so that the rows handled in one gather level have similar lengths.
+ * Shared-memory region of one system (in doubles, element e of system-in-warp grp at [e*G + grp]):
+ *   [0, n)            C_c, concentration of component c; C_0 = 1.0 stands for "no molecule"
+ *   [n, n+NTB+1)      [M]_t per third-body efficiency set; the last one = 1.0 stands for "no third body"
+ *   [n+NTB+1, +NSR*L) q_s, net rate of progress of reaction slot s
  */
 #pragma once
 #ifndef __CUDACC__
 #define __device__
+#define __host__
 #define __forceinline__ inline
 #endif
 
@@ -19,26 +32,52 @@ struct ParamTab {
 };
 struct GlobalTab {
   const unsigned long long *p;
-  __device__ __forceinline__ unsigned long long ld(int i) const { 
+  __device__ __forceinline__ unsigned long long ld(int i) const {
 #ifdef __CUDA_ARCH__
     return __ldg(p + i);
 #else
     return p[i];
 #endif
-   }
+  }
 };
 
-/* Packed mechanism: one blob of 8-byte words, offsets in words. */
+/* species table: 13 words per component */
+#define CKB_SP_INVW 0 /* 1/W                                   */
+#define CKB_SP_W 1    /* W                                     */
+#define CKB_SP_CP 2   /* 5 words: a1..a5 (cp/R)                */
+#define CKB_SP_H 7    /* 6 words: a1, a2/2, .., a5/5, a6 (h/RT) */
+#define CKB_SP_WORDS 13
+/* slot table: 8 words per reaction slot */
+#define CKB_SL_LNAF 0
+#define CKB_SL_BF 1
+#define CKB_SL_THF 2
+#define CKB_SL_LNAR 3 /* -inf when the slot has no reverse reaction */
+#define CKB_SL_BR 4
+#define CKB_SL_THR 5
+#define CKB_SL_IDXA 6 /* 16-bit fields: region offsets (in doubles, x G) of reactant molecules 0,1,2 and of [M] */
+#define CKB_SL_IDXB 7 /* 16-bit fields: product molecules 0,1,2; field 3 unused                              */
+#define CKB_SL_WORDS 8
+
 struct DevMech {
-  int K, n, NS, NTB;
-  int o_invW, o_W;          /* [K] 1/W_k, W_k                                                    */
-  int o_cp, o_h;            /* [5][K] cp/R coefficients; [6][K] h/(RT) coefficients (a_i/i, a6)  */
-  int o_lnAf, o_bf, o_thf;  /* [NS] forward ln A, beta, E/R_c                                    */
-  int o_lnAr, o_br, o_thr;  /* [NS] reverse (ln A = -inf when the slot has no reverse reaction)  */
-  int o_idx;                /* [NS] bytes 0-2 side-A species, 3-5 side-B species, bits 48-63 third-body set */
-  int o_tbptr, o_tbsp, o_tbam1; /* [NTB+1], [nnz], [nnz]: listed species and (alpha - 1)         */
-  int o_gptr, o_gat;        /* [K+1], [nnz]: species-major gather list, entry = coef(double, low 16 mantissa bits = slot) */
+  int K, n;          /* species, unknowns (K+1)                                                           */
+  int L;             /* lanes per system this packing is for                                              */
+  int NV;            /* gather levels = ceil(n / L)                                                       */
+  int NS, NSR;       /* reaction slots (fused forward/reverse pairs), slot rounds = ceil(NS / L)          */
+  int NTB, NTBR, TBE;/* third-body sets, set rounds = ceil(NTB / L), listed entries per set (padded)      */
+  int o_sp;          /* [NV][13][L]        species table                                                  */
+  int o_sl;          /* [NSR][8][L]        slot table                                                     */
+  int o_tb;          /* [NTBR][TBE][2][L]  (alpha-1, region offset of the species)                        */
+  int o_glen;        /* [NV]               steps of gather level i (uniform over lanes, rows zero-padded) */
+  int o_gat;         /* [sum glen][L]      gather entries: double coefficient, low 16 mantissa bits =
+                                           offset (in doubles, x G) of q_s inside the q region            */
+  int o_rkc;         /* RKC coefficients for s = 2..s_tab: [s-2] -> mu~_1; stages at o_rkcs               */
+  int o_rkcs;        /* [(s-2)(s-1)/2 + (j-2)][4] = mu_j, nu_j, mu~_j, gamma~_j, j = 2..s                  */
+  int s_tab;
   int words;
+  int o_perm;        /* [n] original state row (0 = T, 1 + species index) of component c                    */
 };
+
+/* doubles of shared memory per system: C region, [M] region, q region */
+__host__ __device__ __forceinline__ int region_doubles(const DevMech &m) { return m.n + m.NTB + 1 + m.NSR * m.L; }
 
 }  // namespace ckb
