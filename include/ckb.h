@@ -141,6 +141,15 @@ int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, dou
  */
 int ckb_fp64_probe(int32_t kind, int64_t iters, double *per_second, void *stream);
 
+/*
+ * ckb_mech_pack_stats: host-only (no CUDA call).  Validates `d`, packs it for `lanes` lanes per system
+ * (1, 8, 16 or 32) and reports the packing: stats[0] fused reaction slots, [1] slot rounds per f(y),
+ * [2] gather steps per f(y), [3] shared-memory bank-conflict replays left in the gather per f(y) after
+ * scheduling (lanes = 32 only, else 0), [4] the same for the concentration reads, [5] table size in
+ * 8-byte words, [6] shared-memory doubles per system, [7] register slots per lane (NV).
+ */
+int ckb_mech_pack_stats(const ckb_mech_desc *d, int32_t lanes, int32_t *stats8);
+
 const char *ckb_strerror(int code);
 const char *ckb_last_cuda_error(void);
 

@@ -21,7 +21,7 @@ ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
 
 # every symbol include/ckb.h declares
 EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "ckb_integrate_host",
-           "ckb_rhs", "ckb_fp64_probe", "ckb_strerror", "ckb_last_cuda_error")
+           "ckb_rhs", "ckb_fp64_probe", "ckb_mech_pack_stats", "ckb_strerror", "ckb_last_cuda_error")
 
 
 class CkbError(RuntimeError):
@@ -75,6 +75,8 @@ def lib():
     L.ckb_rhs.restype = C.c_int
     L.ckb_fp64_probe.argtypes = [i32, i64, C.POINTER(dbl), vp]
     L.ckb_fp64_probe.restype = C.c_int
+    L.ckb_mech_pack_stats.argtypes = [C.POINTER(_Desc), i32, C.POINTER(i32)]
+    L.ckb_mech_pack_stats.restype = C.c_int
     L.ckb_strerror.argtypes = [C.c_int]
     L.ckb_strerror.restype = C.c_char_p
     L.ckb_last_cuda_error.argtypes = []
@@ -109,6 +111,33 @@ def _dev_ptr(t, dtype, where):
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
         raise TypeError(f"{where}: expected a contiguous CUDA tensor of {dtype}")
     return C.c_void_p(t.data_ptr())
+
+
+def _make_desc(mech):
+    keep = dict(
+        mol_weight=_f64(mech.mol_weight), nasa=_f64(mech.nasa), arr_A=_f64(mech.arr_A),
+        arr_beta=_f64(mech.arr_beta), arr_E=_f64(mech.arr_E),
+        reac_ptr=_i32(mech.reac_ptr), reac_species=_i32(mech.reac_species), reac_nu=_i32(mech.reac_nu),
+        prod_ptr=_i32(mech.prod_ptr), prod_species=_i32(mech.prod_species), prod_nu=_i32(mech.prod_nu),
+        tb_reaction=_i32(mech.tb_reaction), tb_ptr=_i32(mech.tb_ptr), tb_species=_i32(mech.tb_species),
+        tb_eff=_f64(mech.tb_eff))
+    d = _Desc()
+    d.n_species = int(keep["mol_weight"].shape[0])
+    d.n_reactions = int(keep["arr_A"].shape[0])
+    d.n_third_body = int(keep["tb_reaction"].shape[0])
+    for k, v in keep.items():
+        setattr(d, k, v.ctypes.data)
+    return d, keep
+
+
+def pack_stats(mech, lanes=32):
+    """ckb_mech_pack_stats (host only, no GPU needed): dict of the packing report for `lanes` lanes per system."""
+    d, _keep = _make_desc(mech)
+    out = (C.c_int32 * 8)()
+    _check(lib().ckb_mech_pack_stats(C.byref(d), int(lanes), out), "ckb_mech_pack_stats")
+    names = ("slots", "slot_rounds", "gather_steps", "gather_conflict_replays", "conc_conflict_replays",
+             "table_words", "shared_doubles_per_system", "register_slots")
+    return dict(zip(names, list(out)))
 
 
 class Mech:

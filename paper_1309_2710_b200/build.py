@@ -33,6 +33,17 @@ def instantiations():
     return out
 
 
+def min_blocks(L: int, NV: int) -> int:
+    """Resident 128-thread blocks per SM that the register allocation of integrate_kernel<L, NV> must allow
+    (launch bounds): 4 -> <= 128 registers, 3 -> <= 168, 2 -> <= 255.  Chosen so that no instantiation spills."""
+    doubles = NV  # register slots per stage vector
+    if doubles <= int(os.environ.get("CKB_MINB4_MAXNV", "2")):
+        return int(os.environ.get("CKB_MINB_SMALL", "4"))
+    if doubles <= 4:
+        return 3
+    return 2
+
+
 def _digest(extra: str) -> str:
     h = hashlib.sha256(extra.encode())
     for root in (CSRC, os.path.join(HERE, "..", "include")):
@@ -53,9 +64,9 @@ def _run(cmd, verbose):
 
 def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
-    flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else [])
+    flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("CKB_DEFS", "").split()  # tuning knobs
     stamp = os.path.join(OBJ, "stamp")
-    digest = _digest(" ".join(flags))
+    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", ""))
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     jobs = []
@@ -64,7 +75,8 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
         jobs.append((obj, [NVCC, *flags, "-c", os.path.join(CSRC, src), "-o", obj]))
     for (L, NV) in instantiations():
         obj = os.path.join(OBJ, f"ckb_inst_L{L}_NV{NV}.o")
-        jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", "-c",
+        jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_MINB={min_blocks(L, NV)}",
+                           f"-DCKB_UNROLL_SLOTS={1 if L == 1 else 2}", "-c",
                            os.path.join(CSRC, "ckb_inst.cu"), "-o", obj]))
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         list(ex.map(lambda j: _run(j[1], verbose or ptxas_v), jobs))

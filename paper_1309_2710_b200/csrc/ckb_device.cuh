@@ -24,6 +24,10 @@ namespace ckb {
 /* R20: physical constants */
 #define CKB_RU 8.314462618e7 /* erg/(mol K) */
 
+#ifndef CKB_UNROLL_SLOTS
+#define CKB_UNROLL_SLOTS 1 /* reaction slots in flight per lane: 2 slots = 4 independent exp chains */
+#endif
+
 /* exp(x) for the Arrhenius coefficients (Eq. 5): x = k ln2 + r, |r| <= ln2/2; e^r = 1 + r + r^2 q(r) with
  * q of degree 9 fitted at Chebyshev nodes (truncation 1.7e-17 relative); 2^k by exponent arithmetic with k
  * clamped to the normal range, so x << -708 gives ~1e-308 (not 0, not NaN) and the code has no branch.
@@ -141,8 +145,10 @@ struct Sys {
     gsync();
     /* Eq. 4-5: q_s = [M] (k_f prod C_reactants - k_r prod C_products); absent molecules point at C_0 = 1 */
     {
+      constexpr int US = CKB_UNROLL_SLOTS;
       int b = m.o_sl + g;
       double *q = sQ + g * G;
+#pragma unroll US
       for (int r = 0; r < m.NSR; r++, b += CKB_SL_WORDS * L, q += L * G) {
         const double xf = fma(-td(b + CKB_SL_THF * L), invT, fma(td(b + CKB_SL_BF * L), lnT, td(b + CKB_SL_LNAF * L)));
         const double xr = fma(-td(b + CKB_SL_THR * L), invT, fma(td(b + CKB_SL_BR * L), lnT, td(b + CKB_SL_LNAR * L)));
@@ -161,12 +167,21 @@ struct Sys {
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       const int len = (int)tw(m.o_glen + i);
-      double acc = 0.0;
-      for (int t = 0; t < len; t++, gp += L) {
-        const unsigned long long w = tw(gp);
-        const double coef = __longlong_as_double((long long)(w & ~0xFFFFull));
-        acc = fma(coef, sQ[(unsigned)w & 0xFFFFu], acc);
+      double acc0 = 0.0, acc1 = 0.0;
+      if (L == 1) { /* one entry per word: double coefficient, low 16 mantissa bits = q offset (a constant-bank operand) */
+        for (int t = 0; t < len; t++, gp += L) {
+          const unsigned long long w = tw(gp);
+          acc0 = fma(__longlong_as_double((long long)(w & ~0xFFFFull)), sQ[(unsigned)w & 0xFFFFu], acc0);
+        }
+      } else { /* two entries per word: (int16 coefficient << 16) | q offset */
+        for (int t = 0; t < len; t++, gp += L) {
+          const unsigned long long w = tw(gp);
+          const unsigned lo = (unsigned)w, hi = (unsigned)(w >> 32);
+          acc0 = fma((double)((int)lo >> 16), sQ[lo & 0xFFFFu], acc0);
+          acc1 = fma((double)((int)hi >> 16), sQ[hi & 0xFFFFu], acc1);
+        }
       }
+      const double acc = acc0 + acc1;
       f[i] = td(m.o_sp + i * CKB_SP_WORDS * L + g + CKB_SP_W * L) * acc * invrho;
       s3 = fma(hrt[i], acc, s3);
     }
@@ -686,6 +701,9 @@ struct Rkc {
  * sub-stepping, so finished lanes never idle behind a slow neighbour (divergence control).
  * ---------------------------------------------------------------------------------------------- */
 #define CKB_BLOCK 128
+#ifndef CKB_MINB
+#define CKB_MINB 1 /* resident blocks per SM the register allocation must allow (set per instantiation) */
+#endif
 
 template <class S>
 __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem) {
@@ -711,7 +729,7 @@ template <class S>
 struct IntegratorOf<S, 1> { typedef Rkc<S> type; };
 
 template <int L, int NV, class TAB, int METHOD>
-__global__ void __launch_bounds__(CKB_BLOCK)
+__global__ void __launch_bounds__(CKB_BLOCK, CKB_MINB)
 integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, double *__restrict__ states,
                  const double *__restrict__ pressure, double p_uniform, long long N, long long ld, double t0,
                  double dt, double rtol, double atol, int *__restrict__ status, int *__restrict__ stats,

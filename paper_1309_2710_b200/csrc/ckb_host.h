@@ -30,6 +30,9 @@ struct Packed {
   std::vector<unsigned long long> blob; /* host copy of the packed tables */
   unsigned long long *d_blob = nullptr;
   int rc = CKB_EUNSUPPORTED;            /* CKB_OK when this packing exists */
+  /* schedule report (L = 32): gather steps per f(y), bank-conflict replays left in the gather and in the
+   * concentration reads */
+  int gather_steps = 0, gather_excess_wavefronts = 0, slot_excess_wavefronts = 0;
 };
 struct Parsed;
 int parse_mechanism(const ckb_mech_desc *d, Parsed &P);

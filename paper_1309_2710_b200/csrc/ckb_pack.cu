@@ -179,6 +179,190 @@ static void rkc_coefficients(int s, double *mut1, double *stages) {
   }
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * Bank-conflict-aware scheduling.  Shared memory has 32 four-byte banks; a 64-bit warp
+ * access is served half-warp by half-warp, and is conflict free when the 16 lanes of a half-warp touch 16
+ * distinct bank pairs (or the same address).  Where a lane reads is table data, so the packer chooses it:
+ *   - place_slots(): which reaction slot each lane evaluates in each round, and in which order it reads the
+ *     molecules of a side, so that the concentration reads of a half-warp collide as little as possible;
+ *   - colour_gather(): the order in which each lane walks its gather row, by edge-colouring the bipartite
+ *     multigraph (lane, bank pair of q_s): every step reads 16 distinct bank pairs per half-warp (Koenig:
+ *     max-degree many steps suffice).
+ * Both only reorder commutative products / sums: the result changes by rounding only.
+ * ---------------------------------------------------------------------------------------------- */
+namespace {
+
+struct Placed {
+  int slot = -1;          /* index into Parsed::slots, -1 = padding */
+  int a[3] = {0, 0, 0};   /* components read as reactant molecules (0 = none -> C_0 = 1) */
+  int b[3] = {0, 0, 0};   /* components read as product molecules */
+};
+
+/* greedy: fill rounds position by position with the remaining slot (and molecule order) that adds the fewest
+ * bank-pair collisions to its half-warp's six concentration reads */
+std::vector<Placed> place_slots(const Parsed &P, const std::vector<int> &comp_of_sp, int L, int NSR, bool optimise) {
+  const int NS = (int)P.slots.size();
+  std::vector<Placed> out((size_t)NSR * L);
+  auto comps = [&](int s, int a[3], int b[3]) {
+    const Rx &x = P.rx[P.slots[s].f];
+    const bool rev = P.slots[s].r >= 0;
+    for (int q = 0; q < 3; q++) {
+      a[q] = q < (int)x.reac.size() ? comp_of_sp[x.reac[q]] : 0;
+      /* a slot without reverse multiplies k_r = 0 by 1, never by a concentration */
+      b[q] = (rev && q < (int)x.prod.size()) ? comp_of_sp[x.prod[q]] : 0;
+    }
+  };
+  if (!optimise || L != 32) {
+    for (int s = 0; s < NS; s++) {
+      out[s].slot = s;
+      comps(s, out[s].a, out[s].b);
+    }
+    return out;
+  }
+  std::vector<char> used(NS, 0);
+  int left = NS;
+  for (int r = 0; r < NSR && left > 0; r++) {
+    for (int h = 0; h < 2 && left > 0; h++) {
+      /* comp_at[k][bp] = component already read through bank pair bp by instruction k in this half-warp (0 = free) */
+      int comp_at[6][16];
+      for (auto &row : comp_at)
+        for (int &v : row) v = 0;
+      for (int l = 0; l < 16 && left > 0; l++) {
+        int best = -1, best_cost = 1 << 30, best_a[3] = {0, 0, 0}, best_b[3] = {0, 0, 0};
+        for (int s = 0; s < NS && best_cost > 0; s++) {
+          if (used[s]) continue;
+          int a[3], b[3];
+          comps(s, a, b);
+          std::sort(a, a + 3, std::greater<int>());
+          std::sort(b, b + 3, std::greater<int>());
+          /* try every order of the molecules on each side */
+          int pa[3] = {a[0], a[1], a[2]};
+          do {
+            int ca = 0;
+            for (int q = 0; q < 3; q++)
+              if (pa[q] && comp_at[q][pa[q] & 15] && comp_at[q][pa[q] & 15] != pa[q]) ca++;
+            int pb[3] = {b[0], b[1], b[2]};
+            do {
+              int cb = 0;
+              for (int q = 0; q < 3; q++)
+                if (pb[q] && comp_at[3 + q][pb[q] & 15] && comp_at[3 + q][pb[q] & 15] != pb[q]) cb++;
+              if (ca + cb < best_cost) {
+                best_cost = ca + cb;
+                best = s;
+                for (int q = 0; q < 3; q++) { best_a[q] = pa[q]; best_b[q] = pb[q]; }
+              }
+            } while (std::prev_permutation(pb, pb + 3));
+          } while (std::prev_permutation(pa, pa + 3));
+        }
+        Placed &pl = out[(size_t)r * 32 + h * 16 + l];
+        pl.slot = best;
+        for (int q = 0; q < 3; q++) {
+          pl.a[q] = best_a[q];
+          pl.b[q] = best_b[q];
+          if (best_a[q] && !comp_at[q][best_a[q] & 15]) comp_at[q][best_a[q] & 15] = best_a[q];
+          if (best_b[q] && !comp_at[3 + q][best_b[q] & 15]) comp_at[3 + q][best_b[q] & 15] = best_b[q];
+        }
+        used[best] = 1;
+        left--;
+      }
+    }
+  }
+  return out;
+}
+
+struct GEntry { int pos, coef; };
+
+/* One gather level: rows[g] = entries lane g must sum.  Returns steps[t][g] (pos = -1: idle).  With
+ * `optimise`, a proper edge colouring of (lane, pos mod 16) per half-warp; else row order. */
+std::vector<std::vector<GEntry>> colour_gather(const std::vector<std::vector<GEntry>> &rows, int L, bool optimise) {
+  size_t maxlen = 0;
+  for (auto &r : rows) maxlen = std::max(maxlen, r.size());
+  if (!optimise || L != 32) {
+    std::vector<std::vector<GEntry>> steps(maxlen, std::vector<GEntry>(L, GEntry{-1, 0}));
+    for (int g = 0; g < L; g++)
+      for (size_t t = 0; t < rows[g].size(); t++) steps[t][g] = rows[g][t];
+    return steps;
+  }
+  std::vector<std::vector<GEntry>> steps;
+  for (int h = 0; h < 2; h++) {
+    /* degrees */
+    int deg_l[16] = {0}, deg_r[16] = {0};
+    for (int l = 0; l < 16; l++)
+      for (auto &e : rows[h * 16 + l]) { deg_l[l]++; deg_r[e.pos & 15]++; }
+    int D = 0;
+    for (int q = 0; q < 16; q++) D = std::max(D, std::max(deg_l[q], deg_r[q]));
+    /* colour[c][l] = index into rows[h*16+l] of the edge of colour c at lane l, rcol[c][bp] = lane using bank pair bp */
+    std::vector<std::vector<int>> at_l(D, std::vector<int>(16, -1)), at_r(D, std::vector<int>(16, -1));
+    for (int l = 0; l < 16; l++) {
+      const auto &row = rows[h * 16 + l];
+      for (int ei = 0; ei < (int)row.size(); ei++) {
+        const int bp = row[ei].pos & 15;
+        int ca = 0, cb = 0;
+        while (at_l[ca][l] >= 0) ca++;       /* colour free at the lane */
+        while (at_r[cb][bp] >= 0) cb++;      /* colour free at the bank pair */
+        if (ca != cb) {
+          /* flip the ca/cb alternating path that starts at bank pair bp (it has an edge of colour ca, none of cb) */
+          int cur_bp = bp, c_have = ca, c_want = cb;
+          std::vector<std::pair<int, int>> path; /* (lane, edge index) along the path */
+          while (true) {
+            const int ln = at_r[c_have][cur_bp];
+            if (ln < 0) break;
+            const int e2 = at_l[c_have][ln];
+            path.push_back({ln, e2});
+            /* next: at lane ln, the edge of colour c_want */
+            const int e3 = at_l[c_want][ln];
+            if (e3 < 0) break;
+            path.push_back({ln, e3});
+            cur_bp = rows[h * 16 + ln][e3].pos & 15;
+          }
+          /* remove the path's edges from the tables, then re-insert with swapped colours */
+          std::vector<int> cols(path.size());
+          for (size_t q = 0; q < path.size(); q++) cols[q] = (q % 2 == 0) ? c_have : c_want;
+          for (size_t q = 0; q < path.size(); q++) {
+            const int ln = path[q].first, e = path[q].second, b2 = rows[h * 16 + ln][e].pos & 15;
+            at_l[cols[q]][ln] = -1;
+            at_r[cols[q]][b2] = -1;
+          }
+          for (size_t q = 0; q < path.size(); q++) {
+            const int ln = path[q].first, e = path[q].second, b2 = rows[h * 16 + ln][e].pos & 15;
+            const int nc = (cols[q] == c_have) ? c_want : c_have;
+            at_l[nc][ln] = e;
+            at_r[nc][b2] = ln;
+          }
+          /* now ca is free at bp as well */
+        }
+        at_l[ca][l] = ei;
+        at_r[ca][bp] = l;
+      }
+    }
+    if ((int)steps.size() < D) steps.resize(D, std::vector<GEntry>(32, GEntry{-1, 0}));
+    for (int c = 0; c < D; c++)
+      for (int l = 0; l < 16; l++)
+        if (at_l[c][l] >= 0) steps[c][h * 16 + l] = rows[h * 16 + l][at_l[c][l]];
+  }
+  return steps;
+}
+
+/* bank-pair collisions a schedule causes (excess wavefronts of 64-bit half-warp accesses), for the packing report */
+int excess_wavefronts(const std::vector<int> &addr_of_lane /* 32 entries, -1 = none */) {
+  int excess = 0;
+  for (int h = 0; h < 2; h++) {
+    std::map<int, std::vector<int>> by_bp;
+    for (int l = 0; l < 16; l++) {
+      const int a = addr_of_lane[h * 16 + l];
+      if (a < 0) continue;
+      auto &v = by_bp[a & 15];
+      if (std::find(v.begin(), v.end(), a) == v.end()) v.push_back(a);
+    }
+    int worst = 1;
+    for (auto &kv : by_bp) worst = std::max(worst, (int)kv.second.size());
+    excess += worst - 1;
+  }
+  return excess;
+}
+
+}  // namespace
+
 int pack_for(const Parsed &P, int L, Packed &out) {
   const int K = P.K, n = K + 1, G = 32 / L;
   const int NS = (int)P.slots.size(), NTB = (int)P.sets.size();
@@ -188,6 +372,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   for (auto &s : P.sets) TBE = std::max(TBE, (int)s.size());
   /* 16-bit region offsets */
   if ((long long)(n + NTB) * G > 65535 || (long long)NSR * L * G > 65535) return CKB_EUNSUPPORTED;
+  const bool optimise = true;
 
   /* components: 0 = T, then species by decreasing gather-row length */
   std::vector<int> sp_of_comp(n, -1), comp_of_sp(K);
@@ -201,30 +386,50 @@ int pack_for(const Parsed &P, int L, Packed &out) {
       comp_of_sp[order[c - 1]] = c;
     }
   }
-  std::vector<int> glen(NV, 0);
-  for (int c = 1; c < n; c++) glen[c / L] = std::max(glen[c / L], (int)P.rows[sp_of_comp[c]].size());
-  const int gsteps = std::accumulate(glen.begin(), glen.end(), 0);
+  /* which lane evaluates which slot, and the gather schedule of every level */
+  const std::vector<Placed> placed = place_slots(P, comp_of_sp, L, NSR, optimise);
+  std::vector<int> pos_of_slot(NS, -1);
+  for (int q = 0; q < NSR * L; q++)
+    if (placed[q].slot >= 0) pos_of_slot[placed[q].slot] = q;
+  std::vector<std::vector<std::vector<GEntry>>> sched(NV);
+  std::vector<int> glen(NV, 0); /* 64-bit words per lane: two entries per word */
+  for (int i = 0; i < NV; i++) {
+    std::vector<std::vector<GEntry>> rows(L);
+    for (int g = 0; g < L; g++) {
+      const int c = g + L * i;
+      if (c < 1 || c >= n) continue;
+      for (auto &sc : P.rows[sp_of_comp[c]]) rows[g].push_back(GEntry{pos_of_slot[sc.first], sc.second});
+    }
+    sched[i] = colour_gather(rows, L, optimise);
+    glen[i] = (L == 1) ? (int)sched[i].size() : ((int)sched[i].size() + 1) / 2;
+  }
+  const int gwords = std::accumulate(glen.begin(), glen.end(), 0);
   const int s_tab = (L == 1) ? 12 : 48;
 
   ckb::DevMech &m = out.dm;
   m.K = K; m.n = n; m.L = L; m.NV = NV; m.NS = NS; m.NSR = NSR; m.NTB = NTB; m.NTBR = NTBR; m.TBE = TBE;
   int off = 0;
-  auto take = [&off](size_t words) { int o = off; off += (int)words; return o; };
+  auto take = [&off](size_t words) { /* every table starts on a 256-byte boundary: whole 128-byte lines per warp load */
+    off = (off + 31) & ~31;
+    int o = off;
+    off += (int)words;
+    return o;
+  };
   m.o_sp = take((size_t)NV * CKB_SP_WORDS * L);
   m.o_sl = take((size_t)NSR * CKB_SL_WORDS * L);
   m.o_tb = take((size_t)NTBR * TBE * 2 * L);
+  m.o_gat = take((size_t)gwords * L);
   m.o_glen = take(NV);
-  m.o_gat = take((size_t)gsteps * L);
-  m.o_perm = take(n);
+  m.o_perm = off; off += n;
   m.s_tab = s_tab;
-  m.o_rkc = take(s_tab - 1);
-  m.o_rkcs = take((size_t)4 * (s_tab - 1) * s_tab / 2);
+  m.o_rkc = off; off += s_tab - 1;
+  m.o_rkcs = off; off += 4 * (s_tab - 1) * s_tab / 2;
   m.words = off;
   std::vector<unsigned long long> &b = out.blob;
   b.assign((size_t)off, 0ull);
   auto putd = [&b](int o, double x) { b[(size_t)o] = dbits(x); };
 
-  for (int c = 0; c < NV * L; c++) { /* species table; T and padding components keep zeros (W = 1) */
+  for (int c = 0; c < NV * L; c++) { /* species table; T and padding components keep zeros */
     const int i = c / L, g = c % L, base = m.o_sp + i * CKB_SP_WORDS * L + g;
     if (c >= 1 && c < n) {
       const int k = sp_of_comp[c];
@@ -240,30 +445,28 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   }
   for (int c = 0; c < n; c++) b[(size_t)m.o_perm + c] = (unsigned long long)(c == 0 ? 0 : 1 + sp_of_comp[c]);
 
-  const double NEG_INF = -1.0e4; /* stands for ln 0: ckb_exp() returns ~1e-308 for it, no special case on the device */
-  for (int s = 0; s < NSR * L; s++) {
-    const int r = s / L, g = s % L, base = m.o_sl + r * CKB_SL_WORDS * L + g;
+  const double LN_ZERO = -1.0e4; /* stands for ln 0: ckb_exp() returns ~1e-308 for it, no special case on the device */
+  for (int q = 0; q < NSR * L; q++) {
+    const int r = q / L, g = q % L, base = m.o_sl + r * CKB_SL_WORDS * L + g;
+    const Placed &pl = placed[q];
     unsigned long long wa = 0, wb = 0;
-    if (s < NS) {
-      const int f = P.slots[s].f, rv = P.slots[s].r;
-      putd(base + CKB_SL_LNAF * L, P.A[f] > 0.0 ? std::log(P.A[f]) : NEG_INF);
+    if (pl.slot >= 0) {
+      const int f = P.slots[pl.slot].f, rv = P.slots[pl.slot].r;
+      putd(base + CKB_SL_LNAF * L, P.A[f] > 0.0 ? std::log(P.A[f]) : LN_ZERO);
       putd(base + CKB_SL_BF * L, P.beta[f]);
       putd(base + CKB_SL_THF * L, P.E[f] / RC_CAL);
-      putd(base + CKB_SL_LNAR * L, (rv >= 0 && P.A[rv] > 0.0) ? std::log(P.A[rv]) : NEG_INF);
+      putd(base + CKB_SL_LNAR * L, (rv >= 0 && P.A[rv] > 0.0) ? std::log(P.A[rv]) : LN_ZERO);
       putd(base + CKB_SL_BR * L, rv >= 0 ? P.beta[rv] : 0.0);
       putd(base + CKB_SL_THR * L, rv >= 0 ? P.E[rv] / RC_CAL : 0.0);
-      const Rx &x = P.rx[f];
-      for (int q = 0; q < 3; q++) {
-        /* absent molecule -> C_0 = 1; a slot without reverse multiplies k_r = 0 by 1, never by a concentration */
-        const unsigned long long ao = q < (int)x.reac.size() ? (unsigned)(comp_of_sp[x.reac[q]] * G) : 0u;
-        const unsigned long long bo = (rv >= 0 && q < (int)x.prod.size()) ? (unsigned)(comp_of_sp[x.prod[q]] * G) : 0u;
-        wa |= ao << (16 * q);
-        wb |= bo << (16 * q);
+      for (int k = 0; k < 3; k++) {
+        wa |= (unsigned long long)(pl.a[k] * G) << (16 * k);
+        wb |= (unsigned long long)(pl.b[k] * G) << (16 * k);
       }
-      wa |= (unsigned long long)((n + (x.tbset >= 0 ? x.tbset : NTB)) * G) << 48;
+      const int ts = P.rx[f].tbset;
+      wa |= (unsigned long long)((n + (ts >= 0 ? ts : NTB)) * G) << 48;
     } else { /* padding slot: q = 0 */
-      putd(base + CKB_SL_LNAF * L, NEG_INF);
-      putd(base + CKB_SL_LNAR * L, NEG_INF);
+      putd(base + CKB_SL_LNAF * L, LN_ZERO);
+      putd(base + CKB_SL_LNAR * L, LN_ZERO);
       wa = (unsigned long long)((n + NTB) * G) << 48;
     }
     b[(size_t)base + CKB_SL_IDXA * L] = wa;
@@ -279,20 +482,60 @@ int pack_for(const Parsed &P, int L, Packed &out) {
       }
     }
   }
-  {
-    int step0 = 0;
+  { /* gather entries: (coefficient int16 << 16) | (q offset), two per word; an idle lane reads, with
+       coefficient 0, a q whose bank pair nobody in its half-warp uses in that step */
+    int w0 = 0;
+    out.gather_steps = 0;
+    out.gather_excess_wavefronts = 0;
     for (int i = 0; i < NV; i++) {
       b[(size_t)m.o_glen + i] = (unsigned long long)glen[i];
-      for (int g = 0; g < L; g++) {
-        const int c = g + L * i;
-        if (c < 1 || c >= n) continue;
-        const auto &row = P.rows[sp_of_comp[c]];
-        for (int t = 0; t < (int)row.size(); t++)
-          b[(size_t)m.o_gat + (size_t)(step0 + t) * L + g] =
-              (dbits((double)row[t].second) & ~0xFFFFull) | (unsigned long long)(row[t].first * G);
+      const int per_word = (L == 1) ? 1 : 2;
+      for (int t = 0; t < per_word * glen[i]; t++) {
+        std::vector<int> addr(32, -1);
+        for (int g = 0; g < L; g++) {
+          GEntry e = t < (int)sched[i].size() ? sched[i][t][g] : GEntry{-1, 0};
+          if (e.pos < 0) {
+            e.coef = 0;
+            e.pos = g % 16;
+            if (L == 32 && t < (int)sched[i].size()) {
+              bool busy[16] = {false};
+              for (int l = 0; l < 16; l++) {
+                const GEntry &o = sched[i][t][(g / 16) * 16 + l];
+                if (o.pos >= 0) busy[o.pos & 15] = true;
+              }
+              for (int l = 0; l < 16; l++)
+                if (addr[(g / 16) * 16 + l] >= 0) busy[addr[(g / 16) * 16 + l] & 15] = true;
+              for (int r0 = 0; r0 < 16; r0++)
+                if (!busy[r0]) { e.pos = r0; break; }
+            }
+          }
+          if (L == 32) addr[g] = e.pos;
+          if (L == 1) { /* double coefficient with the q offset in its 16 lowest mantissa bits */
+            b[(size_t)m.o_gat + (size_t)(w0 + t) * L + g] =
+                (dbits((double)e.coef) & ~0xFFFFull) | (unsigned long long)(e.pos * G);
+          } else {
+            const unsigned long long ent =
+                ((unsigned long long)((unsigned)(e.coef & 0xFFFF)) << 16) | (unsigned long long)(e.pos * G);
+            b[(size_t)m.o_gat + (size_t)(w0 + t / 2) * L + g] |= ent << (32 * (t & 1));
+          }
+        }
+        if (L == 32) out.gather_excess_wavefronts += excess_wavefronts(addr);
+        out.gather_steps++;
       }
-      step0 += glen[i];
+      w0 += glen[i];
     }
+  }
+  if (L == 32) { /* report: excess wavefronts of the concentration reads per f(y) */
+    out.slot_excess_wavefronts = 0;
+    for (int r = 0; r < NSR; r++)
+      for (int k = 0; k < 6; k++) {
+        std::vector<int> addr(32, -1);
+        for (int g = 0; g < 32; g++) {
+          const Placed &pl = placed[(size_t)r * 32 + g];
+          addr[g] = k < 3 ? pl.a[k] : pl.b[k - 3];
+        }
+        out.slot_excess_wavefronts += excess_wavefronts(addr);
+      }
   }
   for (int s = 2; s <= s_tab; s++) {
     double mut1;
@@ -304,7 +547,6 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   }
   return CKB_OK;
 }
-
 
 /* parse once, pack for every lanes-per-system value; the thread-per-ODE packing must fit the kernel
  * parameter space (CKB_PARAM_WORDS) */
@@ -329,3 +571,22 @@ int load_packings(const ckb_mech_desc *d, ckb_mech *m) {
 }
 
 }  // namespace ckb_host
+
+extern "C" int ckb_mech_pack_stats(const ckb_mech_desc *d, int32_t lanes, int32_t *stats8) {
+  if (!d || !stats8 || (lanes != 1 && lanes != 8 && lanes != 16 && lanes != 32)) return CKB_EINVAL;
+  ckb_host::Parsed P;
+  int rc = ckb_host::parse_mechanism(d, P);
+  if (rc != CKB_OK) return rc;
+  ckb_host::Packed pk;
+  rc = ckb_host::pack_for(P, lanes, pk);
+  if (rc != CKB_OK) return rc;
+  stats8[0] = pk.dm.NS;
+  stats8[1] = pk.dm.NSR;
+  stats8[2] = pk.gather_steps;
+  stats8[3] = pk.gather_excess_wavefronts;
+  stats8[4] = pk.slot_excess_wavefronts;
+  stats8[5] = pk.dm.words;
+  stats8[6] = ckb::region_doubles(pk.dm);
+  stats8[7] = pk.dm.NV;
+  return CKB_OK;
+}

@@ -67,9 +67,10 @@ struct DevMech {
   int o_sp;          /* [NV][13][L]        species table                                                  */
   int o_sl;          /* [NSR][8][L]        slot table                                                     */
   int o_tb;          /* [NTBR][TBE][2][L]  (alpha-1, region offset of the species)                        */
-  int o_glen;        /* [NV]               steps of gather level i (uniform over lanes, rows zero-padded) */
-  int o_gat;         /* [sum glen][L]      gather entries: double coefficient, low 16 mantissa bits =
-                                           offset (in doubles, x G) of q_s inside the q region            */
+  int o_glen;        /* [NV]               64-bit words per lane of gather level i (uniform over lanes)   */
+  int o_gat;         /* [sum glen][L]      gather entries.  L > 1: two per word, (int16 coefficient << 16) |
+                                           offset (in doubles, x G) of q_s inside the q region; L = 1: one
+                                           per word, double coefficient with the offset in its low 16 bits */
   int o_rkc;         /* RKC coefficients for s = 2..s_tab: [s-2] -> mu~_1; stages at o_rkcs               */
   int o_rkcs;        /* [(s-2)(s-1)/2 + (j-2)][4] = mu_j, nu_j, mu~_j, gamma~_j, j = 2..s                  */
   int s_tab;
