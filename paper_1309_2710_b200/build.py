@@ -70,7 +70,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     jobs = []
-    for src in ("ckb_api.cu", "ckb_pack.cu", "ckb_probe.cu"):
+    for src in ("ckb_api.cu", "ckb_pack.cu", "ckb_order.cu", "ckb_probe.cu"):
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
         jobs.append((obj, [NVCC, *flags, "-c", os.path.join(CSRC, src), "-o", obj]))
     for (L, NV) in instantiations():

@@ -121,6 +121,8 @@ void ckb_mech_free(ckb_mech *m) {
   for (int i = 0; i < 4; i++)
     if (m->pk[i].d_blob) cudaFree(m->pk[i].d_blob);
   if (m->d_counters) cudaFree(m->d_counters);
+  if (m->d_order) cudaFree(m->d_order);
+  if (m->d_bins) cudaFree(m->d_bins);
   if (m->ws_states) cudaFree(m->ws_states);
   if (m->ws_pressure) cudaFree(m->ws_pressure);
   if (m->ws_status) cudaFree(m->ws_status);
@@ -150,7 +152,12 @@ int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, dou
   if (N == 0) return CKB_OK;
   if (!states || ld < N) return CKB_EINVAL;
   ckb_host::IntegrateArgs a{states, pressure, p_uniform, (long long)N, (long long)ld, t, dt, rtol, atol,
-                  status, stats, (cudaStream_t)stream};
+                  status, stats, (cudaStream_t)stream, nullptr};
+  /* queue order: hottest systems first (row 0 of states = T); pointless when every system starts at once */
+  if (N >= 4096) {
+    rc = ckb_host::make_queue_order(m, states, N, a.stream, &a.order);
+    if (rc) return rc;
+  }
   return dispatch_integrate(m, l, method, a);
 }
 

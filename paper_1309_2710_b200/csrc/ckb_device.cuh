@@ -733,20 +733,22 @@ __global__ void __launch_bounds__(CKB_BLOCK, CKB_MINB)
 integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, double *__restrict__ states,
                  const double *__restrict__ pressure, double p_uniform, long long N, long long ld, double t0,
                  double dt, double rtol, double atol, int *__restrict__ status, int *__restrict__ stats,
-                 unsigned long long *__restrict__ counter) {
+                 unsigned long long *__restrict__ counter, const int *__restrict__ order) {
   extern __shared__ double smem[];
   typedef Sys<L, NV, TAB> S;
   S sys(m, tab);
   sys_setup(sys, m, smem);
   constexpr int G = S::G;
   const long long n_groups = (long long)gridDim.x * (CKB_BLOCK / 32) * G;
-  long long ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L;
+  long long qi = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L;
+  long long ode = 0;
   typename IntegratorOf<S, METHOD>::type integ;
   bool need_load = true;
   double f[NV];
   while (true) {
     if (need_load) {
-      if (ode >= N) break;
+      if (qi >= N) break;
+      ode = order ? (long long)order[qi] : qi; /* queue position -> system */
       sys.set_pressure(pressure ? pressure[ode] : p_uniform);
       double y0[NV];
 #pragma unroll
@@ -777,7 +779,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
       unsigned long long nx = 0;
       if (sys.g == 0) nx = atomicAdd(counter, 1ull);
       if (L > 1) nx = __shfl_sync(sys.mask, nx, sys.src0);
-      ode = n_groups + (long long)nx;
+      qi = n_groups + (long long)nx;
       need_load = true;
     }
   }

@@ -52,6 +52,10 @@ struct ckb_mech {
   /* work-queue counters of the persistent kernels: a ring, one slot per launch in flight */
   unsigned long long *d_counters = nullptr;
   mutable std::atomic<unsigned> next_counter{0};
+  /* queue order scratch (ckb_order.cu), grow-only; calls on one handle must be stream-ordered */
+  mutable int *d_order = nullptr;
+  mutable unsigned *d_bins = nullptr;
+  mutable size_t order_cap = 0;
 };
 
 
@@ -62,7 +66,10 @@ namespace ckb_host {
 struct IntegrateArgs {
   double *states; const double *pressure; double p_uniform; long long N, ld;
   double t, dt, rtol, atol; int *status, *stats; cudaStream_t stream;
+  const int *order; /* queue order (device) or NULL */
 };
+
+int make_queue_order(const ckb_mech *m, const double *T, long long N, cudaStream_t s, const int **order);
 struct RhsArgs {
   const double *states; const double *pressure; double p_uniform; long long N, ld; double *dydt; int repeat;
   cudaStream_t stream;

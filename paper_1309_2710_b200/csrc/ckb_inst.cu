@@ -72,7 +72,7 @@ static int launch(const ckb_mech *m, const IntegrateArgs &a) {
   Tab tab;
   make_tab(m, tab);
   kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(pack_of(m).dm, tab, a.states, a.pressure, a.p_uniform, a.N, a.ld,
-                                                       a.t, a.dt, a.rtol, a.atol, a.status, a.stats, counter);
+                                                       a.t, a.dt, a.rtol, a.atol, a.status, a.stats, counter, a.order);
   CK(cudaGetLastError());
   return CKB_OK;
 }
