@@ -33,10 +33,17 @@ def instantiations():
     return out
 
 
+def systems_per_group(L: int, NV: int) -> int:
+    """Systems a group of L lanes evaluates together (template parameter M).  M = 2 shares table loads and index
+    decoding between two systems of a warp and interleaves their chains, but measured slower on B200 than M = 1
+    (129k vs 144k ODE/s on configs[3]: twice the registers, half the resident warps) -- kept as a knob."""
+    return int(os.environ.get("CKB_M32", "1")) if L == 32 else 1
+
+
 def min_blocks(L: int, NV: int) -> int:
     """Resident 128-thread blocks per SM that the register allocation of integrate_kernel<L, NV> must allow
     (launch bounds): 4 -> <= 128 registers, 3 -> <= 168, 2 -> <= 255.  Chosen so that no instantiation spills."""
-    doubles = NV  # register slots per stage vector
+    doubles = NV * systems_per_group(L, NV)  # register slots per stage vector
     if doubles <= int(os.environ.get("CKB_MINB4_MAXNV", "2")):
         return int(os.environ.get("CKB_MINB_SMALL", "4"))
     if doubles <= 4:
@@ -66,7 +73,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     os.makedirs(OBJ, exist_ok=True)
     flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("CKB_DEFS", "").split()  # tuning knobs
     stamp = os.path.join(OBJ, "stamp")
-    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", ""))
+    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", ""))
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     jobs = []
@@ -76,7 +83,8 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     for (L, NV) in instantiations():
         obj = os.path.join(OBJ, f"ckb_inst_L{L}_NV{NV}.o")
         jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_MINB={min_blocks(L, NV)}",
-                           f"-DCKB_UNROLL_SLOTS={1 if L == 1 else 2}", "-c",
+                           f"-DCKB_UNROLL_SLOTS={1 if L == 1 else int(os.environ.get('CKB_US', '1'))}",
+                           f"-DCKB_M={systems_per_group(L, NV)}", "-c",
                            os.path.join(CSRC, "ckb_inst.cu"), "-o", obj]))
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         list(ex.map(lambda j: _run(j[1], verbose or ptxas_v), jobs))

@@ -56,24 +56,27 @@ __device__ __forceinline__ double ckb_exp(double x) {
  * Sys<L, NV, TAB>: one ODE system on L lanes with NV register slots per lane; tables from the kernel
  * parameter bank (ParamTab) or global/L1 (GlobalTab).
  * ---------------------------------------------------------------------------------------------- */
-template <int L_, int NV_, class TAB>
+template <int L_, int NV_, class TAB, int M_ = 1>
 struct Sys {
-  static constexpr int L = L_, NV = NV_, G = 32 / L_;
+  /* M systems share the lanes of a group and are evaluated together: every table word is loaded and decoded
+   * once for all of them, and their (independent) dependency chains interleave -- DESIGN.md 6.5. */
+  static constexpr int L = L_, NV = NV_, G = 32 / L_, M = M_;
   const DevMech &m;
   const TAB &tab;
-  double *sR;      /* this system's shared region (ckb_tables.h), element e at sR[e*G] */
-  double *sQ;      /* = sR + (n + NTB + 1) * G */
+  double *sR;      /* shared region of system 0 of this group (ckb_tables.h), element e at sR[e*G]; system q at + q*RS */
+  int RS;          /* doubles between the regions of two systems of the group */
+  int qoff;        /* (n + NTB + 1) * G: start of the q region */
   unsigned mask;   /* lanes of this group */
   int g;           /* lane within the group */
   int src0;        /* warp lane that holds component 0 (T) */
-  double pR, Rp;   /* p / Ru and Ru / p (R24: pressure constant over the call) */
+  double pR[M], Rp[M]; /* p / Ru and Ru / p (R24: pressure constant over the call) */
 
   __device__ __forceinline__ Sys(const DevMech &m_, const TAB &tab_) : m(m_), tab(tab_) {}
   __device__ __forceinline__ unsigned long long tw(int i) const { return tab.ld(i); }
   __device__ __forceinline__ double td(int i) const { return __longlong_as_double((long long)tab.ld(i)); }
-  __device__ __forceinline__ void set_pressure(double p) {
-    pR = p / CKB_RU;
-    Rp = CKB_RU / p;
+  __device__ __forceinline__ void set_pressure(int q, double p) {
+    pR[q] = p / CKB_RU;
+    Rp[q] = CKB_RU / p;
   }
 
   __device__ __forceinline__ void gsync() const {
@@ -95,99 +98,164 @@ struct Sys {
   }
   __device__ __forceinline__ bool valid(int i) const { return g + L * i < m.n; }
 
-  /* f(y): Eq. 2-6.  y, f: component (g + L*i) in slot i. */
-  __device__ __forceinline__ void rhs(const double (&y)[NV], double (&f)[NV]) {
+  /* f(y): Eq. 2-6 for the M systems of the group.  y, f: [system][slot], component (g + L*i) in slot i. */
+  __device__ __forceinline__ void rhs(const double (&y)[M][NV], double (&f)[M][NV]) {
     const int n = m.n;
-    const double T = bcast0(y[0]);
-    const double invT = 1.0 / T;
-    const double lnT = log(T);
-    double s1 = 0.0, s2 = 0.0;
-    double hrt[NV], yw[NV];
+    double T[M], invT[M], lnT[M], s1[M], s2[M];
+    double hrt[M][NV], yw[M][NV];
+#pragma unroll
+    for (int q = 0; q < M; q++) {
+      T[q] = bcast0(y[q][0]);
+      invT[q] = 1.0 / T[q];
+      lnT[q] = log(T[q]);
+      s1[q] = 0.0;
+      s2[q] = 0.0;
+    }
     /* species table rows of T and of padding components are all zero: no branch needed */
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       const int b = m.o_sp + i * CKB_SP_WORDS * L + g;
       /* R8a: cp_k/R = a1 + a2 T + ... + a5 T^4;  h_k/(RT) = a1 + a2 T/2 + ... + a5 T^4/5 + a6/T */
-      double cp = td(b + (CKB_SP_CP + 4) * L);
-      double h = td(b + (CKB_SP_H + 4) * L);
+      double cc[5], hc[6];
 #pragma unroll
-      for (int q = 3; q >= 0; q--) {
-        cp = fma(cp, T, td(b + (CKB_SP_CP + q) * L));
-        h = fma(h, T, td(b + (CKB_SP_H + q) * L));
+      for (int k = 0; k < 5; k++) cc[k] = td(b + (CKB_SP_CP + k) * L);
+#pragma unroll
+      for (int k = 0; k < 6; k++) hc[k] = td(b + (CKB_SP_H + k) * L);
+      const double iw = td(b + CKB_SP_INVW * L);
+#pragma unroll
+      for (int q = 0; q < M; q++) {
+        double cp = cc[4], h = hc[4];
+#pragma unroll
+        for (int k = 3; k >= 0; k--) {
+          cp = fma(cp, T[q], cc[k]);
+          h = fma(h, T[q], hc[k]);
+        }
+        h = fma(hc[5], invT[q], h);
+        const double v = y[q][i] * iw; /* Y_k / W_k */
+        yw[q][i] = v;
+        hrt[q][i] = h;
+        s1[q] += v;
+        s2[q] = fma(v, cp, s2[q]);
       }
-      h = fma(td(b + (CKB_SP_H + 5) * L), invT, h);
-      const double v = y[i] * td(b + CKB_SP_INVW * L); /* Y_k / W_k */
-      yw[i] = v;
-      hrt[i] = h;
-      s1 += v;
-      s2 = fma(v, cp, s2);
     }
-    s1 = gsum(s1);
-    s2 = gsum(s2);
-    /* R9a: ideal gas at constant pressure: rho = p / (Ru T sum_k Y_k/W_k), C_k = rho Y_k / W_k */
-    const double ctot = pR * invT;
-    const double rho = ctot * (1.0 / s1);
-    const double invrho = s1 * T * Rp;
 #pragma unroll
-    for (int i = 0; i < NV; i++) {
-      const int c = g + L * i;
-      if (c >= 1 && c < n) sR[c * G] = rho * yw[i];
+    for (int o = L / 2; o > 0; o >>= 1) {
+#pragma unroll
+      for (int q = 0; q < M; q++) {
+        s1[q] += __shfl_xor_sync(mask, s1[q], o);
+        s2[q] += __shfl_xor_sync(mask, s2[q], o);
+      }
+    }
+    /* R9a: ideal gas at constant pressure: rho = p / (Ru T sum_k Y_k/W_k), C_k = rho Y_k / W_k */
+    double ctot[M], invrho[M];
+#pragma unroll
+    for (int q = 0; q < M; q++) {
+      ctot[q] = pR[q] * invT[q];
+      const double rho = ctot[q] * (1.0 / s1[q]);
+      invrho[q] = s1[q] * T[q] * Rp[q];
+#pragma unroll
+      for (int i = 0; i < NV; i++) {
+        const int c = g + L * i;
+        if (c >= 1 && c < n) sR[q * RS + c * G] = rho * yw[q][i];
+      }
     }
     gsync();
     /* R22: [M] = sum_k alpha_k C_k = C_tot + sum_listed (alpha_k - 1) C_k, one value per efficiency set */
     for (int r = 0; r < m.NTBR; r++) {
-      double M = ctot;
+      double Mc[M];
+#pragma unroll
+      for (int q = 0; q < M; q++) Mc[q] = ctot[q];
       int b = m.o_tb + r * m.TBE * 2 * L + g;
-      for (int e = 0; e < m.TBE; e++, b += 2 * L) M = fma(td(b), sR[(int)tw(b + L)], M);
+      for (int e = 0; e < m.TBE; e++, b += 2 * L) {
+        const double am1 = td(b);
+        const int off = (int)tw(b + L);
+#pragma unroll
+        for (int q = 0; q < M; q++) Mc[q] = fma(am1, sR[q * RS + off], Mc[q]);
+      }
       const int t = r * L + g;
-      if (t < m.NTB) sR[(n + t) * G] = M;
+      if (t < m.NTB) {
+#pragma unroll
+        for (int q = 0; q < M; q++) sR[q * RS + (n + t) * G] = Mc[q];
+      }
     }
     gsync();
     /* Eq. 4-5: q_s = [M] (k_f prod C_reactants - k_r prod C_products); absent molecules point at C_0 = 1 */
     {
       constexpr int US = CKB_UNROLL_SLOTS;
       int b = m.o_sl + g;
-      double *q = sQ + g * G;
+      double *qp = sR + qoff + g * G;
 #pragma unroll US
-      for (int r = 0; r < m.NSR; r++, b += CKB_SL_WORDS * L, q += L * G) {
-        const double xf = fma(-td(b + CKB_SL_THF * L), invT, fma(td(b + CKB_SL_BF * L), lnT, td(b + CKB_SL_LNAF * L)));
-        const double xr = fma(-td(b + CKB_SL_THR * L), invT, fma(td(b + CKB_SL_BR * L), lnT, td(b + CKB_SL_LNAR * L)));
+      for (int r = 0; r < m.NSR; r++, b += CKB_SL_WORDS * L, qp += L * G) {
+        const double lnAf = td(b + CKB_SL_LNAF * L), bf = td(b + CKB_SL_BF * L), thf = td(b + CKB_SL_THF * L);
+        const double lnAr = td(b + CKB_SL_LNAR * L), br = td(b + CKB_SL_BR * L), thr = td(b + CKB_SL_THR * L);
         const unsigned long long wa = tw(b + CKB_SL_IDXA * L), wb = tw(b + CKB_SL_IDXB * L);
         const unsigned alo = (unsigned)wa, ahi = (unsigned)(wa >> 32), blo = (unsigned)wb, bhi = (unsigned)(wb >> 32);
-        const double pf = sR[alo & 0xFFFFu] * sR[alo >> 16] * sR[ahi & 0xFFFFu];
-        const double pr = sR[blo & 0xFFFFu] * sR[blo >> 16] * sR[bhi & 0xFFFFu];
-        const double kf = ckb_exp(xf), kr = ckb_exp(xr);
-        *q = (kf * pf - kr * pr) * sR[ahi >> 16];
+        const unsigned a0 = alo & 0xFFFFu, a1 = alo >> 16, a2 = ahi & 0xFFFFu, tb = ahi >> 16;
+        const unsigned b0 = blo & 0xFFFFu, b1 = blo >> 16, b2 = bhi & 0xFFFFu;
+#pragma unroll
+        for (int q = 0; q < M; q++) {
+          const double *c = sR + q * RS;
+          const double xf = fma(-thf, invT[q], fma(bf, lnT[q], lnAf));
+          const double xr = fma(-thr, invT[q], fma(br, lnT[q], lnAr));
+          const double pf = c[a0] * c[a1] * c[a2];
+          const double pr = c[b0] * c[b1] * c[b2];
+          const double kf = ckb_exp(xf), kr = ckb_exp(xr);
+          qp[q * RS] = (kf * pf - kr * pr) * c[tb];
+        }
       }
     }
     gsync();
     /* Eq. 3: omega_c = sum_s (nu''_cs - nu'_cs) q_s (gather);  Eq. 2: dY_k/dt = W_k omega_k / rho */
-    double s3 = 0.0;
+    double s3[M];
+#pragma unroll
+    for (int q = 0; q < M; q++) s3[q] = 0.0;
     int gp = m.o_gat + g;
+    const double *sQ = sR + qoff;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       const int len = (int)tw(m.o_glen + i);
-      double acc0 = 0.0, acc1 = 0.0;
+      double acc0[M], acc1[M];
+#pragma unroll
+      for (int q = 0; q < M; q++) acc0[q] = acc1[q] = 0.0;
       if (L == 1) { /* one entry per word: double coefficient, low 16 mantissa bits = q offset (a constant-bank operand) */
         for (int t = 0; t < len; t++, gp += L) {
           const unsigned long long w = tw(gp);
-          acc0 = fma(__longlong_as_double((long long)(w & ~0xFFFFull)), sQ[(unsigned)w & 0xFFFFu], acc0);
+          const double coef = __longlong_as_double((long long)(w & ~0xFFFFull));
+          const unsigned o = (unsigned)w & 0xFFFFu;
+#pragma unroll
+          for (int q = 0; q < M; q++) acc0[q] = fma(coef, sQ[q * RS + o], acc0[q]);
         }
       } else { /* two entries per word: (int16 coefficient << 16) | q offset */
         for (int t = 0; t < len; t++, gp += L) {
           const unsigned long long w = tw(gp);
           const unsigned lo = (unsigned)w, hi = (unsigned)(w >> 32);
-          acc0 = fma((double)((int)lo >> 16), sQ[lo & 0xFFFFu], acc0);
-          acc1 = fma((double)((int)hi >> 16), sQ[hi & 0xFFFFu], acc1);
+          const double c0 = (double)((int)lo >> 16), c1 = (double)((int)hi >> 16);
+          const unsigned o0 = lo & 0xFFFFu, o1 = hi & 0xFFFFu;
+#pragma unroll
+          for (int q = 0; q < M; q++) {
+            acc0[q] = fma(c0, sQ[q * RS + o0], acc0[q]);
+            acc1[q] = fma(c1, sQ[q * RS + o1], acc1[q]);
+          }
         }
       }
-      const double acc = acc0 + acc1;
-      f[i] = td(m.o_sp + i * CKB_SP_WORDS * L + g + CKB_SP_W * L) * acc * invrho;
-      s3 = fma(hrt[i], acc, s3);
+      const double W = td(m.o_sp + i * CKB_SP_WORDS * L + g + CKB_SP_W * L);
+#pragma unroll
+      for (int q = 0; q < M; q++) {
+        const double acc = acc0[q] + acc1[q];
+        f[q][i] = W * acc * invrho[q];
+        s3[q] = fma(hrt[q][i], acc, s3[q]);
+      }
     }
-    s3 = gsum(s3);
+#pragma unroll
+    for (int o = L / 2; o > 0; o >>= 1) {
+#pragma unroll
+      for (int q = 0; q < M; q++) s3[q] += __shfl_xor_sync(mask, s3[q], o);
+    }
     /* Eq. 6: dT/dt = -(Ru T sum_k (h_k/RT) omega_k) / (rho cp), cp = Ru sum_k Y_k (cp_k/R) / W_k */
-    if (g == 0) f[0] = -(T * s3 * invrho) / s2;
+    if (g == 0) {
+#pragma unroll
+      for (int q = 0; q < M; q++) f[q][0] = -(T[q] * s3[q] * invrho[q]) / s2[q];
+    }
   }
 };
 
@@ -707,18 +775,21 @@ struct Rkc {
 
 template <class S>
 __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem) {
-  constexpr int L = S::L, G = S::G;
+  constexpr int L = S::L, G = S::G, M = S::M;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int grp = lane / L;
   sys.g = lane % L;
   sys.src0 = grp * L;
   sys.mask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (grp * L));
-  const int per_warp = region_doubles(m) * G;
-  sys.sR = smem + (size_t)warp * per_warp + grp;
-  sys.sQ = sys.sR + (m.n + m.NTB + 1) * G;
+  sys.RS = region_doubles(m) * G;
+  sys.qoff = (m.n + m.NTB + 1) * G;
+  sys.sR = smem + (size_t)warp * sys.RS * M + grp;
   if (sys.g == 0) {
-    sys.sR[0] = 1.0;                   /* "absent molecule" concentration */
-    sys.sR[(m.n + m.NTB) * G] = 1.0;   /* "no third body" */
+#pragma unroll
+    for (int q = 0; q < M; q++) {
+      sys.sR[q * sys.RS] = 1.0;                         /* "absent molecule" concentration */
+      sys.sR[q * sys.RS + (m.n + m.NTB) * G] = 1.0;     /* "no third body" */
+    }
   }
   sys.gsync();
 }
@@ -728,59 +799,89 @@ struct IntegratorOf { typedef Rkck<S> type; };
 template <class S>
 struct IntegratorOf<S, 1> { typedef Rkc<S> type; };
 
-template <int L, int NV, class TAB, int METHOD>
+template <int L, int NV, class TAB, int METHOD, int M>
 __global__ void __launch_bounds__(CKB_BLOCK, CKB_MINB)
 integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, double *__restrict__ states,
                  const double *__restrict__ pressure, double p_uniform, long long N, long long ld, double t0,
                  double dt, double rtol, double atol, int *__restrict__ status, int *__restrict__ stats,
                  unsigned long long *__restrict__ counter, const int *__restrict__ order) {
   extern __shared__ double smem[];
-  typedef Sys<L, NV, TAB> S;
+  typedef Sys<L, NV, TAB, M> S;
   S sys(m, tab);
   sys_setup(sys, m, smem);
   constexpr int G = S::G;
-  const long long n_groups = (long long)gridDim.x * (CKB_BLOCK / 32) * G;
-  long long qi = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L;
-  long long ode = 0;
-  typename IntegratorOf<S, METHOD>::type integ;
-  bool need_load = true;
-  double f[NV];
+  /* queue positions: every group starts with M of its own, then pulls from the counter */
+  const long long n_static = (long long)gridDim.x * (CKB_BLOCK / 32) * G * M;
+  const long long grp_id = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L;
+  typename IntegratorOf<S, METHOD>::type integ[M];
+  long long qi[M], ode[M];
+  bool need_load[M], active[M];
+  double y[M][NV], f[M][NV];
+#pragma unroll
+  for (int q = 0; q < M; q++) {
+    qi[q] = grp_id * M + q;
+    ode[q] = 0;
+    need_load[q] = true;
+    active[q] = true;
+    sys.set_pressure(q, 1.0);
+#pragma unroll
+    for (int i = 0; i < NV; i++) y[q][i] = 0.0;
+  }
   while (true) {
-    if (need_load) {
-      if (qi >= N) break;
-      ode = order ? (long long)order[qi] : qi; /* queue position -> system */
-      sys.set_pressure(pressure ? pressure[ode] : p_uniform);
-      double y0[NV];
+    bool any = false;
 #pragma unroll
-      for (int i = 0; i < NV; i++) {
-        const int c = sys.g + L * i;
-        y0[i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode] : 0.0;
-      }
-      integ.start(y0, t0, t0 + dt, rtol, atol, m.n);
-      need_load = false;
-    }
-    sys.rhs(integ.w, f);
-    if (integ.advance(sys, f)) {
-      int st[4];
-      integ.result(st);
+    for (int q = 0; q < M; q++) {
+      if (need_load[q] && active[q]) {
+        if (qi[q] >= N) {
+          active[q] = false; /* queue exhausted: this slot idles (its f(y) input stays at the last finite state) */
+        } else {
+          ode[q] = order ? (long long)order[qi[q]] : qi[q]; /* queue position -> system */
+          sys.set_pressure(q, pressure ? pressure[ode[q]] : p_uniform);
+          double y0[NV];
 #pragma unroll
-      for (int i = 0; i < NV; i++) {
-        const int c = sys.g + L * i;
-        if (c < m.n) states[(size_t)sys.tw(m.o_perm + c) * ld + ode] = integ.y[i];
-      }
-      if (sys.g == 0) {
-        if (status) status[ode] = integ.status;
-        if (stats) {
-#pragma unroll
-          for (int q = 0; q < 4; q++) stats[(size_t)q * N + ode] = st[q];
+          for (int i = 0; i < NV; i++) {
+            const int c = sys.g + L * i;
+            y0[i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode[q]] : 0.0;
+          }
+          integ[q].start(y0, t0, t0 + dt, rtol, atol, m.n);
+          need_load[q] = false;
         }
       }
-      /* next system: lane refill (L = 1) / group refill */
-      unsigned long long nx = 0;
-      if (sys.g == 0) nx = atomicAdd(counter, 1ull);
-      if (L > 1) nx = __shfl_sync(sys.mask, nx, sys.src0);
-      qi = n_groups + (long long)nx;
-      need_load = true;
+      any = any || active[q];
+    }
+    if (!any) break;
+#pragma unroll
+    for (int q = 0; q < M; q++) {
+      if (active[q]) {
+#pragma unroll
+        for (int i = 0; i < NV; i++) y[q][i] = integ[q].w[i];
+      }
+    }
+    sys.rhs(y, f);
+#pragma unroll
+    for (int q = 0; q < M; q++) {
+      if (active[q] && integ[q].advance(sys, f[q])) {
+        int st[4];
+        integ[q].result(st);
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+          const int c = sys.g + L * i;
+          if (c < m.n) states[(size_t)sys.tw(m.o_perm + c) * ld + ode[q]] = integ[q].y[i];
+        }
+        if (sys.g == 0) {
+          if (status) status[ode[q]] = integ[q].status;
+          if (stats) {
+#pragma unroll
+            for (int k = 0; k < 4; k++) stats[(size_t)k * N + ode[q]] = st[k];
+          }
+        }
+        /* next system: lane refill (L = 1) / group refill */
+        unsigned long long nx = 0;
+        if (sys.g == 0) nx = atomicAdd(counter, 1ull);
+        if (L > 1) nx = __shfl_sync(sys.mask, nx, sys.src0);
+        qi[q] = n_static + (long long)nx;
+        need_load[q] = true;
+      }
     }
   }
 }
@@ -791,30 +892,30 @@ rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, c
            const double *__restrict__ pressure, double p_uniform, long long N, long long ld,
            double *__restrict__ dydt, int repeat) {
   extern __shared__ double smem[];
-  typedef Sys<L, NV, TAB> S;
+  typedef Sys<L, NV, TAB, 1> S;
   S sys(m, tab);
   sys_setup(sys, m, smem);
   const long long ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * S::G + (threadIdx.x & 31) / L;
   if (ode >= N) return;
-  sys.set_pressure(pressure ? pressure[ode] : p_uniform);
-  double y[NV], f[NV];
+  sys.set_pressure(0, pressure ? pressure[ode] : p_uniform);
+  double y[1][NV], f[1][NV];
 #pragma unroll
   for (int i = 0; i < NV; i++) {
     const int c = sys.g + L * i;
-    y[i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode] : 0.0;
+    y[0][i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode] : 0.0;
   }
   for (int r = 0; r < repeat; r++) {
     sys.rhs(y, f);
     if (r + 1 < repeat) {
       /* keep the repeats from being folded: feed a zero-weight dependence on f back into y */
 #pragma unroll
-      for (int i = 0; i < NV; i++) y[i] = fma(f[i], 0.0, y[i]);
+      for (int i = 0; i < NV; i++) y[0][i] = fma(f[0][i], 0.0, y[0][i]);
     }
   }
 #pragma unroll
   for (int i = 0; i < NV; i++) {
     const int c = sys.g + L * i;
-    if (c < m.n) dydt[(size_t)sys.tw(m.o_perm + c) * ld + ode] = f[i];
+    if (c < m.n) dydt[(size_t)sys.tw(m.o_perm + c) * ld + ode] = f[0][i];
   }
 }
 

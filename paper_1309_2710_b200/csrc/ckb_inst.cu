@@ -8,6 +8,9 @@
 #include "ckb_device.cuh"
 #include "ckb_host.h"
 
+#ifndef CKB_M
+#define CKB_M 1 /* systems evaluated together per group */
+#endif
 #ifndef CKB_L
 #error "compile with -DCKB_L=.. -DCKB_NV=.."
 #endif
@@ -28,9 +31,9 @@ typedef ckb::GlobalTab Tab;
 
 static const Packed &pack_of(const ckb_mech *m) { return m->pk[pack_index(L)]; }
 
-static size_t smem_bytes(const ckb_mech *m) {
+static size_t smem_bytes(const ckb_mech *m, int M) {
   const ckb::DevMech &dm = pack_of(m).dm;
-  return (size_t)ckb::region_doubles(dm) * (32 / L) * (CKB_BLOCK / 32) * sizeof(double);
+  return (size_t)ckb::region_doubles(dm) * (32 / L) * M * (CKB_BLOCK / 32) * sizeof(double);
 }
 
 template <class KERN>
@@ -43,15 +46,15 @@ static int prep(KERN kern, size_t smem) {
 static void make_tab(const ckb_mech *m, ckb::ParamTab &t) { std::memcpy(t.w, pack_of(m).blob.data(), pack_of(m).blob.size() * 8); }
 static void make_tab(const ckb_mech *m, ckb::GlobalTab &t) { t.p = pack_of(m).d_blob; }
 
-static long long n_blocks(long long N) {
-  const long long per_block = (long long)(CKB_BLOCK / 32) * (32 / L);
+static long long n_blocks(long long N, int M) {
+  const long long per_block = (long long)(CKB_BLOCK / 32) * (32 / L) * M;
   return (N + per_block - 1) / per_block;
 }
 
 template <int METHOD>
 static int launch(const ckb_mech *m, const IntegrateArgs &a) {
-  auto kern = ckb::integrate_kernel<L, NV, Tab, METHOD>;
-  const size_t smem = smem_bytes(m);
+  auto kern = ckb::integrate_kernel<L, NV, Tab, METHOD, CKB_M>;
+  const size_t smem = smem_bytes(m, CKB_M);
   int rc = prep(kern, smem);
   if (rc) return rc;
   /* persistent grid: resident capacity of the device (a multiple of the SM count), capped by the batch */
@@ -65,7 +68,7 @@ static int launch(const ckb_mech *m, const IntegrateArgs &a) {
     resident = sms * per_sm;
     resident_smem = (int)smem;
   }
-  long long blocks = n_blocks(a.N);
+  long long blocks = n_blocks(a.N, CKB_M);
   if (blocks > resident) blocks = resident;
   unsigned long long *counter = m->d_counters + (m->next_counter.fetch_add(1) % CKB_COUNTER_RING);
   CK(cudaMemsetAsync(counter, 0, 8, a.stream));
@@ -85,10 +88,10 @@ int CKB_CAT(integrate_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, int method, cons
 
 int CKB_CAT(rhs_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const RhsArgs &a) {
   auto kern = ckb::rhs_kernel<L, NV, Tab>;
-  const size_t smem = smem_bytes(m);
+  const size_t smem = smem_bytes(m, 1);
   int rc = prep(kern, smem);
   if (rc) return rc;
-  const long long blocks = n_blocks(a.N);
+  const long long blocks = n_blocks(a.N, 1);
   if (blocks > 2147483647LL) return CKB_EINVAL;
   Tab tab;
   make_tab(m, tab);
