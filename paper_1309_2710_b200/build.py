@@ -53,6 +53,7 @@ def min_blocks(L: int, NV: int) -> int:
 
 def _digest(extra: str) -> str:
     h = hashlib.sha256(extra.encode())
+    h.update(open(os.path.abspath(__file__), "rb").read())  # the per-instantiation knobs live in this file
     for root in (CSRC, os.path.join(HERE, "..", "include")):
         for fn in sorted(os.listdir(root)):
             if fn.endswith((".cu", ".cuh", ".h")):
