@@ -99,13 +99,15 @@ struct Sys {
   __device__ __forceinline__ bool valid(int i) const { return g + L * i < m.n; }
 
   /* f(y): Eq. 2-6 for the M systems of the group.  y, f: [system][slot], component (g + L*i) in slot i. */
-  __device__ __forceinline__ void rhs(const double (&y)[M][NV], double (&f)[M][NV]) {
+  /* Y(q, i): slot i of the argument of system q (read in place from the integrators' registers) */
+  template <class GetY>
+  __device__ __forceinline__ void rhs(GetY Y, double (&f)[M][NV]) {
     const int n = m.n;
     double T[M], invT[M], lnT[M], s1[M], s2[M];
     double hrt[M][NV], yw[M][NV];
 #pragma unroll
     for (int q = 0; q < M; q++) {
-      T[q] = bcast0(y[q][0]);
+      T[q] = bcast0(Y(q, 0));
       invT[q] = 1.0 / T[q];
       lnT[q] = log(T[q]);
       s1[q] = 0.0;
@@ -131,7 +133,7 @@ struct Sys {
           h = fma(h, T[q], hc[k]);
         }
         h = fma(hc[5], invT[q], h);
-        const double v = y[q][i] * iw; /* Y_k / W_k */
+        const double v = Y(q, i) * iw; /* Y_k / W_k */
         yw[q][i] = v;
         hrt[q][i] = h;
         s1[q] += v;
@@ -192,15 +194,24 @@ struct Sys {
         const unsigned alo = (unsigned)wa, ahi = (unsigned)(wa >> 32), blo = (unsigned)wb, bhi = (unsigned)(wb >> 32);
         const unsigned a0 = alo & 0xFFFFu, a1 = alo >> 16, a2 = ahi & 0xFFFFu, tb = ahi >> 16;
         const unsigned b0 = blo & 0xFFFFu, b1 = blo >> 16, b2 = bhi & 0xFFFFu;
+        /* round flags, same for every lane (uniform branches); thread-per-ODE reads are conflict-free broadcasts
+           anyway, so there the branches would only cost */
+        const unsigned fl = (L == 1) ? 3u : (unsigned)tw(m.o_rflag + r);
 #pragma unroll
         for (int q = 0; q < M; q++) {
           const double *c = sR + q * RS;
           const double xf = fma(-thf, invT[q], fma(bf, lnT[q], lnAf));
           const double xr = fma(-thr, invT[q], fma(br, lnT[q], lnAr));
-          const double pf = c[a0] * c[a1] * c[a2];
-          const double pr = c[b0] * c[b1] * c[b2];
+          double pf = c[a0] * c[a1];
+          double pr = c[b0] * c[b1];
+          if (fl & 1u) {
+            pf *= c[a2];
+            pr *= c[b2];
+          }
           const double kf = ckb_exp(xf), kr = ckb_exp(xr);
-          qp[q * RS] = (kf * pf - kr * pr) * c[tb];
+          double qv = kf * pf - kr * pr;
+          if (fl & 2u) qv *= c[tb];
+          qp[q * RS] = qv;
         }
       }
     }
@@ -816,7 +827,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
   typename IntegratorOf<S, METHOD>::type integ[M];
   long long qi[M], ode[M];
   bool need_load[M], active[M];
-  double y[M][NV], f[M][NV];
+  double f[M][NV];
 #pragma unroll
   for (int q = 0; q < M; q++) {
     qi[q] = grp_id * M + q;
@@ -825,7 +836,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
     active[q] = true;
     sys.set_pressure(q, 1.0);
 #pragma unroll
-    for (int i = 0; i < NV; i++) y[q][i] = 0.0;
+    for (int i = 0; i < NV; i++) integ[q].w[i] = 1.0; /* finite argument for a slot that never gets a system */
   }
   while (true) {
     bool any = false;
@@ -850,14 +861,8 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
       any = any || active[q];
     }
     if (!any) break;
-#pragma unroll
-    for (int q = 0; q < M; q++) {
-      if (active[q]) {
-#pragma unroll
-        for (int i = 0; i < NV; i++) y[q][i] = integ[q].w[i];
-      }
-    }
-    sys.rhs(y, f);
+    /* an idle slot (queue exhausted) keeps evaluating its last argument: harmless, never stored */
+    sys.rhs([&](int q, int i) -> double { return integ[q].w[i]; }, f);
 #pragma unroll
     for (int q = 0; q < M; q++) {
       if (active[q] && integ[q].advance(sys, f[q])) {
@@ -905,7 +910,7 @@ rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, c
     y[0][i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode] : 0.0;
   }
   for (int r = 0; r < repeat; r++) {
-    sys.rhs(y, f);
+    sys.rhs([&](int, int i) -> double { return y[0][i]; }, f);
     if (r + 1 < repeat) {
       /* keep the repeats from being folded: feed a zero-weight dependence on f back into y */
 #pragma unroll

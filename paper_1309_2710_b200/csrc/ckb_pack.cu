@@ -213,13 +213,30 @@ std::vector<Placed> place_slots(const Parsed &P, const std::vector<int> &comp_of
     }
   };
   if (!optimise || L != 32) {
-    for (int s = 0; s < NS; s++) {
-      out[s].slot = s;
-      comps(s, out[s].a, out[s].b);
+    std::vector<int> order(NS);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int u, int v) {
+      auto c = [&](int s) {
+        const Rx &x = P.rx[P.slots[s].f];
+        return (x.reac.size() > 2 || (P.slots[s].r >= 0 && x.prod.size() > 2)) ? 0 : (x.tbset >= 0 ? 1 : 2);
+      };
+      return c(u) < c(v);
+    });
+    for (int q = 0; q < NS; q++) {
+      out[q].slot = order[q];
+      comps(order[q], out[q].a, out[q].b);
+      std::sort(out[q].a, out[q].a + 3, std::greater<int>()); /* present molecules first */
+      std::sort(out[q].b, out[q].b + 3, std::greater<int>());
     }
     return out;
   }
   std::vector<char> used(NS, 0);
+  std::vector<int> cls(NS, 2);
+  for (int s = 0; s < NS; s++) {
+    const Rx &x = P.rx[P.slots[s].f];
+    if (x.reac.size() > 2 || (P.slots[s].r >= 0 && x.prod.size() > 2)) cls[s] = 0;
+    else if (x.tbset >= 0) cls[s] = 1;
+  }
   int left = NS;
   for (int r = 0; r < NSR && left > 0; r++) {
     for (int h = 0; h < 2 && left > 0; h++) {
@@ -229,13 +246,19 @@ std::vector<Placed> place_slots(const Parsed &P, const std::vector<int> &comp_of
         for (int &v : row) v = 0;
       for (int l = 0; l < 16 && left > 0; l++) {
         int best = -1, best_cost = 1 << 30, best_a[3] = {0, 0, 0}, best_b[3] = {0, 0, 0};
+        /* slots are handed out class by class (third molecule first, then third body, then the rest), so that
+           whole rounds can skip the reads they do not need (per-round flags) */
+        int cur_class = 3;
+        for (int s = 0; s < NS; s++)
+          if (!used[s]) cur_class = std::min(cur_class, cls[s]);
         for (int s = 0; s < NS && best_cost > 0; s++) {
-          if (used[s]) continue;
+          if (used[s] || cls[s] != cur_class) continue;
           int a[3], b[3];
           comps(s, a, b);
           std::sort(a, a + 3, std::greater<int>());
           std::sort(b, b + 3, std::greater<int>());
           /* try every order of the molecules on each side */
+          const int na = (a[0] != 0) + (a[1] != 0) + (a[2] != 0), nb = (b[0] != 0) + (b[1] != 0) + (b[2] != 0);
           int pa[3] = {a[0], a[1], a[2]};
           do {
             int ca = 0;
@@ -251,8 +274,8 @@ std::vector<Placed> place_slots(const Parsed &P, const std::vector<int> &comp_of
                 best = s;
                 for (int q = 0; q < 3; q++) { best_a[q] = pa[q]; best_b[q] = pb[q]; }
               }
-            } while (std::prev_permutation(pb, pb + 3));
-          } while (std::prev_permutation(pa, pa + 3));
+            } while (std::prev_permutation(pb, pb + nb));
+          } while (std::prev_permutation(pa, pa + na));
         }
         Placed &pl = out[(size_t)r * 32 + h * 16 + l];
         pl.slot = best;
@@ -420,6 +443,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   m.o_tb = take((size_t)NTBR * TBE * 2 * L);
   m.o_gat = take((size_t)gwords * L);
   m.o_glen = take(NV);
+  m.o_rflag = off; off += NSR;
   m.o_perm = off; off += n;
   m.s_tab = s_tab;
   m.o_rkc = off; off += s_tab - 1;
@@ -471,6 +495,11 @@ int pack_for(const Parsed &P, int L, Packed &out) {
     }
     b[(size_t)base + CKB_SL_IDXA * L] = wa;
     b[(size_t)base + CKB_SL_IDXB * L] = wb;
+    /* round flags: 1 = some slot of the round reads a third molecule, 2 = some slot has a third body */
+    if (pl.slot >= 0) {
+      if (pl.a[2] || pl.b[2]) b[(size_t)m.o_rflag + r] |= 1ull;
+      if (P.rx[P.slots[pl.slot].f].tbset >= 0) b[(size_t)m.o_rflag + r] |= 2ull;
+    }
   }
   for (int t = 0; t < NTBR * L; t++) { /* third-body sets, padded with (alpha - 1) = 0 on C_0 */
     const int r = t / L, g = t % L;

@@ -66,6 +66,7 @@ struct DevMech {
   int NTB, NTBR, TBE;/* third-body sets, set rounds = ceil(NTB / L), listed entries per set (padded)      */
   int o_sp;          /* [NV][13][L]        species table                                                  */
   int o_sl;          /* [NSR][8][L]        slot table                                                     */
+  int o_rflag;       /* [NSR]              round flags: 1 = a third molecule is read, 2 = a third body is read   */
   int o_tb;          /* [NTBR][TBE][2][L]  (alpha-1, region offset of the species)                        */
   int o_glen;        /* [NV]               64-bit words per lane of gather level i (uniform over lanes)   */
   int o_gat;         /* [sum glen][L]      gather entries.  L > 1: two per word, (int16 coefficient << 16) |
