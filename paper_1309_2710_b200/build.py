@@ -40,9 +40,13 @@ def systems_per_group(L: int, NV: int) -> int:
     return int(os.environ.get("CKB_M32", "1")) if L == 32 else 1
 
 
-def min_blocks(L: int, NV: int) -> int:
+def min_blocks(L: int, NV: int, method: str = "rkck") -> int:
     """Resident 128-thread blocks per SM that the register allocation of integrate_kernel<L, NV> must allow
     (launch bounds): 4 -> <= 128 registers, 3 -> <= 168, 2 -> <= 255.  Chosen so that no instantiation spills."""
+    if L == 1:  # thread-per-ODE: k3..k5 (RKCK) / v (RKC) sit in shared scratch so that 3 blocks fit
+        if method == "rkc":
+            return 2
+        return int(os.environ.get("CKB_MINB_L1", "3")) if NV <= 14 else 2
     doubles = NV * systems_per_group(L, NV)  # register slots per stage vector
     if doubles <= int(os.environ.get("CKB_MINB4_MAXNV", "2")):
         return int(os.environ.get("CKB_MINB_SMALL", "4"))
@@ -74,7 +78,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     os.makedirs(OBJ, exist_ok=True)
     flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("CKB_DEFS", "").split()  # tuning knobs
     stamp = os.path.join(OBJ, "stamp")
-    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", ""))
+    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", ""))
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     jobs = []
@@ -83,7 +87,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
         jobs.append((obj, [NVCC, *flags, "-c", os.path.join(CSRC, src), "-o", obj]))
     for (L, NV) in instantiations():
         obj = os.path.join(OBJ, f"ckb_inst_L{L}_NV{NV}.o")
-        jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_MINB={min_blocks(L, NV)}",
+        jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_MINB={min_blocks(L, NV)}", f"-DCKB_MINB_RKC={min_blocks(L, NV, 'rkc')}",
                            f"-DCKB_UNROLL_SLOTS={1 if L == 1 else int(os.environ.get('CKB_US', '1'))}",
                            f"-DCKB_M={systems_per_group(L, NV)}", "-c",
                            os.path.join(CSRC, "ckb_inst.cu"), "-o", obj]))

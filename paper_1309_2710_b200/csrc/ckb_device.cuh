@@ -66,6 +66,9 @@ struct Sys {
   double *sR;      /* shared region of system 0 of this group (ckb_tables.h), element e at sR[e*G]; system q at + q*RS */
   int RS;          /* doubles between the regions of two systems of the group */
   int qoff;        /* (n + NTB + 1) * G: start of the q region */
+  double *sX;      /* scratch of the integrator behind the region (XVec), same interleave */
+  double *sH;      /* thread-per-ODE: h_k/(RT) parked here between the two halves of f(y) instead of in registers */
+  static constexpr int HDOUBLES = (L_ == 1) ? NV_ : 0;
   unsigned mask;   /* lanes of this group */
   int g;           /* lane within the group */
   int src0;        /* warp lane that holds component 0 (T) */
@@ -104,7 +107,7 @@ struct Sys {
   __device__ __forceinline__ void rhs(GetY Y, double (&f)[M][NV]) {
     const int n = m.n;
     double T[M], invT[M], lnT[M], s1[M], s2[M];
-    double hrt[M][NV], yw[M][NV];
+    double hrt[M][L == 1 ? 1 : NV], yw[M][L == 1 ? 1 : NV];
 #pragma unroll
     for (int q = 0; q < M; q++) {
       T[q] = bcast0(Y(q, 0));
@@ -134,8 +137,12 @@ struct Sys {
         }
         h = fma(hc[5], invT[q], h);
         const double v = Y(q, i) * iw; /* Y_k / W_k */
-        yw[q][i] = v;
-        hrt[q][i] = h;
+        if (L == 1) {
+          sH[i * G] = h;
+        } else {
+          yw[q][i] = v;
+          hrt[q][i] = h;
+        }
         s1[q] += v;
         s2[q] = fma(v, cp, s2[q]);
       }
@@ -158,7 +165,8 @@ struct Sys {
 #pragma unroll
       for (int i = 0; i < NV; i++) {
         const int c = g + L * i;
-        if (c >= 1 && c < n) sR[q * RS + c * G] = rho * yw[q][i];
+        if (c >= 1 && c < n)
+          sR[q * RS + c * G] = rho * (L == 1 ? Y(q, i) * td(m.o_sp + i * CKB_SP_WORDS * L + g + CKB_SP_INVW * L) : yw[q][i]);
       }
     }
     gsync();
@@ -254,7 +262,7 @@ struct Sys {
       for (int q = 0; q < M; q++) {
         const double acc = acc0[q] + acc1[q];
         f[q][i] = W * acc * invrho[q];
-        s3[q] = fma(hrt[q][i], acc, s3[q]);
+        s3[q] = fma(L == 1 ? sH[i * G] : hrt[q][i], acc, s3[q]);
       }
     }
 #pragma unroll
@@ -292,6 +300,21 @@ struct Sys {
  * The arithmetic and the order of the controller decisions follow DESIGN.md section 4 step by step.
  * ============================================================================================== */
 
+/* A stage vector that lives in registers, or -- for thread-per-ODE, where registers per thread are what limits
+ * the resident warps -- in the system's shared scratch area sX (interleaved like the region: conflict free). */
+template <class S, int SLOT, bool IN_SMEM>
+struct XVec {
+  double r[IN_SMEM ? 1 : S::NV];
+  __device__ __forceinline__ double get(const S &sys, int i) const {
+    if (IN_SMEM) return sys.sX[(SLOT * S::NV + i) * S::G];
+    return r[IN_SMEM ? 0 : i];
+  }
+  __device__ __forceinline__ void set(const S &sys, int i, double x) {
+    if (IN_SMEM) sys.sX[(SLOT * S::NV + i) * S::G] = x;
+    else r[IN_SMEM ? 0 : i] = x;
+  }
+};
+
 /* RKCK: Eq. 7-17, Table 1; R1-R7, R25. */
 template <class S>
 struct Rkck {
@@ -309,7 +332,12 @@ struct Rkck {
   static constexpr double SAFETY = 0.9; /* P:144 */
 
   double w[NV];                 /* the next argument of f */
-  double y[NV], k1[NV], k2[NV], k3[NV], k4[NV], k5[NV];
+  static constexpr bool XS = (S::L == 1); /* k3..k5 in shared scratch */
+  static constexpr int XDOUBLES = XS ? 3 * NV : 0;
+  double y[NV], k1[NV], k2[NV];
+  XVec<S, 0, XS> k3;
+  XVec<S, 1, XS> k4;
+  XVec<S, 2, XS> k5;
   double t, h, t1, rtol, atol;
   int stage, nfe, nacc, nrej, attempts, status;
   bool last, saw_nonfinite;
@@ -378,24 +406,27 @@ struct Rkck {
       case 3:
 #pragma unroll
         for (int i = 0; i < NV; i++) {
-          k3[i] = h * f[i];
-          w[i] = fma(B43, k3[i], fma(B42, k2[i], fma(B41, k1[i], y[i])));
+          const double k3i = h * f[i];
+          k3.set(sys, i, k3i);
+          w[i] = fma(B43, k3i, fma(B42, k2[i], fma(B41, k1[i], y[i])));
         }
         stage = 4;
         return false;
       case 4:
 #pragma unroll
         for (int i = 0; i < NV; i++) {
-          k4[i] = h * f[i];
-          w[i] = fma(B54, k4[i], fma(B53, k3[i], fma(B52, k2[i], fma(B51, k1[i], y[i]))));
+          const double k4i = h * f[i], k3i = k3.get(sys, i);
+          k4.set(sys, i, k4i);
+          w[i] = fma(B54, k4i, fma(B53, k3i, fma(B52, k2[i], fma(B51, k1[i], y[i]))));
         }
         stage = 5;
         return false;
       case 5:
 #pragma unroll
         for (int i = 0; i < NV; i++) {
-          k5[i] = h * f[i];
-          w[i] = fma(B65, k5[i], fma(B64, k4[i], fma(B63, k3[i], fma(B62, k2[i], fma(B61, k1[i], y[i])))));
+          const double k5i = h * f[i], k3i = k3.get(sys, i), k4i = k4.get(sys, i);
+          k5.set(sys, i, k5i);
+          w[i] = fma(B65, k5i, fma(B64, k4i, fma(B63, k3i, fma(B62, k2[i], fma(B61, k1[i], y[i])))));
         }
         stage = 6;
         return false;
@@ -407,8 +438,9 @@ struct Rkck {
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       const double k6 = h * f[i];
-      const double yn = fma(C6, k6, fma(C4, k4[i], fma(C3, k3[i], fma(C1, k1[i], y[i]))));
-      const double dl = fma(D6, k6, fma(D5, k5[i], fma(D4, k4[i], fma(D3, k3[i], D1 * k1[i]))));
+      const double k3i = k3.get(sys, i), k4i = k4.get(sys, i), k5i = k5.get(sys, i);
+      const double yn = fma(C6, k6, fma(C4, k4i, fma(C3, k3i, fma(C1, k1[i], y[i]))));
+      const double dl = fma(D6, k6, fma(D5, k5i, fma(D4, k4i, fma(D3, k3i, D1 * k1[i]))));
       w[i] = yn;
       if (sys.valid(i)) {
         const double d0 = fma(rtol, fabs(y[i]) + fabs(k1[i]), atol);
@@ -491,7 +523,10 @@ struct Rkc {
   enum { S_F0 = 1, S_PM = 2, S_H0 = 3, S_STAGE = 4, S_FINAL = 5 };
 
   double w[NV];                                   /* the next argument of f: y, z (power method), w_{j-1} */
-  double y[NV], f0[NV], wjm2[NV], v[NV];
+  static constexpr bool XS = (S::L == 1); /* eigenvector estimate v in shared scratch */
+  static constexpr int XDOUBLES = XS ? NV : 0;
+  double y[NV], f0[NV], wjm2[NV];
+  XVec<S, 0, XS> v;
   double t, h, t1, Dt, rtol, atol, nd;
   double sigma, err_old, h_old;
   double pm_d, pm_sigma;                          /* power method: displacement size, last estimate */
@@ -521,20 +556,21 @@ struct Rkc {
   __device__ __forceinline__ void pm_begin(const S &sys, bool have_v, bool initial) {
     if (!have_v) {
 #pragma unroll
-      for (int i = 0; i < NV; i++) v[i] = f0[i];
+      for (int i = 0; i < NV; i++) v.set(sys, i, f0[i]);
     }
     double a = 0.0, b = 0.0;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       a = fma(y[i], y[i], a);
-      b = fma(v[i], v[i], b);
+      const double vi = v.get(sys, i);
+      b = fma(vi, vi, b);
     }
     const double ynrm = sqrt(sys.gsum(a)), vnrm = sqrt(sys.gsum(b));
     if (ynrm != 0.0 && vnrm != 0.0) {
       pm_d = ynrm * CKB_SQRTU;
       const double r = pm_d / vnrm;
 #pragma unroll
-      for (int i = 0; i < NV; i++) w[i] = fma(v[i], r, y[i]);
+      for (int i = 0; i < NV; i++) w[i] = fma(v.get(sys, i), r, y[i]);
     } else if (ynrm != 0.0) {
       pm_d = ynrm * CKB_SQRTU;
 #pragma unroll
@@ -543,7 +579,7 @@ struct Rkc {
       pm_d = CKB_U;
       const double r = pm_d / vnrm;
 #pragma unroll
-      for (int i = 0; i < NV; i++) w[i] = v[i] * r;
+      for (int i = 0; i < NV; i++) w[i] = v.get(sys, i) * r;
     } else {
       pm_d = CKB_U;
 #pragma unroll
@@ -653,7 +689,7 @@ struct Rkc {
           }
         }
 #pragma unroll
-        for (int i = 0; i < NV; i++) v[i] = w[i] - y[i];
+        for (int i = 0; i < NV; i++) v.set(sys, i, w[i] - y[i]);
         sigma = 1.2 * pm_sigma; /* R18 */
         sigma_fresh = true;
         need_sigma = false;
@@ -783,18 +819,23 @@ struct Rkc {
 #ifndef CKB_MINB
 #define CKB_MINB 1 /* resident blocks per SM the register allocation must allow (set per instantiation) */
 #endif
+#ifndef CKB_MINB_RKC
+#define CKB_MINB_RKC CKB_MINB /* the same for the RKC kernels (more controller state) */
+#endif
 
 template <class S>
-__device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem) {
+__device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem, int xdoubles) {
   constexpr int L = S::L, G = S::G, M = S::M;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int grp = lane / L;
   sys.g = lane % L;
   sys.src0 = grp * L;
   sys.mask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (grp * L));
-  sys.RS = region_doubles(m) * G;
+  sys.RS = (region_doubles(m) + xdoubles) * G;
   sys.qoff = (m.n + m.NTB + 1) * G;
   sys.sR = smem + (size_t)warp * sys.RS * M + grp;
+  sys.sX = sys.sR + region_doubles(m) * G;
+  sys.sH = sys.sX + (xdoubles - S::HDOUBLES) * G;
   if (sys.g == 0) {
 #pragma unroll
     for (int q = 0; q < M; q++) {
@@ -811,7 +852,7 @@ template <class S>
 struct IntegratorOf<S, 1> { typedef Rkc<S> type; };
 
 template <int L, int NV, class TAB, int METHOD, int M>
-__global__ void __launch_bounds__(CKB_BLOCK, CKB_MINB)
+__global__ void __launch_bounds__(CKB_BLOCK, METHOD == 0 ? CKB_MINB : CKB_MINB_RKC)
 integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, double *__restrict__ states,
                  const double *__restrict__ pressure, double p_uniform, long long N, long long ld, double t0,
                  double dt, double rtol, double atol, int *__restrict__ status, int *__restrict__ stats,
@@ -819,7 +860,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
   extern __shared__ double smem[];
   typedef Sys<L, NV, TAB, M> S;
   S sys(m, tab);
-  sys_setup(sys, m, smem);
+  sys_setup(sys, m, smem, IntegratorOf<S, METHOD>::type::XDOUBLES + S::HDOUBLES);
   constexpr int G = S::G;
   /* queue positions: every group starts with M of its own, then pulls from the counter */
   const long long n_static = (long long)gridDim.x * (CKB_BLOCK / 32) * G * M;
@@ -899,7 +940,7 @@ rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, c
   extern __shared__ double smem[];
   typedef Sys<L, NV, TAB, 1> S;
   S sys(m, tab);
-  sys_setup(sys, m, smem);
+  sys_setup(sys, m, smem, S::HDOUBLES);
   const long long ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * S::G + (threadIdx.x & 31) / L;
   if (ode >= N) return;
   sys.set_pressure(0, pressure ? pressure[ode] : p_uniform);

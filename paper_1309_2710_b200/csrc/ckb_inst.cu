@@ -31,9 +31,9 @@ typedef ckb::GlobalTab Tab;
 
 static const Packed &pack_of(const ckb_mech *m) { return m->pk[pack_index(L)]; }
 
-static size_t smem_bytes(const ckb_mech *m, int M) {
+static size_t smem_bytes(const ckb_mech *m, int M, int xdoubles) {
   const ckb::DevMech &dm = pack_of(m).dm;
-  return (size_t)ckb::region_doubles(dm) * (32 / L) * M * (CKB_BLOCK / 32) * sizeof(double);
+  return (size_t)(ckb::region_doubles(dm) + xdoubles) * (32 / L) * M * (CKB_BLOCK / 32) * sizeof(double);
 }
 
 template <class KERN>
@@ -54,7 +54,7 @@ static long long n_blocks(long long N, int M) {
 template <int METHOD>
 static int launch(const ckb_mech *m, const IntegrateArgs &a) {
   auto kern = ckb::integrate_kernel<L, NV, Tab, METHOD, CKB_M>;
-  const size_t smem = smem_bytes(m, CKB_M);
+  const size_t smem = smem_bytes(m, CKB_M, ckb::IntegratorOf<ckb::Sys<L, NV, Tab, CKB_M>, METHOD>::type::XDOUBLES + ckb::Sys<L, NV, Tab, CKB_M>::HDOUBLES);
   int rc = prep(kern, smem);
   if (rc) return rc;
   /* persistent grid: resident capacity of the device (a multiple of the SM count), capped by the batch */
@@ -88,7 +88,7 @@ int CKB_CAT(integrate_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, int method, cons
 
 int CKB_CAT(rhs_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const RhsArgs &a) {
   auto kern = ckb::rhs_kernel<L, NV, Tab>;
-  const size_t smem = smem_bytes(m, 1);
+  const size_t smem = smem_bytes(m, 1, ckb::Sys<L, NV, Tab, 1>::HDOUBLES);
   int rc = prep(kern, smem);
   if (rc) return rc;
   const long long blocks = n_blocks(a.N, 1);
