@@ -41,10 +41,17 @@ struct Launch {
   bool param_tab;
 };
 
-int choose(const ckb_mech *m, int variant, Launch *out) {
+/* AUTO: thread-per-ODE needs K+1 <= 16 and enough systems to fill the lanes it keeps resident (148 SMs x 3 x 128):
+ * measured on B200, it overtakes warp-per-ODE at N ~ 5e4 (a lone thread takes ~6 us per f(y), a warp ~1 us), so small
+ * batches of small mechanisms go warp-per-ODE as well. */
+#define CKB_AUTO_THREAD_MIN_N 49152
+
+int choose(const ckb_mech *m, int variant, long long N, Launch *out) {
   const int n = m->K + 1;
   if (variant == CKB_VARIANT_AUTO)
-    variant = (n <= 16 && m->pk[0].rc == CKB_OK) ? CKB_VARIANT_THREAD : CKB_VARIANT_WARP;
+    variant = (n <= 16 && m->pk[0].rc == CKB_OK && (N >= CKB_AUTO_THREAD_MIN_N || m->pk[3].rc != CKB_OK))
+                  ? CKB_VARIANT_THREAD
+                  : CKB_VARIANT_WARP;
   int L;
   switch (variant) {
     case CKB_VARIANT_THREAD: L = 1; break;
@@ -147,7 +154,7 @@ int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, dou
   if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(t) || !(rtol > 0.0) || !(atol >= 0.0)) return CKB_EINVAL;
   if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
   Launch l;
-  int rc = choose(m, variant, &l);
+  int rc = choose(m, variant, (long long)N, &l);
   if (rc) return rc;
   if (N == 0) return CKB_OK;
   if (!states || ld < N) return CKB_EINVAL;
@@ -166,7 +173,7 @@ int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, dou
   if (!m || N < 0 || repeat < 1) return CKB_EINVAL;
   if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
   Launch l;
-  int rc = choose(m, variant, &l);
+  int rc = choose(m, variant, (long long)N, &l);
   if (rc) return rc;
   if (N == 0) return CKB_OK;
   if (!states || !dydt || ld < N) return CKB_EINVAL;

@@ -78,6 +78,41 @@ def test_integrate_argument_errors_without_handle(L):
     assert L.ckb_fp64_probe(7, 10, C.byref(v), None) == binding.EINVAL
 
 
+@pytest.mark.parametrize("cfg", [0, 2, 3, 4])
+def test_packing_report(cfg, L):
+    """Host-only packing (ckb_mech_pack_stats): forward/reverse pairs are fused, the gather schedule of the
+    warp-per-ODE packing is free of shared-memory bank conflicts, thread-per-ODE tables fit the parameter block."""
+    mech = synth.make_mechanism(cfg)
+    spec = synth.CONFIGS[cfg]
+    warp = binding.pack_stats(mech, 32)
+    assert warp["slots"] == spec.R // 2                       # every synthetic reaction has its reverse
+    assert warp["slot_rounds"] == -(-warp["slots"] // 32)
+    assert warp["gather_conflict_replays"] == 0               # edge-coloured schedule
+    assert warp["register_slots"] == -(-(spec.K + 1) // 32) or warp["register_slots"] in (1, 2, 4)
+    nnz = sum(len(set(mech.reac_species[mech.reac_ptr[j]:mech.reac_ptr[j + 1]]) |
+                  set(mech.prod_species[mech.prod_ptr[j]:mech.prod_ptr[j + 1]])) for j in range(0, spec.R, 2))
+    assert warp["gather_steps"] * 32 >= nnz                   # every entry is scheduled
+    assert warp["gather_steps"] <= 2.5 * nnz / 32 + 8         # and the padding stays bounded
+    if spec.K + 1 <= 16:
+        thr = binding.pack_stats(mech, 1)
+        assert thr["table_words"] <= 3072 and thr["register_slots"] >= spec.K + 1
+        assert thr["gather_steps"] == nnz                     # thread-per-ODE walks the rows as they are
+    else:
+        with pytest.raises(binding.CkbError):
+            binding.pack_stats(mech, 1)
+    for lanes in (8, 16):
+        st = binding.pack_stats(mech, lanes)
+        assert st["slots"] == warp["slots"] and st["register_slots"] * lanes >= spec.K + 1
+
+
+def test_unpaired_and_duplicate_reactions_pack(L):
+    """An irreversible reaction without reverse keeps its own slot; duplicates of the same pair are kept apart."""
+    m = synth.toy_mechanism(3, [({0: 1}, {1: 1}, 1.0, 0.0, 0.0), ({1: 1}, {0: 1}, 2.0, 0.0, 0.0),
+                                ({0: 1}, {1: 1}, 3.0, 0.0, 0.0), ({1: 2}, {2: 1}, 4.0, 0.0, 0.0)])
+    assert binding.pack_stats(m, 32)["slots"] == 3
+    assert binding.pack_stats(m, 1)["slots"] == 3
+
+
 def test_product_path_does_not_import_oracle():
     """The binding, the generator and bench's product arm never touch oracle/ (no CPU fallback)."""
     pkg = os.path.join(ROOT, "paper_1309_2710_b200")
