@@ -37,14 +37,35 @@ static __constant__ double c_expq[10] = {
     0.0013888888917367081, 0.00019841269863171557, 2.4801521057868204e-05, 2.7557268276905696e-06,
     2.7620201591031547e-07, 2.5100472505694996e-08};
 
-__device__ __forceinline__ double ckb_exp(double x) {
-  const double t = fma(x, 1.4426950408889634, 6755399441055744.0); /* 1.5 * 2^52: round to nearest integer */
-  const double kd = t - 6755399441055744.0;
-  double r = fma(kd, -0.6931471805599453, x);
-  r = fma(kd, -2.3190468138462996e-17, r);
-  double p = c_expq[9];
+/* The constants of ckb_exp: either operands from the constant bank (PIN = false; thread-per-ODE, where registers
+ * are scarce) or pinned in registers for the duration of the slot loop (PIN = true; otherwise the compiler
+ * re-materialises them with ~12 extra instructions per reaction slot). */
+template <bool PIN>
+struct ExpConst {
+  double log2e, ln2hi, ln2lo, q[10];
+  __device__ __forceinline__ ExpConst() {
+    log2e = 1.4426950408889634;
+    ln2hi = -0.6931471805599453;
+    ln2lo = -2.3190468138462996e-17;
 #pragma unroll
-  for (int i = 8; i >= 0; i--) p = fma(p, r, c_expq[i]);
+    for (int i = 0; i < 10; i++) q[i] = c_expq[i];
+    if (PIN) {
+      asm volatile("" : "+d"(log2e), "+d"(ln2hi), "+d"(ln2lo));
+#pragma unroll
+      for (int i = 0; i < 10; i++) asm volatile("" : "+d"(q[i]));
+    }
+  }
+};
+
+template <bool PIN>
+__device__ __forceinline__ double ckb_exp(double x, const ExpConst<PIN> &c) {
+  const double t = fma(x, c.log2e, 6755399441055744.0); /* 1.5 * 2^52: round to nearest integer */
+  const double kd = t - 6755399441055744.0;
+  double r = fma(kd, c.ln2hi, x);
+  r = fma(kd, c.ln2lo, r);
+  double p = c.q[9];
+#pragma unroll
+  for (int i = 8; i >= 0; i--) p = fma(p, r, c.q[i]);
   p = fma(p, r, 1.0);
   p = fma(p, r, 1.0);
   int k = __double2loint(t);
@@ -178,9 +199,10 @@ struct Sys {
       int b = m.o_tb + r * m.TBE * 2 * L + g;
       for (int e = 0; e < m.TBE; e++, b += 2 * L) {
         const double am1 = td(b);
-        const int off = (int)tw(b + L);
+        const unsigned off = (unsigned)tw(b + L); /* byte offset */
 #pragma unroll
-        for (int q = 0; q < M; q++) Mc[q] = fma(am1, sR[q * RS + off], Mc[q]);
+        for (int q = 0; q < M; q++)
+          Mc[q] = fma(am1, *reinterpret_cast<const double *>(reinterpret_cast<const char *>(sR + q * RS) + off), Mc[q]);
       }
       const int t = r * L + g;
       if (t < m.NTB) {
@@ -189,9 +211,11 @@ struct Sys {
       }
     }
     gsync();
-    /* Eq. 4-5: q_s = [M] (k_f prod C_reactants - k_r prod C_products); absent molecules point at C_0 = 1 */
+    /* Eq. 4-5: q_s = [M] (k_f prod C_reactants - k_r prod C_products); absent molecules point at C_0 = 1, an
+     * absent third body at a 1.0.  The 16-bit fields are BYTE offsets into the system's region. */
     {
       constexpr int US = CKB_UNROLL_SLOTS;
+      const ExpConst<(L > 1)> ec;
       int b = m.o_sl + g;
       double *qp = sR + qoff + g * G;
 #pragma unroll US
@@ -202,24 +226,17 @@ struct Sys {
         const unsigned alo = (unsigned)wa, ahi = (unsigned)(wa >> 32), blo = (unsigned)wb, bhi = (unsigned)(wb >> 32);
         const unsigned a0 = alo & 0xFFFFu, a1 = alo >> 16, a2 = ahi & 0xFFFFu, tb = ahi >> 16;
         const unsigned b0 = blo & 0xFFFFu, b1 = blo >> 16, b2 = bhi & 0xFFFFu;
-        /* round flags, same for every lane (uniform branches); thread-per-ODE reads are conflict-free broadcasts
-           anyway, so there the branches would only cost */
-        const unsigned fl = (L == 1) ? 3u : (unsigned)tw(m.o_rflag + r);
 #pragma unroll
         for (int q = 0; q < M; q++) {
-          const double *c = sR + q * RS;
+          const char *c = reinterpret_cast<const char *>(sR + q * RS);
+#define CKB_AT(off) (*reinterpret_cast<const double *>(c + (off)))
           const double xf = fma(-thf, invT[q], fma(bf, lnT[q], lnAf));
           const double xr = fma(-thr, invT[q], fma(br, lnT[q], lnAr));
-          double pf = c[a0] * c[a1];
-          double pr = c[b0] * c[b1];
-          if (fl & 1u) {
-            pf *= c[a2];
-            pr *= c[b2];
-          }
-          const double kf = ckb_exp(xf), kr = ckb_exp(xr);
-          double qv = kf * pf - kr * pr;
-          if (fl & 2u) qv *= c[tb];
-          qp[q * RS] = qv;
+          const double pf = CKB_AT(a0) * CKB_AT(a1) * CKB_AT(a2);
+          const double pr = CKB_AT(b0) * CKB_AT(b1) * CKB_AT(b2);
+          const double kf = ckb_exp(xf, ec), kr = ckb_exp(xr, ec);
+          qp[q * RS] = (kf * pf - kr * pr) * CKB_AT(tb);
+#undef CKB_AT
         }
       }
     }
@@ -242,7 +259,8 @@ struct Sys {
           const double coef = __longlong_as_double((long long)(w & ~0xFFFFull));
           const unsigned o = (unsigned)w & 0xFFFFu;
 #pragma unroll
-          for (int q = 0; q < M; q++) acc0[q] = fma(coef, sQ[q * RS + o], acc0[q]);
+          for (int q = 0; q < M; q++)
+            acc0[q] = fma(coef, *reinterpret_cast<const double *>(reinterpret_cast<const char *>(sQ + q * RS) + o), acc0[q]);
         }
       } else { /* two entries per word: (int16 coefficient << 16) | q offset */
         for (int t = 0; t < len; t++, gp += L) {
@@ -252,8 +270,9 @@ struct Sys {
           const unsigned o0 = lo & 0xFFFFu, o1 = hi & 0xFFFFu;
 #pragma unroll
           for (int q = 0; q < M; q++) {
-            acc0[q] = fma(c0, sQ[q * RS + o0], acc0[q]);
-            acc1[q] = fma(c1, sQ[q * RS + o1], acc1[q]);
+            const char *qb = reinterpret_cast<const char *>(sQ + q * RS);
+            acc0[q] = fma(c0, *reinterpret_cast<const double *>(qb + o0), acc0[q]);
+            acc1[q] = fma(c1, *reinterpret_cast<const double *>(qb + o1), acc1[q]);
           }
         }
       }

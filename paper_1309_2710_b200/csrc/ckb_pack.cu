@@ -393,8 +393,8 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   if (NV < 0) return CKB_EUNSUPPORTED;
   int TBE = 0;
   for (auto &s : P.sets) TBE = std::max(TBE, (int)s.size());
-  /* 16-bit region offsets */
-  if ((long long)(n + NTB) * G > 65535 || (long long)NSR * L * G > 65535) return CKB_EUNSUPPORTED;
+  /* 16-bit region offsets, in bytes */
+  if ((long long)(n + NTB) * G * 8 > 65535 || (long long)NSR * L * G * 8 > 65535) return CKB_EUNSUPPORTED;
   const bool optimise = true;
 
   /* components: 0 = T, then species by decreasing gather-row length */
@@ -483,15 +483,15 @@ int pack_for(const Parsed &P, int L, Packed &out) {
       putd(base + CKB_SL_BR * L, rv >= 0 ? P.beta[rv] : 0.0);
       putd(base + CKB_SL_THR * L, rv >= 0 ? P.E[rv] / RC_CAL : 0.0);
       for (int k = 0; k < 3; k++) {
-        wa |= (unsigned long long)(pl.a[k] * G) << (16 * k);
-        wb |= (unsigned long long)(pl.b[k] * G) << (16 * k);
+        wa |= (unsigned long long)(pl.a[k] * G * 8) << (16 * k);
+        wb |= (unsigned long long)(pl.b[k] * G * 8) << (16 * k);
       }
       const int ts = P.rx[f].tbset;
-      wa |= (unsigned long long)((n + (ts >= 0 ? ts : NTB)) * G) << 48;
+      wa |= (unsigned long long)((n + (ts >= 0 ? ts : NTB)) * G * 8) << 48;
     } else { /* padding slot: q = 0 */
       putd(base + CKB_SL_LNAF * L, LN_ZERO);
       putd(base + CKB_SL_LNAR * L, LN_ZERO);
-      wa = (unsigned long long)((n + NTB) * G) << 48;
+      wa = (unsigned long long)((n + NTB) * G * 8) << 48;
     }
     b[(size_t)base + CKB_SL_IDXA * L] = wa;
     b[(size_t)base + CKB_SL_IDXB * L] = wb;
@@ -507,7 +507,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
       const int base = m.o_tb + ((r * TBE + e) * 2) * L + g;
       if (t < NTB && e < (int)P.sets[t].size()) {
         putd(base, P.sets[t][e].second - 1.0);
-        b[(size_t)base + L] = (unsigned long long)(comp_of_sp[P.sets[t][e].first] * G);
+        b[(size_t)base + L] = (unsigned long long)(comp_of_sp[P.sets[t][e].first] * G * 8);
       }
     }
   }
@@ -541,10 +541,10 @@ int pack_for(const Parsed &P, int L, Packed &out) {
           if (L == 32) addr[g] = e.pos;
           if (L == 1) { /* double coefficient with the q offset in its 16 lowest mantissa bits */
             b[(size_t)m.o_gat + (size_t)(w0 + t) * L + g] =
-                (dbits((double)e.coef) & ~0xFFFFull) | (unsigned long long)(e.pos * G);
+                (dbits((double)e.coef) & ~0xFFFFull) | (unsigned long long)(e.pos * G * 8);
           } else {
             const unsigned long long ent =
-                ((unsigned long long)((unsigned)(e.coef & 0xFFFF)) << 16) | (unsigned long long)(e.pos * G);
+                ((unsigned long long)((unsigned)(e.coef & 0xFFFF)) << 16) | (unsigned long long)(e.pos * G * 8);
             b[(size_t)m.o_gat + (size_t)(w0 + t / 2) * L + g] |= ent << (32 * (t & 1));
           }
         }

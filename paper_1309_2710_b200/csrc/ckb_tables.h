@@ -54,7 +54,7 @@ struct GlobalTab {
 #define CKB_SL_LNAR 3 /* -inf when the slot has no reverse reaction */
 #define CKB_SL_BR 4
 #define CKB_SL_THR 5
-#define CKB_SL_IDXA 6 /* 16-bit fields: region offsets (in doubles, x G) of reactant molecules 0,1,2 and of [M] */
+#define CKB_SL_IDXA 6 /* 16-bit fields: region BYTE offsets (x G) of reactant molecules 0,1,2 and of [M] */
 #define CKB_SL_IDXB 7 /* 16-bit fields: product molecules 0,1,2; field 3 unused                              */
 #define CKB_SL_WORDS 8
 
@@ -67,10 +67,10 @@ struct DevMech {
   int o_sp;          /* [NV][13][L]        species table                                                  */
   int o_sl;          /* [NSR][8][L]        slot table                                                     */
   int o_rflag;       /* [NSR]              round flags: 1 = a third molecule is read, 2 = a third body is read   */
-  int o_tb;          /* [NTBR][TBE][2][L]  (alpha-1, region offset of the species)                        */
+  int o_tb;          /* [NTBR][TBE][2][L]  (alpha-1, region byte offset of the species)                        */
   int o_glen;        /* [NV]               64-bit words per lane of gather level i (uniform over lanes)   */
   int o_gat;         /* [sum glen][L]      gather entries.  L > 1: two per word, (int16 coefficient << 16) |
-                                           offset (in doubles, x G) of q_s inside the q region; L = 1: one
+                                           BYTE offset (x G) of q_s inside the q region; L = 1: one
                                            per word, double coefficient with the offset in its low 16 bits */
   int o_rkc;         /* RKC coefficients for s = 2..s_tab: [s-2] -> mu~_1; stages at o_rkcs               */
   int o_rkcs;        /* [(s-2)(s-1)/2 + (j-2)][4] = mu_j, nu_j, mu~_j, gamma~_j, j = 2..s                  */
