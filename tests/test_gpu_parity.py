@@ -166,6 +166,36 @@ def test_queue_refill_and_order_large_batch():
     assert np.abs(a[0][0] - b[0][0])[same].max() <= 1e-8 * 2000
 
 
+@pytest.mark.parametrize("cfg,n_sample", [(1, 4000), (2, 1500), (3, 160), (4, 64)])
+def test_full_size_sampled(cfg, n_sample):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (AUTO variant, uniform pressure, no
+    stats-free shortcut): sampled systems against the oracle one by one, invariants on all of them."""
+    import torch
+    from paper_1309_2710_b200 import binding
+    spec = synth.CONFIGS[cfg]
+    N = {1: 1 << 19, 2: 1 << 18, 3: 1 << 17, 4: 1 << 16}[cfg]
+    mech = synth.make_mechanism(cfg)
+    states, p = synth.make_states(cfg, N)
+    m = binding.mech_load(mech)
+    dev = torch.from_numpy(states).cuda()
+    stats = torch.zeros((4, N), dtype=torch.int32, device="cuda")
+    status = torch.full((N,), -1, dtype=torch.int32, device="cuda")
+    binding.integrate(m, dev, spec.dt[0], RTOL, ATOL, spec.method, p=p, status=status, stats=stats)
+    torch.cuda.synchronize()
+    y, st, stt = dev.cpu().numpy(), status.cpu().numpy(), stats.cpu().numpy()
+    m.close()
+    assert np.isin(st, (0, 4)).all() and np.isfinite(y).all()
+    assert np.abs(y[1:].sum(0) - 1.0).max() < 1e-11                       # sum Y conserved (linear invariant)
+    aw = np.array([synth.ATOMIC_WEIGHT[e] for e in mech.elements])
+    Z = lambda s_: (mech.elem_counts * aw).T @ (s_[1:] / mech.mol_weight[:, None])
+    assert np.abs(Z(y) - Z(states)).max() < 1e-11                          # element mass conserved
+    assert (stt[0] > 0).all() and (stt[1] >= 1).all()
+    pick = np.random.default_rng(11 + cfg).choice(N, size=n_sample, replace=False)
+    ora = _oracle(mech, np.ascontiguousarray(states[:, pick]), p, spec.dt[0], spec.method)
+    rep = _compare((y[:, pick], st[pick], stt[:, pick]), ora, max_flip_frac=5e-3)
+    print(f"full size cfg{cfg} N={N}: {rep}")
+
+
 def test_empty_and_single():
     import torch
     from paper_1309_2710_b200 import binding
