@@ -82,11 +82,14 @@ struct Sys {
   /* M systems share the lanes of a group and are evaluated together: every table word is loaded and decoded
    * once for all of them, and their (independent) dependency chains interleave -- DESIGN.md 6.5. */
   static constexpr int L = L_, NV = NV_, G = 32 / L_, M = M_;
+  /* shared-memory interleave: thread-per-ODE interleaves the 32 systems of a warp element by element (conflict
+   * free: all lanes read the same element); lane-distributed mappings give every system a contiguous region */
+  static constexpr int GI = (L_ == 1) ? 32 : 1;
   const DevMech &m;
   const TAB &tab;
   double *sR;      /* shared region of system 0 of this group (ckb_tables.h), element e at sR[e*G]; system q at + q*RS */
   int RS;          /* doubles between the regions of two systems of the group */
-  int qoff;        /* (n + NTB + 1) * G: start of the q region */
+  int qoff;        /* (n + NTB + 1) * GI: start of the q region */
   double *sX;      /* scratch of the integrator behind the region (XVec), same interleave */
   double *sH;      /* thread-per-ODE: h_k/(RT) parked here between the two halves of f(y) instead of in registers */
   static constexpr int HDOUBLES = (L_ == 1) ? NV_ : 0;
@@ -159,7 +162,7 @@ struct Sys {
         h = fma(hc[5], invT[q], h);
         const double v = Y(q, i) * iw; /* Y_k / W_k */
         if (L == 1) {
-          sH[i * G] = h;
+          sH[i * GI] = h;
         } else {
           yw[q][i] = v;
           hrt[q][i] = h;
@@ -187,7 +190,7 @@ struct Sys {
       for (int i = 0; i < NV; i++) {
         const int c = g + L * i;
         if (c >= 1 && c < n)
-          sR[q * RS + c * G] = rho * (L == 1 ? Y(q, i) * td(m.o_sp + i * CKB_SP_WORDS * L + g + CKB_SP_INVW * L) : yw[q][i]);
+          sR[q * RS + c * GI] = rho * (L == 1 ? Y(q, i) * td(m.o_sp + i * CKB_SP_WORDS * L + g + CKB_SP_INVW * L) : yw[q][i]);
       }
     }
     gsync();
@@ -207,7 +210,7 @@ struct Sys {
       const int t = r * L + g;
       if (t < m.NTB) {
 #pragma unroll
-        for (int q = 0; q < M; q++) sR[q * RS + (n + t) * G] = Mc[q];
+        for (int q = 0; q < M; q++) sR[q * RS + (n + t) * GI] = Mc[q];
       }
     }
     gsync();
@@ -217,9 +220,9 @@ struct Sys {
       constexpr int US = CKB_UNROLL_SLOTS;
       const ExpConst<(L > 1)> ec;
       int b = m.o_sl + g;
-      double *qp = sR + qoff + g * G;
+      double *qp = sR + qoff + g * GI;
 #pragma unroll US
-      for (int r = 0; r < m.NSR; r++, b += CKB_SL_WORDS * L, qp += L * G) {
+      for (int r = 0; r < m.NSR; r++, b += CKB_SL_WORDS * L, qp += L * GI) {
         const double lnAf = td(b + CKB_SL_LNAF * L), bf = td(b + CKB_SL_BF * L), thf = td(b + CKB_SL_THF * L);
         const double lnAr = td(b + CKB_SL_LNAR * L), br = td(b + CKB_SL_BR * L), thr = td(b + CKB_SL_THR * L);
         const unsigned long long wa = tw(b + CKB_SL_IDXA * L), wb = tw(b + CKB_SL_IDXB * L);
@@ -281,7 +284,7 @@ struct Sys {
       for (int q = 0; q < M; q++) {
         const double acc = acc0[q] + acc1[q];
         f[q][i] = W * acc * invrho[q];
-        s3[q] = fma(L == 1 ? sH[i * G] : hrt[q][i], acc, s3[q]);
+        s3[q] = fma(L == 1 ? sH[i * GI] : hrt[q][i], acc, s3[q]);
       }
     }
 #pragma unroll
@@ -325,11 +328,11 @@ template <class S, int SLOT, bool IN_SMEM>
 struct XVec {
   double r[IN_SMEM ? 1 : S::NV];
   __device__ __forceinline__ double get(const S &sys, int i) const {
-    if (IN_SMEM) return sys.sX[(SLOT * S::NV + i) * S::G];
+    if (IN_SMEM) return sys.sX[(SLOT * S::NV + i) * S::GI];
     return r[IN_SMEM ? 0 : i];
   }
   __device__ __forceinline__ void set(const S &sys, int i, double x) {
-    if (IN_SMEM) sys.sX[(SLOT * S::NV + i) * S::G] = x;
+    if (IN_SMEM) sys.sX[(SLOT * S::NV + i) * S::GI] = x;
     else r[IN_SMEM ? 0 : i] = x;
   }
 };
@@ -826,7 +829,7 @@ struct Rkc {
 
 /* ------------------------------------------------------------------------------------------------
  * Kernels.  Block = CKB_BLOCK threads; a warp holds G = 32/L systems at a time.
- * Shared memory per warp: region_doubles(m) * G doubles (ckb_tables.h).
+ * Shared memory per warp: (region_doubles(m) + scratch) * G * M doubles (ckb_tables.h).
  *
  * integrate_kernel is persistent: the grid is sized to the resident capacity of the GPU (a multiple of the
  * SM count) and every group of L lanes pulls system indices -- first its own global group index, then
@@ -850,16 +853,18 @@ __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem
   sys.g = lane % L;
   sys.src0 = grp * L;
   sys.mask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (grp * L));
-  sys.RS = (region_doubles(m) + xdoubles) * G;
-  sys.qoff = (m.n + m.NTB + 1) * G;
-  sys.sR = smem + (size_t)warp * sys.RS * M + grp;
-  sys.sX = sys.sR + region_doubles(m) * G;
-  sys.sH = sys.sX + (xdoubles - S::HDOUBLES) * G;
+  constexpr int GI = S::GI;
+  sys.RS = (region_doubles(m) + xdoubles) * GI;
+  sys.qoff = (m.n + m.NTB + 1) * GI;
+  /* per warp: G groups x M systems x (region + scratch); interleaved by lane (GI = 32) or one after the other */
+  sys.sR = smem + (size_t)warp * (region_doubles(m) + xdoubles) * G * M + (GI == 1 ? grp * sys.RS * M : grp);
+  sys.sX = sys.sR + region_doubles(m) * GI;
+  sys.sH = sys.sX + (xdoubles - S::HDOUBLES) * GI;
   if (sys.g == 0) {
 #pragma unroll
     for (int q = 0; q < M; q++) {
-      sys.sR[q * sys.RS] = 1.0;                         /* "absent molecule" concentration */
-      sys.sR[q * sys.RS + (m.n + m.NTB) * G] = 1.0;     /* "no third body" */
+      sys.sR[q * sys.RS] = 1.0;                          /* "absent molecule" concentration */
+      sys.sR[q * sys.RS + (m.n + m.NTB) * GI] = 1.0;     /* "no third body" */
     }
   }
   sys.gsync();

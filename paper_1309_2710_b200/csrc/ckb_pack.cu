@@ -212,7 +212,7 @@ std::vector<Placed> place_slots(const Parsed &P, const std::vector<int> &comp_of
       b[q] = (rev && q < (int)x.prod.size()) ? comp_of_sp[x.prod[q]] : 0;
     }
   };
-  if (!optimise || L != 32) {
+  if (!optimise || L < 16) {
     std::vector<int> order(NS);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int u, int v) {
@@ -239,7 +239,7 @@ std::vector<Placed> place_slots(const Parsed &P, const std::vector<int> &comp_of
   }
   int left = NS;
   for (int r = 0; r < NSR && left > 0; r++) {
-    for (int h = 0; h < 2 && left > 0; h++) {
+    for (int h = 0; h < L / 16 && left > 0; h++) {
       /* comp_at[k][bp] = component already read through bank pair bp by instruction k in this half-warp (0 = free) */
       int comp_at[6][16];
       for (auto &row : comp_at)
@@ -277,7 +277,7 @@ std::vector<Placed> place_slots(const Parsed &P, const std::vector<int> &comp_of
             } while (std::prev_permutation(pb, pb + nb));
           } while (std::prev_permutation(pa, pa + na));
         }
-        Placed &pl = out[(size_t)r * 32 + h * 16 + l];
+        Placed &pl = out[(size_t)r * L + h * 16 + l];
         pl.slot = best;
         for (int q = 0; q < 3; q++) {
           pl.a[q] = best_a[q];
@@ -300,14 +300,14 @@ struct GEntry { int pos, coef; };
 std::vector<std::vector<GEntry>> colour_gather(const std::vector<std::vector<GEntry>> &rows, int L, bool optimise) {
   size_t maxlen = 0;
   for (auto &r : rows) maxlen = std::max(maxlen, r.size());
-  if (!optimise || L != 32) {
+  if (!optimise || L < 16) {
     std::vector<std::vector<GEntry>> steps(maxlen, std::vector<GEntry>(L, GEntry{-1, 0}));
     for (int g = 0; g < L; g++)
       for (size_t t = 0; t < rows[g].size(); t++) steps[t][g] = rows[g][t];
     return steps;
   }
   std::vector<std::vector<GEntry>> steps;
-  for (int h = 0; h < 2; h++) {
+  for (int h = 0; h < L / 16; h++) {
     /* degrees */
     int deg_l[16] = {0}, deg_r[16] = {0};
     for (int l = 0; l < 16; l++)
@@ -358,7 +358,7 @@ std::vector<std::vector<GEntry>> colour_gather(const std::vector<std::vector<GEn
         at_r[ca][bp] = l;
       }
     }
-    if ((int)steps.size() < D) steps.resize(D, std::vector<GEntry>(32, GEntry{-1, 0}));
+    if ((int)steps.size() < D) steps.resize(D, std::vector<GEntry>(L, GEntry{-1, 0}));
     for (int c = 0; c < D; c++)
       for (int l = 0; l < 16; l++)
         if (at_l[c][l] >= 0) steps[c][h * 16 + l] = rows[h * 16 + l][at_l[c][l]];
@@ -367,9 +367,9 @@ std::vector<std::vector<GEntry>> colour_gather(const std::vector<std::vector<GEn
 }
 
 /* bank-pair collisions a schedule causes (excess wavefronts of 64-bit half-warp accesses), for the packing report */
-int excess_wavefronts(const std::vector<int> &addr_of_lane /* 32 entries, -1 = none */) {
+int excess_wavefronts(const std::vector<int> &addr_of_lane /* L entries (L = 16 or 32), -1 = none */) {
   int excess = 0;
-  for (int h = 0; h < 2; h++) {
+  for (int h = 0; h < (int)addr_of_lane.size() / 16; h++) {
     std::map<int, std::vector<int>> by_bp;
     for (int l = 0; l < 16; l++) {
       const int a = addr_of_lane[h * 16 + l];
@@ -387,7 +387,8 @@ int excess_wavefronts(const std::vector<int> &addr_of_lane /* 32 entries, -1 = n
 }  // namespace
 
 int pack_for(const Parsed &P, int L, Packed &out) {
-  const int K = P.K, n = K + 1, G = 32 / L;
+  const int K = P.K, n = K + 1;
+  const int G = (L == 1) ? 32 : 1; /* shared-memory interleave of the region (Sys::GI) */
   const int NS = (int)P.slots.size(), NTB = (int)P.sets.size();
   const int NV = pick_nv(L, n), NSR = (NS + L - 1) / L, NTBR = (NTB + L - 1) / L;
   if (NV < 0) return CKB_EUNSUPPORTED;
@@ -520,13 +521,13 @@ int pack_for(const Parsed &P, int L, Packed &out) {
       b[(size_t)m.o_glen + i] = (unsigned long long)glen[i];
       const int per_word = (L == 1) ? 1 : 2;
       for (int t = 0; t < per_word * glen[i]; t++) {
-        std::vector<int> addr(32, -1);
+        std::vector<int> addr(L >= 16 ? L : 0, -1);
         for (int g = 0; g < L; g++) {
           GEntry e = t < (int)sched[i].size() ? sched[i][t][g] : GEntry{-1, 0};
           if (e.pos < 0) {
             e.coef = 0;
             e.pos = g % 16;
-            if (L == 32 && t < (int)sched[i].size()) {
+            if (L >= 16 && t < (int)sched[i].size()) {
               bool busy[16] = {false};
               for (int l = 0; l < 16; l++) {
                 const GEntry &o = sched[i][t][(g / 16) * 16 + l];
@@ -538,7 +539,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
                 if (!busy[r0]) { e.pos = r0; break; }
             }
           }
-          if (L == 32) addr[g] = e.pos;
+          if (L >= 16) addr[g] = e.pos;
           if (L == 1) { /* double coefficient with the q offset in its 16 lowest mantissa bits */
             b[(size_t)m.o_gat + (size_t)(w0 + t) * L + g] =
                 (dbits((double)e.coef) & ~0xFFFFull) | (unsigned long long)(e.pos * G * 8);
@@ -548,19 +549,19 @@ int pack_for(const Parsed &P, int L, Packed &out) {
             b[(size_t)m.o_gat + (size_t)(w0 + t / 2) * L + g] |= ent << (32 * (t & 1));
           }
         }
-        if (L == 32) out.gather_excess_wavefronts += excess_wavefronts(addr);
+        if (L >= 16) out.gather_excess_wavefronts += excess_wavefronts(addr);
         out.gather_steps++;
       }
       w0 += glen[i];
     }
   }
-  if (L == 32) { /* report: excess wavefronts of the concentration reads per f(y) */
+  if (L >= 16) { /* report: excess wavefronts of the concentration reads per f(y) */
     out.slot_excess_wavefronts = 0;
     for (int r = 0; r < NSR; r++)
       for (int k = 0; k < 6; k++) {
-        std::vector<int> addr(32, -1);
-        for (int g = 0; g < 32; g++) {
-          const Placed &pl = placed[(size_t)r * 32 + g];
+        std::vector<int> addr(L, -1);
+        for (int g = 0; g < L; g++) {
+          const Placed &pl = placed[(size_t)r * L + g];
           addr[g] = k < 3 ? pl.a[k] : pl.b[k - 3];
         }
         out.slot_excess_wavefronts += excess_wavefronts(addr);

@@ -8,7 +8,8 @@
  *
  * Components are renumbered: c = 0 is T, c = 1..K are the species sorted by the length of their gather
  * row (longest first), so that the rows handled in one gather level have similar lengths.
- * Shared-memory region of one system (in doubles, element e of system-in-warp grp at [e*G + grp]):
+ * Shared-memory region of one system (in doubles; thread-per-ODE interleaves the 32 systems of a warp, element
+ * e of lane l at [e*32 + l]; the lane-distributed mappings keep each system's region contiguous):
  *   [0, n)            C_c, concentration of component c; C_0 = 1.0 stands for "no molecule"
  *   [n, n+NTB+1)      [M]_t per third-body efficiency set; the last one = 1.0 stands for "no third body"
  *   [n+NTB+1, +NSR*L) q_s, net rate of progress of reaction slot s
