@@ -192,11 +192,23 @@ class GpuCase:
         self.m.close()
 
 
+def measured_traffic(cfg, N):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the integrate kernel for this workload, from the committed
+    ncu --set full capture (profiles/traffic.json, written from the capture named there), per launch; else None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            for e in json.load(fh).get("captures", []):
+                if e["config"] == cfg and e["N"] == N:
+                    return e["dram_bytes_read"] + e["dram_bytes_write"]
+    return None
+
+
 def roofline(case, ms, work, peak_tflops, peak_src):
     flops = case.m.flops_per_rhs * work["rhs_calls"]
     ach = flops / (ms * 1e-3) / 1e12
     return {"bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s", "frac": ach / peak_tflops,
-            "traffic": None, "peak_source": peak_src, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
+            "traffic": measured_traffic(case.cfg, case.N), "peak_source": peak_src, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
             "flops_per_rhs": case.m.flops_per_rhs, "rhs_calls_per_launch": work["rhs_calls"],
             "kernel_ms": ms, "hbm_algorithmic_GBps": 2 * 8 * (case.mech.n_species + 1) * case.N / (ms * 1e-3) / 1e9}
 
@@ -312,7 +324,7 @@ def run_ours(args):
         others = [c for c in (2, 3, 4) if c != args.config] + ([1] if args.config != 1 else [])
         for c in others:
             s2, N2, dt2 = workload(c)
-            for var in (("auto",) if c != 3 else ("warp", "sub16", "sub8")):
+            for var in (("auto",) if c != 3 else ("warp", "sub16")):
                 try:
                     cs = GpuCase(c, N2, dt2, var)
                     wk = cs.work()
@@ -324,8 +336,17 @@ def run_ours(args):
                     del cs
                 except Exception as ex:  # pragma: no cover
                     extra[f"cfg{c}_{var}"] = {"error": str(ex)}
+        # the paper's "similar neighbours" experiment: the same systems sorted by T
+        try:
+            cs = GpuCase(args.config, N, dt, args.variant, "similar")
+            m2 = cs.timed_steps(3, 3)
+            extra["headline_similar_ordering"] = {"odes_per_s": N / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)),
+                                                  "divergence_D_mean": cs.work().get("divergence_D_mean")}
+            cs.close()
+        except Exception as ex:  # pragma: no cover
+            extra["headline_similar_ordering"] = {"error": str(ex)}
         out["configs"] = extra
-    if args.sweep and rank == 0 and world == 1:
+    if (args.sweep or not args.no_extra) and rank == 0 and world == 1:  # ODEs/s versus N (BASELINE.json metric)
         sw = {}
         for n in spec.N_list:
             cs = GpuCase(args.config, n, dt, args.variant, args.ordering)

@@ -23,9 +23,24 @@ __device__ __forceinline__ int order_bin(double T) {
   return (int)x;
 }
 
-__global__ void order_hist_kernel(const double *__restrict__ T, long long N, unsigned *__restrict__ bins) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < N) atomicAdd(&bins[order_bin(T[i])], 1u);
+#define CKB_ORDER_THREADS 512
+#define CKB_ORDER_ITEMS 8 /* systems per thread */
+
+/* block-private histogram in shared memory, then one global atomic per non-empty bin and block */
+__global__ void __launch_bounds__(CKB_ORDER_THREADS)
+order_hist_kernel(const double *__restrict__ T, long long N, unsigned *__restrict__ bins) {
+  __shared__ unsigned s[CKB_ORDER_BINS];
+  for (int b = threadIdx.x; b < CKB_ORDER_BINS; b += CKB_ORDER_THREADS) s[b] = 0u;
+  __syncthreads();
+  const long long base = (long long)blockIdx.x * (CKB_ORDER_THREADS * CKB_ORDER_ITEMS);
+#pragma unroll
+  for (int k = 0; k < CKB_ORDER_ITEMS; k++) {
+    const long long i = base + k * CKB_ORDER_THREADS + threadIdx.x;
+    if (i < N) atomicAdd(&s[order_bin(T[i])], 1u);
+  }
+  __syncthreads();
+  for (int b = threadIdx.x; b < CKB_ORDER_BINS; b += CKB_ORDER_THREADS)
+    if (s[b]) atomicAdd(&bins[b], s[b]);
 }
 
 /* exclusive scan of the bin counts (one block of CKB_ORDER_BINS / 2 threads, two bins per thread) */
@@ -48,10 +63,32 @@ __global__ void order_scan_kernel(unsigned *__restrict__ bins) {
   bins[2 * t + 1] = s[2 * t];
 }
 
-__global__ void order_scatter_kernel(const double *__restrict__ T, long long N, unsigned *__restrict__ bins,
-                                     int *__restrict__ order) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < N) order[atomicAdd(&bins[order_bin(T[i])], 1u)] = (int)i;
+/* rank inside the block by shared atomics, one global atomic per non-empty bin and block for the block's base */
+__global__ void __launch_bounds__(CKB_ORDER_THREADS)
+order_scatter_kernel(const double *__restrict__ T, long long N, unsigned *__restrict__ bins,
+                     int *__restrict__ order) {
+  __shared__ unsigned s[CKB_ORDER_BINS];
+  for (int b = threadIdx.x; b < CKB_ORDER_BINS; b += CKB_ORDER_THREADS) s[b] = 0u;
+  __syncthreads();
+  const long long base = (long long)blockIdx.x * (CKB_ORDER_THREADS * CKB_ORDER_ITEMS);
+  int bin[CKB_ORDER_ITEMS];
+  unsigned rank[CKB_ORDER_ITEMS];
+#pragma unroll
+  for (int k = 0; k < CKB_ORDER_ITEMS; k++) {
+    const long long i = base + k * CKB_ORDER_THREADS + threadIdx.x;
+    bin[k] = -1;
+    if (i < N) {
+      bin[k] = order_bin(T[i]);
+      rank[k] = atomicAdd(&s[bin[k]], 1u);
+    }
+  }
+  __syncthreads();
+  for (int b = threadIdx.x; b < CKB_ORDER_BINS; b += CKB_ORDER_THREADS)
+    if (s[b]) s[b] = atomicAdd(&bins[b], s[b]); /* count -> this block's first position in the bin */
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < CKB_ORDER_ITEMS; k++)
+    if (bin[k] >= 0) order[s[bin[k]] + rank[k]] = (int)(base + k * CKB_ORDER_THREADS + threadIdx.x);
 }
 
 }  // namespace ckb
@@ -72,10 +109,11 @@ int make_queue_order(const ckb_mech *m, const double *T, long long N, cudaStream
   }
   if (!m->d_bins) CK(cudaMalloc((void **)&m->d_bins, CKB_ORDER_BINS * sizeof(unsigned)));
   CK(cudaMemsetAsync(m->d_bins, 0, CKB_ORDER_BINS * sizeof(unsigned), s));
-  const unsigned blocks = (unsigned)((N + 255) / 256);
-  ckb::order_hist_kernel<<<blocks, 256, 0, s>>>(T, N, m->d_bins);
+  const long long per_block = CKB_ORDER_THREADS * CKB_ORDER_ITEMS;
+  const unsigned blocks = (unsigned)((N + per_block - 1) / per_block);
+  ckb::order_hist_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(T, N, m->d_bins);
   ckb::order_scan_kernel<<<1, CKB_ORDER_BINS / 2, 0, s>>>(m->d_bins);
-  ckb::order_scatter_kernel<<<blocks, 256, 0, s>>>(T, N, m->d_bins, m->d_order);
+  ckb::order_scatter_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(T, N, m->d_bins, m->d_order);
   CK(cudaGetLastError());
   *order = m->d_order;
   return CKB_OK;
