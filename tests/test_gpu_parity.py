@@ -251,3 +251,65 @@ def test_linear_invariants_on_gpu():
         Z = lambda s: (mech.elem_counts * aw).T @ (s[1:] / mech.mol_weight[:, None])
         assert np.abs(y[1:].sum(0) - 1.0).max() < 1e-12
         assert np.abs(Z(y) - Z(states)).max() < 1e-12
+
+
+def test_degenerate_mechanisms():
+    """K = 1 (nothing can react), R = 0, an irreversible reaction without reverse, nu = 3, a species on both sides:
+    every mapping against the oracle."""
+    cases = {
+        "one_species": synth.toy_mechanism(1, []),
+        "no_reactions": synth.toy_mechanism(3, []),
+        "irreversible_nu3": synth.toy_mechanism(3, [({0: 3}, {1: 1, 2: 2}, 3e13, 0.5, 2000.0),
+                                                    ({1: 1}, {0: 1}, 4e5, 0.0, 500.0)], W=[10.0, 12.0, 9.0]),
+        "both_sides_tb": synth.toy_mechanism(3, [({0: 1, 1: 1}, {1: 2}, 2e11, 0.0, 1000.0),
+                                                 ({0: 1}, {2: 1}, 1e11, 0.0, 0.0)], W=[10.0, 10.0, 10.0],
+                                             third_body={1: {0: 2.5, 2: 0.5}}),
+    }
+    rng = np.random.default_rng(3)
+    for name, mech in cases.items():
+        K = mech.n_species
+        N = 70
+        states = np.empty((K + 1, N))
+        states[0] = rng.uniform(900, 2000, N)
+        states[1:] = rng.dirichlet(np.ones(K), size=N).T
+        for method in ("rkck", "rkc"):
+            ora = _oracle(mech, states, synth.P_ATM, 1e-6, method)
+            for variant in ("thread", "warp", "sub8", "sub16"):
+                rep = _compare(_run_gpu(mech, states, synth.P_ATM, 1e-6, method, variant=variant), ora)
+                assert rep["flipped"] <= 1, (name, method, variant, rep)
+
+
+def test_failure_status_parity():
+    """A mechanism that blows up (huge rate, huge heat release): the per-system status codes and the kept states
+    agree with the oracle's (R6/R7), and well-behaved systems in the same batch are unaffected."""
+    nasa = np.zeros((2, 7))
+    nasa[:, 0] = 3.5
+    nasa[0, 5], nasa[1, 5] = 2.0e6, -2.0e6          # enormous heat of reaction
+    mech = synth.toy_mechanism(2, [({0: 2}, {1: 2}, 1e30, 4.0, 0.0)], nasa=nasa)
+    N = 64
+    states = np.empty((3, N))
+    states[0] = np.linspace(1000, 3000, N)
+    states[1] = np.linspace(0.0, 1.0, N)            # system 0 has no reactant: stays put
+    states[2] = 1.0 - states[1]
+    for method in ("rkck", "rkc"):
+        yo, so, to = _oracle(mech, states, synth.P_ATM, 1e-3, method)
+        for variant in ("thread", "warp"):
+            yg, sg, tg = _run_gpu_raw(mech, states, synth.P_ATM, 1e-3, method, variant)
+            assert np.array_equal(sg == 0, so == 0), (method, variant, sg, so)
+            ok = (so == 0) & (tg == to).all(axis=0)
+            assert ok[0] and np.allclose(yg[:, ok], yo[:, ok], rtol=1e-8, atol=1e-14)
+            assert np.isin(sg, (0, 1, 2, 3, 4)).all()
+
+
+def _run_gpu_raw(mech, states, p, dt, method, variant):
+    import torch
+    from paper_1309_2710_b200 import binding
+    m = binding.mech_load(mech)
+    N = states.shape[1]
+    buf = torch.from_numpy(states).cuda()
+    status = torch.full((N,), -7, dtype=torch.int32, device="cuda")
+    stats = torch.full((4, N), -7, dtype=torch.int32, device="cuda")
+    binding.integrate(m, buf, dt, RTOL, ATOL, method, p=p, variant=variant, status=status, stats=stats)
+    torch.cuda.synchronize()
+    m.close()
+    return buf.cpu().numpy(), status.cpu().numpy(), stats.cpu().numpy()
