@@ -128,8 +128,13 @@ void ckb_mech_free(ckb_mech *m) {
   for (int i = 0; i < 4; i++)
     if (m->pk[i].d_blob) cudaFree(m->pk[i].d_blob);
   if (m->d_counters) cudaFree(m->d_counters);
-  if (m->d_order) cudaFree(m->d_order);
-  if (m->d_bins) cudaFree(m->d_bins);
+  for (int i = 0; i < CKB_SCRATCH_SLOTS; i++) {
+    if (m->osc[i].d_order) cudaFree(m->osc[i].d_order);
+    if (m->osc[i].d_bins) cudaFree(m->osc[i].d_bins);
+    if (m->hstream[i]) cudaStreamDestroy(m->hstream[i]);
+  }
+  for (int i = 0; i <= CKB_SCRATCH_SLOTS; i++)
+    if (m->hevent[i]) cudaEventDestroy(m->hevent[i]);
   if (m->ws_states) cudaFree(m->ws_states);
   if (m->ws_pressure) cudaFree(m->ws_pressure);
   if (m->ws_status) cudaFree(m->ws_status);
@@ -147,25 +152,35 @@ int ckb_mech_info(const ckb_mech *m, int32_t *n_species, int32_t *n_reactions, i
   return CKB_OK;
 }
 
-int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
-                  int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
-                  int32_t *status, int32_t *stats, void *stream) {
+/* slot: which queue-order scratch to use; n_choice: batch size the AUTO mapping is chosen for (the whole batch
+ * when ckb_integrate_host feeds it in chunks) */
+static int integrate_impl(const ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                          int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                          int32_t variant, int32_t *status, int32_t *stats, cudaStream_t stream, int slot,
+                          int64_t n_choice) {
   if (!m || N < 0 || (method != CKB_METHOD_RKCK && method != CKB_METHOD_RKC)) return CKB_EINVAL;
   if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(t) || !(rtol > 0.0) || !(atol >= 0.0)) return CKB_EINVAL;
   if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
   Launch l;
-  int rc = choose(m, variant, (long long)N, &l);
+  int rc = choose(m, variant, (long long)n_choice, &l);
   if (rc) return rc;
   if (N == 0) return CKB_OK;
   if (!states || ld < N) return CKB_EINVAL;
   ckb_host::IntegrateArgs a{states, pressure, p_uniform, (long long)N, (long long)ld, t, dt, rtol, atol,
-                  status, stats, (cudaStream_t)stream, nullptr};
+                            status, stats, stream, nullptr};
   /* queue order: hottest systems first (row 0 of states = T); pointless when every system starts at once */
   if (N >= 4096) {
-    rc = ckb_host::make_queue_order(m, states, N, a.stream, &a.order);
+    rc = ckb_host::make_queue_order(m, slot, states, N, a.stream, &a.order);
     if (rc) return rc;
   }
   return dispatch_integrate(m, l, method, a);
+}
+
+int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                  int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
+                  int32_t *status, int32_t *stats, void *stream) {
+  return integrate_impl(m, states, pressure, p_uniform, N, ld, t, dt, rtol, atol, method, variant, status, stats,
+                        (cudaStream_t)stream, 0, N);
 }
 
 int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, double p_uniform, int64_t N,
@@ -207,17 +222,36 @@ int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, doub
     CK(cudaMalloc((void **)&m->ws_stats, (size_t)N * 4 * sizeof(int32_t)));
     m->ws_n_cap = (size_t)N;
   }
-  /* host rows have stride ld, the device copy is dense (stride N) */
-  CK(cudaMemcpy2DAsync(m->ws_states, (size_t)N * 8, states, (size_t)ld * 8, (size_t)N * 8, (size_t)n,
-                       cudaMemcpyHostToDevice, s));
-  if (pressure) CK(cudaMemcpyAsync(m->ws_pressure, pressure, (size_t)N * 8, cudaMemcpyHostToDevice, s));
-  int rc = ckb_integrate(m, m->ws_states, pressure ? m->ws_pressure : nullptr, p_uniform, N, N, t, dt, rtol, atol,
-                         method, variant, status ? m->ws_status : nullptr, stats ? m->ws_stats : nullptr, stream);
-  if (rc) return rc;
-  CK(cudaMemcpy2DAsync(states, (size_t)ld * 8, m->ws_states, (size_t)N * 8, (size_t)N * 8, (size_t)n,
-                       cudaMemcpyDeviceToHost, s));
-  if (status) CK(cudaMemcpyAsync(status, m->ws_status, (size_t)N * 4, cudaMemcpyDeviceToHost, s));
-  if (stats) CK(cudaMemcpyAsync(stats, m->ws_stats, (size_t)N * 16, cudaMemcpyDeviceToHost, s));
+  /* Large batches go through in chunks on internal streams, so that the upload of chunk c+1 and the download of
+   * chunk c-1 overlap the kernel of chunk c (PCIe is full duplex).  The device copy is dense (row stride N). */
+  const int chunks = (N >= 65536) ? CKB_SCRATCH_SLOTS : 1;
+  if (chunks > 1 && !m->hstream[0]) {
+    for (int i = 0; i < CKB_SCRATCH_SLOTS; i++) CK(cudaStreamCreateWithFlags(&m->hstream[i], cudaStreamNonBlocking));
+    for (int i = 0; i <= CKB_SCRATCH_SLOTS; i++) CK(cudaEventCreateWithFlags(&m->hevent[i], cudaEventDisableTiming));
+  }
+  if (chunks > 1) CK(cudaEventRecord(m->hevent[CKB_SCRATCH_SLOTS], s)); /* order after the caller's stream */
+  for (int c = 0; c < chunks; c++) {
+    const int64_t c0 = N * c / chunks, c1 = N * (c + 1) / chunks, nc = c1 - c0;
+    cudaStream_t cs = chunks > 1 ? m->hstream[c] : s;
+    if (chunks > 1) CK(cudaStreamWaitEvent(cs, m->hevent[CKB_SCRATCH_SLOTS], 0));
+    CK(cudaMemcpy2DAsync(m->ws_states + c0, (size_t)N * 8, states + c0, (size_t)ld * 8, (size_t)nc * 8, (size_t)n,
+                         cudaMemcpyHostToDevice, cs));
+    if (pressure) CK(cudaMemcpyAsync(m->ws_pressure + c0, pressure + c0, (size_t)nc * 8, cudaMemcpyHostToDevice, cs));
+    int rc = integrate_impl(m, m->ws_states + c0, pressure ? m->ws_pressure + c0 : nullptr, p_uniform, nc, N, t, dt,
+                            rtol, atol, method, variant, status ? m->ws_status + c0 : nullptr,
+                            stats ? m->ws_stats + 4 * c0 : nullptr, cs, c, N);
+    if (rc) return rc;
+    CK(cudaMemcpy2DAsync(states + c0, (size_t)ld * 8, m->ws_states + c0, (size_t)N * 8, (size_t)nc * 8, (size_t)n,
+                         cudaMemcpyDeviceToHost, cs));
+    if (status) CK(cudaMemcpyAsync(status + c0, m->ws_status + c0, (size_t)nc * 4, cudaMemcpyDeviceToHost, cs));
+    if (stats) /* device block [4][nc] -> host rows of stride N */
+      CK(cudaMemcpy2DAsync(stats + c0, (size_t)N * 4, m->ws_stats + 4 * c0, (size_t)nc * 4, (size_t)nc * 4, 4,
+                           cudaMemcpyDeviceToHost, cs));
+    if (chunks > 1) {
+      CK(cudaEventRecord(m->hevent[c], cs));
+      CK(cudaStreamWaitEvent(s, m->hevent[c], 0));
+    }
+  }
   CK(cudaStreamSynchronize(s));
   return CKB_OK;
 }

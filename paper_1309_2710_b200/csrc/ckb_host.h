@@ -41,6 +41,8 @@ int load_packings(const ckb_mech_desc *d, ckb_mech *m);
 inline int pack_index(int L) { return L == 1 ? 0 : L == 8 ? 1 : L == 16 ? 2 : 3; }
 }  // namespace ckb_host
 
+#define CKB_SCRATCH_SLOTS 4
+
 struct ckb_mech {
   ckb_host::Packed pk[4]; /* L = 1, 8, 16, 32 */
   int K = 0, R = 0, NS = 0;
@@ -53,9 +55,10 @@ struct ckb_mech {
   unsigned long long *d_counters = nullptr;
   mutable std::atomic<unsigned> next_counter{0};
   /* queue order scratch (ckb_order.cu), grow-only; calls on one handle must be stream-ordered */
-  mutable int *d_order = nullptr;
-  mutable unsigned *d_bins = nullptr;
-  mutable size_t order_cap = 0;
+  struct OrderScratch { int *d_order = nullptr; unsigned *d_bins = nullptr; size_t cap = 0; };
+  mutable OrderScratch osc[CKB_SCRATCH_SLOTS]; /* slot 0: ckb_integrate; slots 0..: the chunks of ckb_integrate_host */
+  cudaStream_t hstream[CKB_SCRATCH_SLOTS] = {};  /* internal streams of the pipelined host entry */
+  cudaEvent_t hevent[CKB_SCRATCH_SLOTS + 1] = {};
 };
 
 
@@ -69,7 +72,7 @@ struct IntegrateArgs {
   const int *order; /* queue order (device) or NULL */
 };
 
-int make_queue_order(const ckb_mech *m, const double *T, long long N, cudaStream_t s, const int **order);
+int make_queue_order(const ckb_mech *m, int slot, const double *T, long long N, cudaStream_t s, const int **order);
 struct RhsArgs {
   const double *states; const double *pressure; double p_uniform; long long N, ld; double *dydt; int repeat;
   cudaStream_t stream;

@@ -97,25 +97,26 @@ namespace ckb_host {
 
 /* fills m's scratch with the queue order of the N systems whose temperatures are T[0..N); returns the device
  * pointer in *order (NULL: keep index order) */
-int make_queue_order(const ckb_mech *m, const double *T, long long N, cudaStream_t s, const int **order) {
+int make_queue_order(const ckb_mech *m, int slot, const double *T, long long N, cudaStream_t s, const int **order) {
+  ckb_mech::OrderScratch &sc = m->osc[slot];
   *order = nullptr;
   if (N > 2147483647LL) return CKB_OK;
-  if ((size_t)N > m->order_cap) {
-    if (m->d_order) cudaFree(m->d_order);
-    m->d_order = nullptr;
-    m->order_cap = 0;
-    CK(cudaMalloc((void **)&m->d_order, (size_t)N * sizeof(int)));
-    m->order_cap = (size_t)N;
+  if ((size_t)N > sc.cap) {
+    if (sc.d_order) cudaFree(sc.d_order);
+    sc.d_order = nullptr;
+    sc.cap = 0;
+    CK(cudaMalloc((void **)&sc.d_order, (size_t)N * sizeof(int)));
+    sc.cap = (size_t)N;
   }
-  if (!m->d_bins) CK(cudaMalloc((void **)&m->d_bins, CKB_ORDER_BINS * sizeof(unsigned)));
-  CK(cudaMemsetAsync(m->d_bins, 0, CKB_ORDER_BINS * sizeof(unsigned), s));
+  if (!sc.d_bins) CK(cudaMalloc((void **)&sc.d_bins, CKB_ORDER_BINS * sizeof(unsigned)));
+  CK(cudaMemsetAsync(sc.d_bins, 0, CKB_ORDER_BINS * sizeof(unsigned), s));
   const long long per_block = CKB_ORDER_THREADS * CKB_ORDER_ITEMS;
   const unsigned blocks = (unsigned)((N + per_block - 1) / per_block);
-  ckb::order_hist_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(T, N, m->d_bins);
-  ckb::order_scan_kernel<<<1, CKB_ORDER_BINS / 2, 0, s>>>(m->d_bins);
-  ckb::order_scatter_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(T, N, m->d_bins, m->d_order);
+  ckb::order_hist_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(T, N, sc.d_bins);
+  ckb::order_scan_kernel<<<1, CKB_ORDER_BINS / 2, 0, s>>>(sc.d_bins);
+  ckb::order_scatter_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(T, N, sc.d_bins, sc.d_order);
   CK(cudaGetLastError());
-  *order = m->d_order;
+  *order = sc.d_order;
   return CKB_OK;
 }
 

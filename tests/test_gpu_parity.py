@@ -241,6 +241,29 @@ def test_host_entry_matches_device_entry():
     assert np.array_equal(host, dev) and np.array_equal(status, sd) and np.array_equal(stats, td)
 
 
+def test_host_entry_pipelined_chunks():
+    """N >= 65536: ckb_integrate_host feeds the batch in chunks on internal streams; results, status and stats are
+    those of the device entry (a system's result does not depend on the chunk or queue position), with a ragged ld."""
+    import torch
+    from paper_1309_2710_b200 import binding
+    mech = synth.make_mechanism(1)
+    N, ld = 70001, 70013
+    states, p = synth.make_states(1, N)
+    dev, sd, td = _run_gpu(mech, states, p, 1e-6, "rkck", variant="thread")
+    m = binding.mech_load(mech)
+    host = torch.full((10, ld), float("nan"), dtype=torch.float64).pin_memory()
+    host[:, :N] = torch.from_numpy(states)
+    status = np.full(N, -1, dtype=np.int32)
+    stats = np.full((4, N), -1, dtype=np.int32)
+    rc = binding.lib().ckb_integrate_host(m._h, host.data_ptr(), None, float(p), N, ld, 0.0, 1e-6, RTOL, ATOL, 0, 1,
+                                          status.ctypes.data, stats.ctypes.data, None)
+    assert rc == 0
+    m.close()
+    out = host.numpy()
+    assert np.isnan(out[:, N:]).all()
+    assert np.array_equal(out[:, :N], dev) and np.array_equal(status, sd) and np.array_equal(stats, td)
+
+
 def test_linear_invariants_on_gpu():
     """Sum Y and element mass fractions are conserved by the CUDA path (Runge-Kutta methods keep linear invariants)."""
     for cfg, method in ((1, "rkck"), (3, "rkc")):
