@@ -92,7 +92,7 @@ class ClockSampler:
                         self.reasons.add(k)
             except Exception:  # pragma: no cover
                 pass
-            time.sleep(0.002)
+            time.sleep(0.0005)
 
     def __enter__(self):
         if self.nv:
