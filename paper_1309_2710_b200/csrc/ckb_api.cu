@@ -77,6 +77,14 @@ int dispatch_integrate(const ckb_mech *m, const Launch &l, int method, const ckb
   return CKB_EUNSUPPORTED;
 }
 
+int dispatch_proxy(const ckb_mech *m, const Launch &l, const ckb_host::ProxyArgs &a) {
+#define X(L_, NV_) \
+  if (l.L == L_ && l.NV == NV_) return ckb_host::proxy_L##L_##_NV##NV_(m, a);
+  CKB_FOR_THREAD(X)
+#undef X
+  return CKB_EUNSUPPORTED;
+}
+
 int dispatch_rhs(const ckb_mech *m, const Launch &l, const ckb_host::RhsArgs &a) {
 #define X(L_, NV_) \
   if (l.L == L_ && l.NV == NV_) return ckb_host::rhs_L##L_##_NV##NV_(m, a);
@@ -131,6 +139,7 @@ void ckb_mech_free(ckb_mech *m) {
   for (int i = 0; i < CKB_SCRATCH_SLOTS; i++) {
     if (m->osc[i].d_order) cudaFree(m->osc[i].d_order);
     if (m->osc[i].d_bins) cudaFree(m->osc[i].d_bins);
+    if (m->osc[i].d_keys) cudaFree(m->osc[i].d_keys);
     if (m->hstream[i]) cudaStreamDestroy(m->hstream[i]);
   }
   for (int i = 0; i <= CKB_SCRATCH_SLOTS; i++)
@@ -170,7 +179,18 @@ static int integrate_impl(const ckb_mech *m, double *states, const double *press
                             status, stats, stream, nullptr};
   /* queue order: hottest systems first (row 0 of states = T); pointless when every system starts at once */
   if (N >= 4096) {
-    rc = ckb_host::make_queue_order(m, slot, states, N, a.stream, &a.order);
+    if (l.L == 1 && method == CKB_METHOD_RKC) {
+      /* thread-per-ODE RKC: order by the cost proxy || J f / wt || (two evaluations of f per system) */
+      rc = ckb_host::queue_scratch(m, slot, N);
+      if (rc) return rc;
+      ckb_host::ProxyArgs pa{states, pressure, p_uniform, (long long)N, (long long)ld, 1e-3 * dt, rtol, atol,
+                             m->osc[slot].d_keys, stream};
+      rc = dispatch_proxy(m, l, pa);
+      if (rc) return rc;
+      rc = ckb_host::make_queue_order(m, slot, 1, m->osc[slot].d_keys, N, a.stream, &a.order);
+    } else {
+      rc = ckb_host::make_queue_order(m, slot, 0, states, N, a.stream, &a.order);
+    }
     if (rc) return rc;
   }
   return dispatch_integrate(m, l, method, a);

@@ -55,7 +55,7 @@ struct ckb_mech {
   unsigned long long *d_counters = nullptr;
   mutable std::atomic<unsigned> next_counter{0};
   /* queue order scratch (ckb_order.cu), grow-only; calls on one handle must be stream-ordered */
-  struct OrderScratch { int *d_order = nullptr; unsigned *d_bins = nullptr; size_t cap = 0; };
+  struct OrderScratch { int *d_order = nullptr; unsigned *d_bins = nullptr; double *d_keys = nullptr; size_t cap = 0; };
   mutable OrderScratch osc[CKB_SCRATCH_SLOTS]; /* slot 0: ckb_integrate; slots 0..: the chunks of ckb_integrate_host */
   cudaStream_t hstream[CKB_SCRATCH_SLOTS] = {};  /* internal streams of the pipelined host entry */
   cudaEvent_t hevent[CKB_SCRATCH_SLOTS + 1] = {};
@@ -72,7 +72,15 @@ struct IntegrateArgs {
   const int *order; /* queue order (device) or NULL */
 };
 
-int make_queue_order(const ckb_mech *m, int slot, const double *T, long long N, cudaStream_t s, const int **order);
+/* mode 0: keys are temperatures (hottest first); mode 1: keys are cost proxies (largest first, log-spaced bins) */
+int make_queue_order(const ckb_mech *m, int slot, int mode, const double *keys, long long N, cudaStream_t s,
+                     const int **order);
+int queue_scratch(const ckb_mech *m, int slot, long long N);
+
+struct ProxyArgs {
+  const double *states; const double *pressure; double p_uniform; long long N, ld; double h, rtol, atol;
+  double *key; cudaStream_t stream;
+};
 struct RhsArgs {
   const double *states; const double *pressure; double p_uniform; long long N, ld; double *dydt; int repeat;
   cudaStream_t stream;
@@ -95,7 +103,8 @@ inline int pick_nv(int L, int n) {
 
 #define CKB_DECL(L_, NV_)                                                                         \
   int integrate_L##L_##_NV##NV_(const ckb_mech *m, int method, const IntegrateArgs &a);           \
-  int rhs_L##L_##_NV##NV_(const ckb_mech *m, const RhsArgs &a);
+  int rhs_L##L_##_NV##NV_(const ckb_mech *m, const RhsArgs &a);                                    \
+  int proxy_L##L_##_NV##NV_(const ckb_mech *m, const ProxyArgs &a);
 CKB_FOR_THREAD(CKB_DECL)
 CKB_FOR_GROUP(CKB_DECL)
 #undef CKB_DECL

@@ -101,4 +101,24 @@ int CKB_CAT(rhs_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const RhsArgs &a) {
   return CKB_OK;
 }
 
+int CKB_CAT(proxy_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const ProxyArgs &a) {
+#if CKB_L == 1
+  auto kern = ckb::cost_proxy_kernel<L, NV, Tab>;
+  const size_t smem = smem_bytes(m, 1, ckb::Sys<L, NV, Tab, 1>::HDOUBLES);
+  int rc = prep(kern, smem);
+  if (rc) return rc;
+  const long long blocks = n_blocks(a.N, 1);
+  if (blocks > 2147483647LL) return CKB_EINVAL;
+  Tab tab;
+  make_tab(m, tab);
+  kern<<<(unsigned)blocks, CKB_BLOCK, smem, a.stream>>>(pack_of(m).dm, tab, a.states, a.pressure, a.p_uniform, a.N,
+                                                       a.ld, a.h, a.rtol, a.atol, a.key);
+  CK(cudaGetLastError());
+  return CKB_OK;
+#else
+  (void)m; (void)a;
+  return CKB_EUNSUPPORTED; /* the proxy order is only used by thread-per-ODE */
+#endif
+}
+
 }  // namespace ckb_host

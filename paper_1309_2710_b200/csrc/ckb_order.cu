@@ -16,19 +16,29 @@ namespace ckb {
 #define CKB_ORDER_TMIN 200.0
 #define CKB_ORDER_TMAX 4296.0 /* 2 K per bin */
 
-__device__ __forceinline__ int order_bin(double T) {
+/* mode 1: cost-proxy keys, 16 bins per binade over [1, 2^128), largest first */
+__device__ __forceinline__ int order_bin_log(double key) {
+  double x = (double)(CKB_ORDER_BINS - 1) - 16.0 * log2(fmax(key, 1.0));
+  if (!(x >= 0.0)) x = 0.0; /* huge, inf and NaN keys go first */
+  if (x > (double)(CKB_ORDER_BINS - 1)) x = (double)(CKB_ORDER_BINS - 1);
+  return (int)x;
+}
+
+__device__ __forceinline__ int order_bin_T(double T) {
   double x = (CKB_ORDER_TMAX - T) * ((double)CKB_ORDER_BINS / (CKB_ORDER_TMAX - CKB_ORDER_TMIN)); /* hot first */
   if (!(x >= 0.0)) x = 0.0; /* also NaN */
   if (x > (double)(CKB_ORDER_BINS - 1)) x = (double)(CKB_ORDER_BINS - 1);
   return (int)x;
 }
 
+__device__ __forceinline__ int order_bin(double key, int mode) { return mode ? order_bin_log(key) : order_bin_T(key); }
+
 #define CKB_ORDER_THREADS 512
 #define CKB_ORDER_ITEMS 8 /* systems per thread */
 
 /* block-private histogram in shared memory, then one global atomic per non-empty bin and block */
 __global__ void __launch_bounds__(CKB_ORDER_THREADS)
-order_hist_kernel(const double *__restrict__ T, long long N, unsigned *__restrict__ bins) {
+order_hist_kernel(const double *__restrict__ T, long long N, unsigned *__restrict__ bins, int mode) {
   __shared__ unsigned s[CKB_ORDER_BINS];
   for (int b = threadIdx.x; b < CKB_ORDER_BINS; b += CKB_ORDER_THREADS) s[b] = 0u;
   __syncthreads();
@@ -36,7 +46,7 @@ order_hist_kernel(const double *__restrict__ T, long long N, unsigned *__restric
 #pragma unroll
   for (int k = 0; k < CKB_ORDER_ITEMS; k++) {
     const long long i = base + k * CKB_ORDER_THREADS + threadIdx.x;
-    if (i < N) atomicAdd(&s[order_bin(T[i])], 1u);
+    if (i < N) atomicAdd(&s[order_bin(T[i], mode)], 1u);
   }
   __syncthreads();
   for (int b = threadIdx.x; b < CKB_ORDER_BINS; b += CKB_ORDER_THREADS)
@@ -66,7 +76,7 @@ __global__ void order_scan_kernel(unsigned *__restrict__ bins) {
 /* rank inside the block by shared atomics, one global atomic per non-empty bin and block for the block's base */
 __global__ void __launch_bounds__(CKB_ORDER_THREADS)
 order_scatter_kernel(const double *__restrict__ T, long long N, unsigned *__restrict__ bins,
-                     int *__restrict__ order) {
+                     int *__restrict__ order, int mode) {
   __shared__ unsigned s[CKB_ORDER_BINS];
   for (int b = threadIdx.x; b < CKB_ORDER_BINS; b += CKB_ORDER_THREADS) s[b] = 0u;
   __syncthreads();
@@ -78,7 +88,7 @@ order_scatter_kernel(const double *__restrict__ T, long long N, unsigned *__rest
     const long long i = base + k * CKB_ORDER_THREADS + threadIdx.x;
     bin[k] = -1;
     if (i < N) {
-      bin[k] = order_bin(T[i]);
+      bin[k] = order_bin(T[i], mode);
       rank[k] = atomicAdd(&s[bin[k]], 1u);
     }
   }
@@ -97,24 +107,35 @@ namespace ckb_host {
 
 /* fills m's scratch with the queue order of the N systems whose temperatures are T[0..N); returns the device
  * pointer in *order (NULL: keep index order) */
-int make_queue_order(const ckb_mech *m, int slot, const double *T, long long N, cudaStream_t s, const int **order) {
+/* grow-only scratch of one slot: order[N], keys[N], bins */
+int queue_scratch(const ckb_mech *m, int slot, long long N) {
   ckb_mech::OrderScratch &sc = m->osc[slot];
-  *order = nullptr;
-  if (N > 2147483647LL) return CKB_OK;
   if ((size_t)N > sc.cap) {
     if (sc.d_order) cudaFree(sc.d_order);
-    sc.d_order = nullptr;
-    sc.cap = 0;
+    if (sc.d_keys) cudaFree(sc.d_keys);
+    sc.d_order = nullptr; sc.d_keys = nullptr; sc.cap = 0;
     CK(cudaMalloc((void **)&sc.d_order, (size_t)N * sizeof(int)));
+    CK(cudaMalloc((void **)&sc.d_keys, (size_t)N * sizeof(double)));
     sc.cap = (size_t)N;
   }
   if (!sc.d_bins) CK(cudaMalloc((void **)&sc.d_bins, CKB_ORDER_BINS * sizeof(unsigned)));
+  return CKB_OK;
+}
+
+/* fills the slot's scratch with the queue order of N systems by their keys; returns the device pointer in *order */
+int make_queue_order(const ckb_mech *m, int slot, int mode, const double *keys, long long N, cudaStream_t s,
+                     const int **order) {
+  ckb_mech::OrderScratch &sc = m->osc[slot];
+  *order = nullptr;
+  if (N > 2147483647LL) return CKB_OK;
+  int rc = queue_scratch(m, slot, N);
+  if (rc) return rc;
   CK(cudaMemsetAsync(sc.d_bins, 0, CKB_ORDER_BINS * sizeof(unsigned), s));
   const long long per_block = CKB_ORDER_THREADS * CKB_ORDER_ITEMS;
   const unsigned blocks = (unsigned)((N + per_block - 1) / per_block);
-  ckb::order_hist_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(T, N, sc.d_bins);
+  ckb::order_hist_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(keys, N, sc.d_bins, mode);
   ckb::order_scan_kernel<<<1, CKB_ORDER_BINS / 2, 0, s>>>(sc.d_bins);
-  ckb::order_scatter_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(T, N, sc.d_bins, sc.d_order);
+  ckb::order_scatter_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(keys, N, sc.d_bins, sc.d_order, mode);
   CK(cudaGetLastError());
   *order = sc.d_order;
   return CKB_OK;
