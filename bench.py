@@ -304,7 +304,7 @@ def run_ours(args):
         "clocks": clk.summary(),
         # our kernels per ckb_integrate call: integrate_kernel, and for N >= 4096 the queue order (hist, scan, scatter;
         # plus the cost-proxy kernel for thread-per-ODE RKC)
-        "gpu_launches": K * (1 + (3 if N >= 4096 else 0) + (1 if (N >= 49152 and spec.method == "rkc" and spec.K + 1 <= 16 and args.variant in ("auto", "thread")) else 0)),
+        "gpu_launches": K * (1 + (3 if N >= 4096 else 0) + (1 if (N >= 65536 and spec.method == "rkc" and spec.K + 1 <= 16 and args.variant in ("auto", "thread")) else 0)),
         "work_per_step": work,
         "roofline": roofline(case, float(np.mean(ms)), work, peak_flops / 1e12,
                              "measured: ckb_fp64_probe DFMA chains on this GPU (MEASURED_PEAKS.json has no FP64 figure)"),

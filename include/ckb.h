@@ -38,7 +38,7 @@ extern "C" {
 #define CKB_METHOD_RKC 1
 
 /* variant: how ODE systems are mapped onto lanes */
-#define CKB_VARIANT_AUTO 0    /* thread-per-ODE for K+1 <= 16 and N >= 49152, else warp-per-ODE       */
+#define CKB_VARIANT_AUTO 0    /* thread-per-ODE for K+1 <= 16 and N >= 40960 (RKC: 65536), else warp   */
 #define CKB_VARIANT_THREAD 1  /* one thread integrates one system (the paper's mapping)        */
 #define CKB_VARIANT_WARP 2    /* one warp integrates one system; species and reactions over lanes     */
 #define CKB_VARIANT_SUB8 3    /* 8 lanes per system (4 systems per warp)                              */

@@ -42,14 +42,16 @@ struct Launch {
 };
 
 /* AUTO: thread-per-ODE needs K+1 <= 16 and enough systems to fill the lanes it keeps resident (148 SMs x 3 x 128):
- * measured on B200, it overtakes warp-per-ODE at N ~ 5e4 (a lone thread takes ~6 us per f(y), a warp ~1 us), so small
+ * measured on B200, it overtakes warp-per-ODE at N ~ 4e4 (RKCK) / 6.5e4 (RKC) (a lone thread takes ~6 us per f(y), a warp ~1 us), so small
  * batches of small mechanisms go warp-per-ODE as well. */
-#define CKB_AUTO_THREAD_MIN_N 49152
+#define CKB_AUTO_THREAD_MIN_N_RKCK 40960
+#define CKB_AUTO_THREAD_MIN_N_RKC 65536
 
-int choose(const ckb_mech *m, int variant, long long N, Launch *out) {
+int choose(const ckb_mech *m, int variant, long long N, int method, Launch *out) {
   const int n = m->K + 1;
   if (variant == CKB_VARIANT_AUTO)
-    variant = (n <= 16 && m->pk[0].rc == CKB_OK && (N >= CKB_AUTO_THREAD_MIN_N || m->pk[3].rc != CKB_OK))
+    variant = (n <= 16 && m->pk[0].rc == CKB_OK && (N >= (method == CKB_METHOD_RKC ? CKB_AUTO_THREAD_MIN_N_RKC : CKB_AUTO_THREAD_MIN_N_RKCK) ||
+                                                          m->pk[3].rc != CKB_OK))
                   ? CKB_VARIANT_THREAD
                   : CKB_VARIANT_WARP;
   int L;
@@ -171,7 +173,7 @@ static int integrate_impl(const ckb_mech *m, double *states, const double *press
   if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(t) || !(rtol > 0.0) || !(atol >= 0.0)) return CKB_EINVAL;
   if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
   Launch l;
-  int rc = choose(m, variant, (long long)n_choice, &l);
+  int rc = choose(m, variant, (long long)n_choice, method, &l);
   if (rc) return rc;
   if (N == 0) return CKB_OK;
   if (!states || ld < N) return CKB_EINVAL;
@@ -208,7 +210,7 @@ int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, dou
   if (!m || N < 0 || repeat < 1) return CKB_EINVAL;
   if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
   Launch l;
-  int rc = choose(m, variant, (long long)N, &l);
+  int rc = choose(m, variant, (long long)N, CKB_METHOD_RKCK, &l);
   if (rc) return rc;
   if (N == 0) return CKB_OK;
   if (!states || !dydt || ld < N) return CKB_EINVAL;
