@@ -43,6 +43,8 @@ extern "C" {
 #define CKB_VARIANT_WARP 2    /* one warp integrates one system; species and reactions over lanes     */
 #define CKB_VARIANT_SUB8 3    /* 8 lanes per system (4 systems per warp)                              */
 #define CKB_VARIANT_SUB16 4   /* 16 lanes per system (2 systems per warp)                             */
+#define CKB_VARIANT_SUB2 5    /* 2 lanes per system (K+1 <= 16)                                        */
+#define CKB_VARIANT_SUB4 6    /* 4 lanes per system (K+1 <= 16)                                        */
 
 /* per-system status codes written to status[] */
 #define CKB_ST_OK 0
@@ -143,7 +145,7 @@ int ckb_fp64_probe(int32_t kind, int64_t iters, double *per_second, void *stream
 
 /*
  * ckb_mech_pack_stats: host-only (no CUDA call).  Validates `d`, packs it for `lanes` lanes per system
- * (1, 8, 16 or 32) and reports the packing: stats[0] fused reaction slots, [1] slot rounds per f(y),
+ * (1, 2, 4, 8, 16 or 32) and reports the packing: stats[0] fused reaction slots, [1] slot rounds per f(y),
  * [2] gather steps per f(y), [3] shared-memory bank-conflict replays left in the gather per f(y) after
  * scheduling (lanes = 32 only, else 0), [4] the same for the concentration reads, [5] table size in
  * 8-byte words, [6] shared-memory doubles per system, [7] register slots per lane (NV).

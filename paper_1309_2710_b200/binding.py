@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libckb.so")
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
 METHODS = {"rkck": 0, "rkc": 1}
-VARIANTS = {"auto": 0, "thread": 1, "warp": 2, "sub8": 3, "sub16": 4}
+VARIANTS = {"auto": 0, "thread": 1, "warp": 2, "sub8": 3, "sub16": 4, "sub2": 5, "sub4": 6}
 ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
 
 # every symbol include/ckb.h declares

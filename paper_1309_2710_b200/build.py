@@ -47,6 +47,8 @@ def min_blocks(L: int, NV: int, method: str = "rkck") -> int:
         if method == "rkc":
             return 2
         return int(os.environ.get("CKB_MINB_L1", "3")) if NV <= 14 else 2
+    if L in (2, 4):  # few lanes per system: small mechanisms, short stage vectors
+        return int(os.environ.get("CKB_MINB_L24", "4")) if NV <= 5 else 3
     doubles = NV * systems_per_group(L, NV)  # register slots per stage vector
     if doubles <= int(os.environ.get("CKB_MINB4_MAXNV", "2")):
         return int(os.environ.get("CKB_MINB_SMALL", "4"))
@@ -78,7 +80,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     os.makedirs(OBJ, exist_ok=True)
     flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("CKB_DEFS", "").split()  # tuning knobs
     stamp = os.path.join(OBJ, "stamp")
-    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", ""))
+    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", "") + os.environ.get("CKB_MINB_L24", ""))
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     jobs = []

@@ -41,25 +41,36 @@ struct Launch {
   bool param_tab;
 };
 
-/* AUTO: thread-per-ODE needs K+1 <= 16 and enough systems to fill the lanes it keeps resident (148 SMs x 3 x 128):
- * measured on B200, it overtakes warp-per-ODE at N ~ 4e4 (RKCK) / 6.5e4 (RKC) (a lone thread takes ~6 us per f(y), a warp ~1 us), so small
- * batches of small mechanisms go warp-per-ODE as well. */
-#define CKB_AUTO_THREAD_MIN_N_RKCK 40960
-#define CKB_AUTO_THREAD_MIN_N_RKC 65536
+/* AUTO, from the variant map measured on B200: mechanisms with K+1 <= 16 go thread-per-ODE once the batch fills
+ * the lanes that mapping keeps resident several times over (148 SMs x 3 x 128; a lone thread takes ~6 us per f(y)),
+ * 4 lanes per system at mid sizes (4x the systems in flight per f(y) latency), and warp-per-ODE (~1 us per f(y)) for small
+ * batches; larger mechanisms always go warp-per-ODE. */
+#define CKB_AUTO_SUB4_MIN_N_RKCK 12288
+#define CKB_AUTO_SUB4_MIN_N_RKC 24576
+#define CKB_AUTO_THREAD_MIN_N 196608
 
 int choose(const ckb_mech *m, int variant, long long N, int method, Launch *out) {
   const int n = m->K + 1;
-  if (variant == CKB_VARIANT_AUTO)
-    variant = (n <= 16 && m->pk[0].rc == CKB_OK && (N >= (method == CKB_METHOD_RKC ? CKB_AUTO_THREAD_MIN_N_RKC : CKB_AUTO_THREAD_MIN_N_RKCK) ||
-                                                          m->pk[3].rc != CKB_OK))
-                  ? CKB_VARIANT_THREAD
-                  : CKB_VARIANT_WARP;
+  if (variant == CKB_VARIANT_AUTO) {
+    const bool thread_ok = n <= 16 && m->pk[ckb_host::pack_index(1)].rc == CKB_OK;
+    const bool sub4_ok = n <= 16 && m->pk[ckb_host::pack_index(4)].rc == CKB_OK;
+    const bool warp_ok = m->pk[ckb_host::pack_index(32)].rc == CKB_OK;
+    const long long sub4_min = method == CKB_METHOD_RKC ? CKB_AUTO_SUB4_MIN_N_RKC : CKB_AUTO_SUB4_MIN_N_RKCK;
+    if (thread_ok && (N >= CKB_AUTO_THREAD_MIN_N || (!warp_ok && !sub4_ok)))
+      variant = CKB_VARIANT_THREAD;
+    else if (sub4_ok && (N >= sub4_min || !warp_ok))
+      variant = CKB_VARIANT_SUB4;
+    else
+      variant = CKB_VARIANT_WARP;
+  }
   int L;
   switch (variant) {
     case CKB_VARIANT_THREAD: L = 1; break;
     case CKB_VARIANT_SUB8: L = 8; break;
     case CKB_VARIANT_SUB16: L = 16; break;
     case CKB_VARIANT_WARP: L = 32; break;
+    case CKB_VARIANT_SUB2: L = 2; break;
+    case CKB_VARIANT_SUB4: L = 4; break;
     default: return CKB_EINVAL;
   }
   const ckb_host::Packed &pk = m->pk[ckb_host::pack_index(L)];
@@ -119,7 +130,7 @@ int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out) {
     return rc;
   }
   cudaError_t e = cudaMalloc((void **)&m->d_counters, CKB_COUNTER_RING * 8);
-  for (int i = 0; i < 4 && e == cudaSuccess; i++) {
+  for (int i = 0; i < CKB_NPACK && e == cudaSuccess; i++) {
     ckb_host::Packed &p = m->pk[i];
     if (p.rc != CKB_OK) continue;
     e = cudaMalloc((void **)&p.d_blob, p.blob.size() * 8 + 8);
@@ -135,7 +146,7 @@ int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out) {
 
 void ckb_mech_free(ckb_mech *m) {
   if (!m) return;
-  for (int i = 0; i < 4; i++)
+  for (int i = 0; i < CKB_NPACK; i++)
     if (m->pk[i].d_blob) cudaFree(m->pk[i].d_blob);
   if (m->d_counters) cudaFree(m->d_counters);
   for (int i = 0; i < CKB_SCRATCH_SLOTS; i++) {
@@ -181,13 +192,15 @@ static int integrate_impl(const ckb_mech *m, double *states, const double *press
                             status, stats, stream, nullptr};
   /* queue order: hottest systems first (row 0 of states = T); pointless when every system starts at once */
   if (N >= 4096) {
-    if (l.L == 1 && method == CKB_METHOD_RKC) {
-      /* thread-per-ODE RKC: order by the cost proxy || J f / wt || (two evaluations of f per system) */
+    if (l.L <= 4 && method == CKB_METHOD_RKC && m->pk[0].rc == CKB_OK) {
+      /* RKC with 8 or more systems per warp: order by the cost proxy || J f / wt || (two evaluations of f per
+       * system, computed by the thread-per-ODE kernel whatever mapping integrates) */
+      const Launch l1{1, m->pk[0].dm.NV, true};
       rc = ckb_host::queue_scratch(m, slot, N);
       if (rc) return rc;
       ckb_host::ProxyArgs pa{states, pressure, p_uniform, (long long)N, (long long)ld, 1e-3 * dt, rtol, atol,
                              m->osc[slot].d_keys, stream};
-      rc = dispatch_proxy(m, l, pa);
+      rc = dispatch_proxy(m, l1, pa);
       if (rc) return rc;
       rc = ckb_host::make_queue_order(m, slot, 1, m->osc[slot].d_keys, N, a.stream, &a.order);
     } else {

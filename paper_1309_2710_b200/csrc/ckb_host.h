@@ -38,13 +38,14 @@ struct Parsed;
 int parse_mechanism(const ckb_mech_desc *d, Parsed &P);
 int pack_for(const Parsed &P, int L, Packed &out);
 int load_packings(const ckb_mech_desc *d, ckb_mech *m);
-inline int pack_index(int L) { return L == 1 ? 0 : L == 8 ? 1 : L == 16 ? 2 : 3; }
+#define CKB_NPACK 6
+inline int pack_index(int L) { return L == 1 ? 0 : L == 8 ? 1 : L == 16 ? 2 : L == 32 ? 3 : L == 2 ? 4 : 5; }
 }  // namespace ckb_host
 
 #define CKB_SCRATCH_SLOTS 4
 
 struct ckb_mech {
-  ckb_host::Packed pk[4]; /* L = 1, 8, 16, 32 */
+  ckb_host::Packed pk[CKB_NPACK]; /* L = 1, 8, 16, 32, 2, 4 (pack_index) */
   int K = 0, R = 0, NS = 0;
   double flops_per_rhs = 0.0;
   /* grow-only device workspace of ckb_integrate_host */
@@ -88,7 +89,7 @@ struct RhsArgs {
 
 /* the instantiation list: (lanes per system L, register slots per lane NV); a system needs K+1 <= L*NV */
 #define CKB_FOR_THREAD(X) X(1, 4) X(1, 10) X(1, 14) X(1, 16)
-#define CKB_FOR_GROUP(X) X(8, 7) X(8, 14) X(16, 4) X(16, 7) X(32, 1) X(32, 2) X(32, 4)
+#define CKB_FOR_GROUP(X) X(2, 5) X(2, 8) X(4, 3) X(4, 4) X(8, 7) X(8, 14) X(16, 4) X(16, 7) X(32, 1) X(32, 2) X(32, 4)
 
 /* smallest instantiated NV that holds n unknowns on L lanes, or -1 */
 inline int pick_nv(int L, int n) {

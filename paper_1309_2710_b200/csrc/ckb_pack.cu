@@ -588,9 +588,9 @@ int load_packings(const ckb_mech_desc *d, ckb_mech *m) {
   m->R = P.R;
   m->NS = (int)P.slots.size();
   m->flops_per_rhs = P.flops_per_rhs;
-  static const int Ls[4] = {1, 8, 16, 32};
+  static const int Ls[CKB_NPACK] = {1, 8, 16, 32, 2, 4};
   bool any = false;
-  for (int i = 0; i < 4; i++) {
+  for (int i = 0; i < CKB_NPACK; i++) {
     Packed &pk = m->pk[i];
     pk.rc = pack_for(P, Ls[i], pk);
     if (pk.rc == CKB_OK && Ls[i] == 1 && pk.dm.words > CKB_PARAM_WORDS) pk.rc = CKB_EUNSUPPORTED;
@@ -603,7 +603,7 @@ int load_packings(const ckb_mech_desc *d, ckb_mech *m) {
 }  // namespace ckb_host
 
 extern "C" int ckb_mech_pack_stats(const ckb_mech_desc *d, int32_t lanes, int32_t *stats8) {
-  if (!d || !stats8 || (lanes != 1 && lanes != 8 && lanes != 16 && lanes != 32)) return CKB_EINVAL;
+  if (!d || !stats8 || (lanes != 1 && lanes != 2 && lanes != 4 && lanes != 8 && lanes != 16 && lanes != 32)) return CKB_EINVAL;
   ckb_host::Parsed P;
   int rc = ckb_host::parse_mechanism(d, P);
   if (rc != CKB_OK) return rc;

@@ -36,7 +36,7 @@ def test_strerror(L):
 def test_instantiation_list_consistent():
     inst = build.instantiations()
     assert (1, 10) in inst and (1, 14) in inst and (32, 2) in inst and (32, 4) in inst
-    assert {l for l, _ in inst} == {1, 8, 16, 32}              # one packing per lanes-per-system value
+    assert {l for l, _ in inst} == {1, 2, 4, 8, 16, 32}             # one packing per lanes-per-system value
 
 
 def _load(mech):
@@ -103,6 +103,13 @@ def test_packing_report(cfg, L):
     for lanes in (8, 16):
         st = binding.pack_stats(mech, lanes)
         assert st["slots"] == warp["slots"] and st["register_slots"] * lanes >= spec.K + 1
+    for lanes in (2, 4):                                      # few lanes per system: small mechanisms only
+        if spec.K + 1 <= 16:
+            st = binding.pack_stats(mech, lanes)
+            assert st["slots"] == warp["slots"] and st["register_slots"] * lanes >= spec.K + 1
+        else:
+            with pytest.raises(binding.CkbError):
+                binding.pack_stats(mech, lanes)
 
 
 def test_unpaired_and_duplicate_reactions_pack(L):

@@ -75,6 +75,11 @@ CASES = [
     (0, 700, 1e-6, "thread"),
     (2, 300, 1e-6, "warp"),
     (2, 300, 1e-6, "sub8"),
+    (0, 700, 1e-6, "sub4"),
+    (0, 300, 1e-6, "sub2"),
+    (1, 900, 1e-6, "sub4"),
+    (2, 500, 1e-6, "sub4"),
+    (2, 300, 1e-6, "sub2"),
     (3, 256, 1e-6, "auto"),
     (3, 130, 1e-6, "sub8"),
     (3, 130, 1e-6, "sub16"),
@@ -98,7 +103,7 @@ def test_parity_configs(cfg, N, dt, variant):
 
 
 @pytest.mark.parametrize("cfg,method,variant", [(0, "rkc", "thread"), (2, "rkck", "thread"), (0, "rkc", "warp"),
-                                                (3, "rkck", "warp")])
+                                                (3, "rkck", "warp"), (0, "rkc", "sub4"), (2, "rkck", "sub2")])
 def test_parity_other_method(cfg, method, variant):
     """Both integrators on the mechanisms they are not the headline of (RKC on the nonstiff one, RKCK on stiff ones)."""
     mech = synth.make_mechanism(cfg)
@@ -120,7 +125,7 @@ def test_source_term_parity():
     import torch
     import oracle
     from paper_1309_2710_b200 import binding
-    for cfg, variants in ((0, ("thread", "warp", "sub8")), (2, ("thread", "sub16")), (3, ("warp", "sub8", "sub16")),
+    for cfg, variants in ((0, ("thread", "warp", "sub8", "sub2", "sub4")), (2, ("thread", "sub16", "sub2", "sub4")), (3, ("warp", "sub8", "sub16")),
                           (4, ("warp", "sub8"))):
         mech = synth.make_mechanism(cfg)
         om = oracle.OracleMech(mech)
@@ -194,6 +199,36 @@ def test_full_size_sampled(cfg, n_sample):
     ora = _oracle(mech, np.ascontiguousarray(states[:, pick]), p, spec.dt[0], spec.method)
     rep = _compare((y[:, pick], st[pick], stt[:, pick]), ora, max_flip_frac=5e-3)
     print(f"full size cfg{cfg} N={N}: {rep}")
+
+
+@pytest.mark.parametrize("cfg,N,n_sample", [(1, 50000, 1500), (2, 40000, 600)])
+def test_mid_size_auto_sampled(cfg, N, n_sample):
+    """Batch sizes at which AUTO maps small mechanisms onto 4 lanes per system (and orders the RKC queue by the
+    cost proxy): sampled systems against the oracle, invariants on all of them."""
+    import torch
+    from paper_1309_2710_b200 import binding
+    spec = synth.CONFIGS[cfg]
+    mech = synth.make_mechanism(cfg)
+    states, p = synth.make_states(cfg, N)
+    m = binding.mech_load(mech)
+    outs = {}
+    for variant in ("auto", "sub4"):
+        dev = torch.from_numpy(states).cuda()
+        stats = torch.zeros((4, N), dtype=torch.int32, device="cuda")
+        status = torch.full((N,), -1, dtype=torch.int32, device="cuda")
+        binding.integrate(m, dev, spec.dt[0], RTOL, ATOL, spec.method, p=p, status=status, stats=stats,
+                          variant=variant)
+        torch.cuda.synchronize()
+        outs[variant] = (dev.cpu().numpy(), status.cpu().numpy(), stats.cpu().numpy())
+    m.close()
+    y, st, stt = outs["auto"]
+    assert all(np.array_equal(a, b) for a, b in zip(outs["auto"], outs["sub4"]))   # AUTO is sub4 at this size
+    assert np.isin(st, (0, 4)).all() and np.isfinite(y).all()
+    assert np.abs(y[1:].sum(0) - 1.0).max() < 1e-11
+    pick = np.random.default_rng(5 + cfg).choice(N, size=n_sample, replace=False)
+    ora = _oracle(mech, np.ascontiguousarray(states[:, pick]), p, spec.dt[0], spec.method)
+    rep = _compare((y[:, pick], st[pick], stt[:, pick]), ora, max_flip_frac=5e-3)
+    print(f"mid size cfg{cfg} N={N}: {rep}")
 
 
 def test_empty_and_single():
@@ -297,7 +332,7 @@ def test_degenerate_mechanisms():
         states[1:] = rng.dirichlet(np.ones(K), size=N).T
         for method in ("rkck", "rkc"):
             ora = _oracle(mech, states, synth.P_ATM, 1e-6, method)
-            for variant in ("thread", "warp", "sub8", "sub16"):
+            for variant in ("thread", "warp", "sub8", "sub16", "sub2", "sub4"):
                 rep = _compare(_run_gpu(mech, states, synth.P_ATM, 1e-6, method, variant=variant), ora)
                 assert rep["flipped"] <= 1, (name, method, variant, rep)
 
@@ -316,7 +351,7 @@ def test_failure_status_parity():
     states[2] = 1.0 - states[1]
     for method in ("rkck", "rkc"):
         yo, so, to = _oracle(mech, states, synth.P_ATM, 1e-3, method)
-        for variant in ("thread", "warp"):
+        for variant in ("thread", "warp", "sub4"):
             yg, sg, tg = _run_gpu_raw(mech, states, synth.P_ATM, 1e-3, method, variant)
             assert np.array_equal(sg == 0, so == 0), (method, variant, sg, so)
             ok = (so == 0) & (tg == to).all(axis=0)
