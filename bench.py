@@ -51,6 +51,8 @@ def parse():
     ap.add_argument("--dt", type=float, default=0.0)
     ap.add_argument("--variant", default="auto")
     ap.add_argument("--ordering", default="shuffled", choices=["shuffled", "similar"])
+    ap.add_argument("--no-specialize", action="store_true",
+                    help="keep the table-driven thread-per-ODE kernels (no runtime-generated mechanism code)")
     ap.add_argument("--no-extra", action="store_true", help="skip the other configs, e2e and cpu_baseline")
     ap.add_argument("--sweep", action="store_true", help="also sweep N over the config's N_list")
     return ap.parse_args()
@@ -114,6 +116,8 @@ class ClockSampler:
 class GpuCase:
     """One (config, N, dt, variant) workload resident on the GPU."""
 
+    specialize = True   # class-wide switch (--no-specialize)
+
     def __init__(self, cfg, N, dt, variant="auto", ordering="shuffled", device=0):
         import torch
         from paper_1309_2710_b200 import binding
@@ -122,6 +126,15 @@ class GpuCase:
         self.cfg, self.N, self.dt, self.variant = cfg, N, dt, variant
         self.mech = synth.make_mechanism(cfg)
         self.m = binding.mech_load(self.mech)
+        # mechanism-specialised thread-per-ODE kernels (ckb_mech_specialize) where the mapping applies; if the
+        # runtime compiler is missing the table-driven kernels stay in place and the bench line says so
+        self.specialized, self.specialize_error = False, None
+        if GpuCase.specialize and self.mech.n_species + 1 <= 16:
+            try:
+                self.m.specialize()
+                self.specialized = True
+            except binding.CkbError as e:
+                self.specialize_error = str(e)[:200]
         st, self.p = synth.make_states(cfg, N, ordering=ordering)
         self.host0 = st
         self.states0 = torch.from_numpy(st).cuda()
@@ -257,6 +270,7 @@ def run_reference(args):
 
 
 def run_ours(args):
+    GpuCase.specialize = not args.no_specialize
     import torch
     import torch.distributed as dist
     rank = int(os.environ.get("RANK", "0"))
@@ -299,12 +313,13 @@ def run_ours(args):
         "config": {"workload": f"BASELINE.json configs[{args.config}]: {spec.name} species/reactions, {spec.method.upper()}, "
                                f"N={N} per GPU, dt={dt:g} s, rtol={RTOL:g}, atol={ATOL:g}",
                    "N_per_gpu": N, "variant": args.variant, "ordering": args.ordering,
+                   "specialised": case.specialized, **({"specialise_error": case.specialize_error} if case.specialize_error else {}),
                    "l2": "flushed between timed steps (256 MiB write, untimed)",
                    "restart": "every step restarts from the same initial states (device copy, untimed)"},
         "clocks": clk.summary(),
         # our kernels per ckb_integrate call: integrate_kernel, and for N >= 4096 the queue order (hist, scan, scatter;
         # plus the cost-proxy kernel for thread-per-ODE RKC)
-        "gpu_launches": K * (1 + (3 if N >= 4096 else 0) + (1 if (N >= 65536 and spec.method == "rkc" and spec.K + 1 <= 16 and args.variant in ("auto", "thread")) else 0)),
+        "gpu_launches": K * (1 + (3 if N >= 4096 else 0) + (1 if (N >= 24576 and spec.method == "rkc" and spec.K + 1 <= 16 and args.variant in ("auto", "thread", "sub4", "sub2")) else 0)),
         "work_per_step": work,
         "roofline": roofline(case, float(np.mean(ms)), work, peak_flops / 1e12,
                              "measured: ckb_fp64_probe DFMA chains on this GPU (MEASURED_PEAKS.json has no FP64 figure)"),

@@ -96,6 +96,27 @@ int ckb_mech_info(const ckb_mech *m, int32_t *n_species, int32_t *n_reactions, i
                   double *flops_per_rhs);
 
 /*
+ * Mechanism-specialised kernels for the thread-per-ODE mapping (K+1 <= 16).  The paper generated its source-term
+ * subroutines from the mechanism with a code generator and ran them one thread per system; these
+ * calls are that generator: f(y) (Eq. 2-6) is written out as straight-line CUDA with every mechanism constant a
+ * literal and C_k, [M], q_s in registers, compiled with the integrators by the CUDA runtime compiler (NVRTC, found
+ * with dlopen; $CKB_NVRTC overrides the path) and cached on disk (<library directory>/build/jit or $CKB_JIT_CACHE).
+ *
+ * ckb_mech_specialize: build (or fetch from the cache) and load the specialised kernels for the current device;
+ *   afterwards CKB_VARIANT_THREAD (and AUTO where it picks thread-per-ODE), ckb_rhs and the cost-proxy queue order
+ *   run them instead of the table-driven kernels.  Synchronous, seconds when not cached.  Results differ from the
+ *   table-driven kernels by summation order only.  CKB_EUNSUPPORTED: K+1 > 16 or NVRTC not found (the handle keeps
+ *   working with the table-driven kernels); CKB_ECUDA: compilation or loading failed, text via ckb_codegen_log().
+ * ckb_mech_precompile: host-only (no CUDA call): generate and compile for `arch` ("sm_100a" if NULL) into the cache.
+ * ckb_mech_codegen: host-only: the generated f(y) body as text.  Copies at most cap-1 characters plus a NUL into
+ *   buf (buf may be NULL when cap is 0) and stores the size needed, NUL included, in *needed.
+ */
+int ckb_mech_specialize(ckb_mech *m);
+int ckb_mech_precompile(const ckb_mech_desc *d, const char *arch);
+int ckb_mech_codegen(const ckb_mech_desc *d, char *buf, int64_t cap, int64_t *needed);
+const char *ckb_codegen_log(void); /* compiler log of the calling thread's last specialize / precompile */
+
+/*
  * ckb_integrate: advance every system i in [0, N) from t to t+dt, in place.
  *   states   DEVICE  SoA, row-major [(K+1)][ld]: row 0 = T (K), rows 1..K = mass fractions Y_k;
  *                    element (c, i) at states[c*ld + i]; ld >= N.  Caller-owned (e.g. a torch tensor).

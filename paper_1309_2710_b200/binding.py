@@ -21,7 +21,8 @@ ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
 
 # every symbol include/ckb.h declares
 EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "ckb_integrate_host",
-           "ckb_rhs", "ckb_fp64_probe", "ckb_mech_pack_stats", "ckb_strerror", "ckb_last_cuda_error")
+           "ckb_rhs", "ckb_fp64_probe", "ckb_mech_pack_stats", "ckb_strerror", "ckb_last_cuda_error",
+           "ckb_mech_specialize", "ckb_mech_precompile", "ckb_mech_codegen", "ckb_codegen_log")
 
 
 class CkbError(RuntimeError):
@@ -77,6 +78,14 @@ def lib():
     L.ckb_fp64_probe.restype = C.c_int
     L.ckb_mech_pack_stats.argtypes = [C.POINTER(_Desc), i32, C.POINTER(i32)]
     L.ckb_mech_pack_stats.restype = C.c_int
+    L.ckb_mech_specialize.argtypes = [vp]
+    L.ckb_mech_specialize.restype = C.c_int
+    L.ckb_mech_precompile.argtypes = [C.POINTER(_Desc), C.c_char_p]
+    L.ckb_mech_precompile.restype = C.c_int
+    L.ckb_mech_codegen.argtypes = [C.POINTER(_Desc), C.c_char_p, i64, C.POINTER(i64)]
+    L.ckb_mech_codegen.restype = C.c_int
+    L.ckb_codegen_log.argtypes = []
+    L.ckb_codegen_log.restype = C.c_char_p
     L.ckb_strerror.argtypes = [C.c_int]
     L.ckb_strerror.restype = C.c_char_p
     L.ckb_last_cuda_error.argtypes = []
@@ -140,6 +149,24 @@ def pack_stats(mech, lanes=32):
     return dict(zip(names, list(out)))
 
 
+def codegen(mech) -> str:
+    """ckb_mech_codegen (host only): the generated straight-line f(y) of the mechanism as CUDA text."""
+    d, _keep = _make_desc(mech)
+    need = C.c_int64()
+    _check(lib().ckb_mech_codegen(C.byref(d), None, 0, C.byref(need)), "ckb_mech_codegen")
+    buf = C.create_string_buffer(need.value)
+    _check(lib().ckb_mech_codegen(C.byref(d), buf, need.value, C.byref(need)), "ckb_mech_codegen")
+    return buf.value.decode()
+
+
+def precompile(mech, arch="sm_100a") -> None:
+    """ckb_mech_precompile (host only): generate + compile the specialised kernels into the on-disk cache."""
+    d, _keep = _make_desc(mech)
+    rc = lib().ckb_mech_precompile(C.byref(d), arch.encode())
+    if rc != OK:
+        raise CkbError(rc, "ckb_mech_precompile: " + lib().ckb_codegen_log().decode()[-2000:])
+
+
 class Mech:
     """ckb_mech handle.  `mech` is any object that carries the arrays of ckb_mech_desc as attributes."""
 
@@ -163,6 +190,14 @@ class Mech:
         _check(lib().ckb_mech_info(self._h, C.byref(ks), C.byref(rs), C.byref(ns), C.byref(fl)), "ckb_mech_info")
         self.K, self.R, self.n_slots, self.flops_per_rhs = ks.value, rs.value, ns.value, fl.value
 
+    def specialize(self):
+        """ckb_mech_specialize: switch thread-per-ODE launches of this handle to mechanism-specialised kernels."""
+        rc = lib().ckb_mech_specialize(self._h)
+        if rc != OK:
+            raise CkbError(rc, "ckb_mech_specialize: " + lib().ckb_codegen_log().decode()[-2000:])
+        self.specialized = True
+        return self
+
     def close(self):
         if getattr(self, "_h", None) and _lib is not None:
             _lib.ckb_mech_free(self._h)
@@ -171,8 +206,9 @@ class Mech:
     __del__ = close
 
 
-def mech_load(mech) -> Mech:
-    return Mech(mech)
+def mech_load(mech, specialize=False) -> Mech:
+    m = Mech(mech)
+    return m.specialize() if specialize else m
 
 
 def integrate(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None, pressure=None,

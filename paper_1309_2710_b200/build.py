@@ -21,7 +21,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libckb.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", *ARCH]
+FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", OBJ, *ARCH]
 
 
 def instantiations():
@@ -68,6 +68,28 @@ def _digest(extra: str) -> str:
     return h.hexdigest()
 
 
+def _embed_sources():
+    """The device headers as string literals (build/ckb_embed.inc): ckb_gen.cu hands them to the runtime compiler."""
+    out = []
+    for var, fn in (("ckb_embed_tables", "ckb_tables.h"), ("ckb_embed_device", "ckb_device.cuh")):
+        txt = open(os.path.join(CSRC, fn)).read()
+        assert ')CKBSRC"' not in txt
+        # string literals are limited to 64 KiB by some compilers: concatenate raw-string chunks cut at line ends
+        chunks, cur = [], ""
+        for line in txt.splitlines(keepends=True):
+            if len(cur) + len(line) > 12000:
+                chunks.append(cur)
+                cur = ""
+            cur += line
+        chunks.append(cur)
+        out.append("static const char %s[] =\n%s;\n" % (var, "\n".join('R"CKBSRC(%s)CKBSRC"' % c for c in chunks)))
+    path = os.path.join(OBJ, "ckb_embed.inc")
+    new = "".join(out)
+    if not os.path.exists(path) or open(path).read() != new:
+        with open(path, "w") as fh:
+            fh.write(new)
+
+
 def _run(cmd, verbose):
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
@@ -80,23 +102,24 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     os.makedirs(OBJ, exist_ok=True)
     flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("CKB_DEFS", "").split()  # tuning knobs
     stamp = os.path.join(OBJ, "stamp")
-    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", "") + os.environ.get("CKB_MINB_L24", ""))
+    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", "") + os.environ.get("CKB_MINB_L24", "") + os.environ.get("CKB_US_L1", ""))
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
+    _embed_sources()
     jobs = []
-    for src in ("ckb_api.cu", "ckb_pack.cu", "ckb_order.cu", "ckb_probe.cu"):
+    for src in ("ckb_api.cu", "ckb_pack.cu", "ckb_order.cu", "ckb_probe.cu", "ckb_gen.cu"):
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
         jobs.append((obj, [NVCC, *flags, "-c", os.path.join(CSRC, src), "-o", obj]))
     for (L, NV) in instantiations():
         obj = os.path.join(OBJ, f"ckb_inst_L{L}_NV{NV}.o")
         jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_MINB={min_blocks(L, NV)}", f"-DCKB_MINB_RKC={min_blocks(L, NV, 'rkc')}",
-                           f"-DCKB_UNROLL_SLOTS={1 if L == 1 else int(os.environ.get('CKB_US', '1'))}",
+                           f"-DCKB_UNROLL_SLOTS={int(os.environ.get('CKB_US_L1', '1')) if L == 1 else int(os.environ.get('CKB_US', '1'))}",
                            f"-DCKB_M={systems_per_group(L, NV)}", "-c",
                            os.path.join(CSRC, "ckb_inst.cu"), "-o", obj]))
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         list(ex.map(lambda j: _run(j[1], verbose or ptxas_v), jobs))
     tmp = LIB + f".tmp{os.getpid()}"
-    _run([NVCC, "-shared", *ARCH, "-o", tmp, *[j[0] for j in jobs]], verbose)
+    _run([NVCC, "-shared", *ARCH, "-o", tmp, *[j[0] for j in jobs], "-ldl"], verbose)
     os.replace(tmp, LIB)
     with open(stamp, "w") as fh:
         fh.write(digest)

@@ -81,7 +81,9 @@ int choose(const ckb_mech *m, int variant, long long N, int method, Launch *out)
   return CKB_OK;
 }
 
+/* thread-per-ODE launches go to the mechanism-specialised kernels once ckb_mech_specialize() has built them */
 int dispatch_integrate(const ckb_mech *m, const Launch &l, int method, const ckb_host::IntegrateArgs &a) {
+  if (l.L == 1 && m->gen.ok) return ckb_host::gen_integrate(m, method, a);
 #define X(L_, NV_) \
   if (l.L == L_ && l.NV == NV_) return ckb_host::integrate_L##L_##_NV##NV_(m, method, a);
   CKB_FOR_THREAD(X)
@@ -91,6 +93,7 @@ int dispatch_integrate(const ckb_mech *m, const Launch &l, int method, const ckb
 }
 
 int dispatch_proxy(const ckb_mech *m, const Launch &l, const ckb_host::ProxyArgs &a) {
+  if (l.L == 1 && m->gen.ok) return ckb_host::gen_proxy(m, a);
 #define X(L_, NV_) \
   if (l.L == L_ && l.NV == NV_) return ckb_host::proxy_L##L_##_NV##NV_(m, a);
   CKB_FOR_THREAD(X)
@@ -99,6 +102,7 @@ int dispatch_proxy(const ckb_mech *m, const Launch &l, const ckb_host::ProxyArgs
 }
 
 int dispatch_rhs(const ckb_mech *m, const Launch &l, const ckb_host::RhsArgs &a) {
+  if (l.L == 1 && m->gen.ok) return ckb_host::gen_rhs(m, a);
 #define X(L_, NV_) \
   if (l.L == L_ && l.NV == NV_) return ckb_host::rhs_L##L_##_NV##NV_(m, a);
   CKB_FOR_THREAD(X)
@@ -148,6 +152,7 @@ void ckb_mech_free(ckb_mech *m) {
   if (!m) return;
   for (int i = 0; i < CKB_NPACK; i++)
     if (m->pk[i].d_blob) cudaFree(m->pk[i].d_blob);
+  ckb_host::gen_unload(m);
   if (m->d_counters) cudaFree(m->d_counters);
   for (int i = 0; i < CKB_SCRATCH_SLOTS; i++) {
     if (m->osc[i].d_order) cudaFree(m->osc[i].d_order);

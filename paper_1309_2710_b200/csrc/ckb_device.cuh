@@ -14,8 +14,10 @@
  * Nothing here is shared with the CPU checker (constants that appear in both are typed twice).
  */
 #pragma once
+#ifndef __CUDACC_RTC__ /* the runtime compiler has the math functions built in and no host headers */
 #include <math.h>
 #include <stdint.h>
+#endif
 
 #include "ckb_tables.h"
 
@@ -92,7 +94,11 @@ struct Sys {
   int qoff;        /* (n + NTB + 1) * GI: start of the q region */
   double *sX;      /* scratch of the integrator behind the region (XVec), same interleave */
   double *sH;      /* thread-per-ODE: h_k/(RT) parked here between the two halves of f(y) instead of in registers */
+#ifdef CKB_GEN_RHS
+  static constexpr int HDOUBLES = 0;
+#else
   static constexpr int HDOUBLES = (L_ == 1) ? NV_ : 0;
+#endif
   unsigned mask;   /* lanes of this group */
   int g;           /* lane within the group */
   int src0;        /* warp lane that holds component 0 (T) */
@@ -129,6 +135,14 @@ struct Sys {
   /* Y(q, i): slot i of the argument of system q (read in place from the integrators' registers) */
   template <class GetY>
   __device__ __forceinline__ void rhs(GetY Y, double (&f)[M][NV]) {
+#ifdef CKB_GEN_RHS
+    /* mechanism-specialised translation unit (ckb_gen.cu): straight-line f(y) generated from the mechanism,
+     * every table value a literal, C_k, [M] and q_s in registers -- no shared region, no table reads */
+    if constexpr (L == 1 && M == 1) {
+#include CKB_GEN_RHS
+      return;
+    }
+#endif
     const int n = m.n;
     double T[M], invT[M], lnT[M], s1[M], s2[M];
     double hrt[M][L == 1 ? 1 : NV], yw[M][L == 1 ? 1 : NV];
@@ -467,7 +481,7 @@ struct Rkck {
       if (sys.valid(i)) {
         const double d0 = fma(rtol, fabs(y[i]) + fabs(k1[i]), atol);
         double e = fabs(dl) / d0;
-        if (!isfinite(yn) || isnan(e)) e = INFINITY;
+        if (!isfinite(yn) || isnan(e)) e = __longlong_as_double(0x7ff0000000000000LL); /* +inf */
         errmax = fmax(errmax, e);
       }
     }
@@ -854,12 +868,18 @@ __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem
   sys.src0 = grp * L;
   sys.mask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (grp * L));
   constexpr int GI = S::GI;
-  sys.RS = (region_doubles(m) + xdoubles) * GI;
+#ifdef CKB_GEN_RHS
+  const int region = 0; /* generated f(y): only the integrator's scratch lives in shared memory */
+#else
+  const int region = region_doubles(m);
+#endif
+  sys.RS = (region + xdoubles) * GI;
   sys.qoff = (m.n + m.NTB + 1) * GI;
   /* per warp: G groups x M systems x (region + scratch); interleaved by lane (GI = 32) or one after the other */
-  sys.sR = smem + (size_t)warp * (region_doubles(m) + xdoubles) * G * M + (GI == 1 ? grp * sys.RS * M : grp);
-  sys.sX = sys.sR + region_doubles(m) * GI;
+  sys.sR = smem + (size_t)warp * (region + xdoubles) * G * M + (GI == 1 ? grp * sys.RS * M : grp);
+  sys.sX = sys.sR + region * GI;
   sys.sH = sys.sX + (xdoubles - S::HDOUBLES) * GI;
+#ifndef CKB_GEN_RHS
   if (sys.g == 0) {
 #pragma unroll
     for (int q = 0; q < M; q++) {
@@ -867,6 +887,7 @@ __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem
       sys.sR[q * sys.RS + (m.n + m.NTB) * GI] = 1.0;     /* "no third body" */
     }
   }
+#endif
   sys.gsync();
 }
 

@@ -7,7 +7,9 @@
 
 #include <atomic>
 #include <cstdint>
+#include <memory>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/ckb.h"
@@ -34,7 +36,24 @@ struct Packed {
    * concentration reads */
   int gather_steps = 0, gather_excess_wavefronts = 0, slot_excess_wavefronts = 0;
 };
-struct Parsed;
+/* the mechanism as parsed from ckb_mech_desc: what the packer and the code generator work from */
+struct Rx {
+  std::vector<int> reac, prod; /* molecule lists (species repeated nu times), sorted */
+  int tbset = -1;
+};
+struct Parsed {
+  int K = 0, R = 0;
+  std::vector<double> W, nasa;                                  /* [K], [K][7] */
+  std::vector<double> A, beta, E;                               /* [R] */
+  std::vector<Rx> rx;                                           /* [R] */
+  std::vector<std::vector<std::pair<int, double>>> sets;        /* third-body sets: (species, alpha) */
+  struct Slot { int f, r; };
+  std::vector<Slot> slots;                                      /* fused forward/reverse pairs */
+  std::vector<std::vector<std::pair<int, int>>> rows;           /* [K] gather rows: (slot, net coefficient) */
+  double flops_per_rhs = 0.0;
+};
+/* components: 0 = T, then species by decreasing gather-row length (ckb_tables.h) */
+void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<int> &comp_of_sp);
 int parse_mechanism(const ckb_mech_desc *d, Parsed &P);
 int pack_for(const Parsed &P, int L, Packed &out);
 int load_packings(const ckb_mech_desc *d, ckb_mech *m);
@@ -44,7 +63,20 @@ inline int pack_index(int L) { return L == 1 ? 0 : L == 8 ? 1 : L == 16 ? 2 : L 
 
 #define CKB_SCRATCH_SLOTS 4
 
+namespace ckb_host {
+/* mechanism-specialised thread-per-ODE kernels (ckb_gen.cu): integrate RKCK, integrate RKC, rhs, cost proxy */
+struct GenKernels {
+  cudaLibrary_t lib = nullptr;
+  cudaKernel_t k[4] = {};
+  int NV = 0, resident[2] = {0, 0};
+  size_t smem[2] = {0, 0};
+  bool ok = false;
+};
+}  // namespace ckb_host
+
 struct ckb_mech {
+  std::shared_ptr<ckb_host::Parsed> parsed; /* kept for ckb_mech_specialize */
+  ckb_host::GenKernels gen;
   ckb_host::Packed pk[CKB_NPACK]; /* L = 1, 8, 16, 32, 2, 4 (pack_index) */
   int K = 0, R = 0, NS = 0;
   double flops_per_rhs = 0.0;
@@ -101,6 +133,15 @@ inline int pick_nv(int L, int n) {
 #undef X
   return best;
 }
+
+/* ckb_gen.cu */
+std::string generate_rhs(const Parsed &P);
+int gen_load(ckb_mech *m, const std::string &arch);
+void gen_unload(ckb_mech *m);
+int gen_integrate(const ckb_mech *m, int method, const IntegrateArgs &a);
+int gen_rhs(const ckb_mech *m, const RhsArgs &a);
+int gen_proxy(const ckb_mech *m, const ProxyArgs &a);
+const char *gen_log();
 
 #define CKB_DECL(L_, NV_)                                                                         \
   int integrate_L##L_##_NV##NV_(const ckb_mech *m, int method, const IntegrateArgs &a);           \

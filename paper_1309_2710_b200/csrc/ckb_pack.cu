@@ -25,24 +25,7 @@ inline unsigned long long dbits(double x) {
   return u;
 }
 
-struct Rx {
-  std::vector<int> reac, prod; /* molecule lists (species repeated nu times), sorted */
-  int tbset = -1;
-};
-
 }  // namespace
-
-struct Parsed {
-  int K = 0, R = 0;
-  std::vector<double> W, nasa;                                  /* [K], [K][7] */
-  std::vector<double> A, beta, E;                               /* [R] */
-  std::vector<Rx> rx;                                           /* [R] */
-  std::vector<std::vector<std::pair<int, double>>> sets;        /* third-body sets: (species, alpha) */
-  struct Slot { int f, r; };
-  std::vector<Slot> slots;                                      /* fused forward/reverse pairs */
-  std::vector<std::vector<std::pair<int, int>>> rows;           /* [K] gather rows: (slot, net coefficient) */
-  double flops_per_rhs = 0.0;
-};
 
 int parse_mechanism(const ckb_mech_desc *d, Parsed &P) {
   const int K = d->n_species, R = d->n_reactions, R3 = d->n_third_body;
@@ -386,6 +369,19 @@ int excess_wavefronts(const std::vector<int> &addr_of_lane /* L entries (L = 16 
 
 }  // namespace
 
+void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<int> &comp_of_sp) {
+  const int K = P.K, n = K + 1;
+  sp_of_comp.assign(n, -1);
+  comp_of_sp.assign(K, 0);
+  std::vector<int> order(K);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return P.rows[a].size() > P.rows[b].size(); });
+  for (int c = 1; c < n; c++) {
+    sp_of_comp[c] = order[c - 1];
+    comp_of_sp[order[c - 1]] = c;
+  }
+}
+
 int pack_for(const Parsed &P, int L, Packed &out) {
   const int K = P.K, n = K + 1;
   const int G = (L == 1) ? 32 : 1; /* shared-memory interleave of the region (Sys::GI) */
@@ -399,17 +395,8 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   const bool optimise = true;
 
   /* components: 0 = T, then species by decreasing gather-row length */
-  std::vector<int> sp_of_comp(n, -1), comp_of_sp(K);
-  {
-    std::vector<int> order(K);
-    std::iota(order.begin(), order.end(), 0);
-    std::stable_sort(order.begin(), order.end(),
-                     [&](int a, int b) { return P.rows[a].size() > P.rows[b].size(); });
-    for (int c = 1; c < n; c++) {
-      sp_of_comp[c] = order[c - 1];
-      comp_of_sp[order[c - 1]] = c;
-    }
-  }
+  std::vector<int> sp_of_comp, comp_of_sp;
+  component_order(P, sp_of_comp, comp_of_sp);
   /* which lane evaluates which slot, and the gather schedule of every level */
   const std::vector<Placed> placed = place_slots(P, comp_of_sp, L, NSR, optimise);
   std::vector<int> pos_of_slot(NS, -1);
@@ -581,7 +568,8 @@ int pack_for(const Parsed &P, int L, Packed &out) {
 /* parse once, pack for every lanes-per-system value; the thread-per-ODE packing must fit the kernel
  * parameter space (CKB_PARAM_WORDS) */
 int load_packings(const ckb_mech_desc *d, ckb_mech *m) {
-  Parsed P;
+  m->parsed = std::make_shared<Parsed>();
+  Parsed &P = *m->parsed;
   int rc = parse_mechanism(d, P);
   if (rc != CKB_OK) return rc;
   m->K = P.K;
