@@ -26,6 +26,12 @@ namespace ckb {
 /* R20: physical constants */
 #define CKB_RU 8.314462618e7 /* erg/(mol K) */
 
+#ifndef CKB_XS_RKCK_K12
+#define CKB_XS_RKCK_K12 0 /* thread-per-ODE RKCK: 1 = k1, k2 live in the shared scratch too */
+#endif
+#ifndef CKB_XS_RKC_F0
+#define CKB_XS_RKC_F0 0 /* thread-per-ODE RKC: 1 = f0 and w_{j-2} live in the shared scratch too */
+#endif
 #ifndef CKB_UNROLL_SLOTS
 #define CKB_UNROLL_SLOTS 1 /* reaction slots in flight per lane: 2 slots = 4 independent exp chains */
 #endif
@@ -369,8 +375,11 @@ struct Rkck {
 
   double w[NV];                 /* the next argument of f */
   static constexpr bool XS = (S::L == 1); /* k3..k5 in shared scratch */
-  static constexpr int XDOUBLES = XS ? 3 * NV : 0;
-  double y[NV], k1[NV], k2[NV];
+  static constexpr bool XS12 = XS && (CKB_XS_RKCK_K12 != 0); /* k1, k2 as well (specialised kernels: 4 blocks per SM) */
+  static constexpr int XDOUBLES = XS ? (XS12 ? 5 : 3) * NV : 0;
+  double y[NV];
+  XVec<S, 3, XS12> k1;
+  XVec<S, 4, XS12> k2;
   XVec<S, 0, XS> k3;
   XVec<S, 1, XS> k4;
   XVec<S, 2, XS> k5;
@@ -379,14 +388,14 @@ struct Rkck {
   bool last, saw_nonfinite;
 
   /* R5 clip, then either evaluate k1 (stage 1) or go on with the stages (k1 kept and rescaled, R25) */
-  __device__ __forceinline__ void begin_attempt(bool have_k1) {
+  __device__ __forceinline__ void begin_attempt(const S &sys, bool have_k1) {
     last = false;
     if (1.1 * h >= t1 - t) {
       const double hn = t1 - t;
       if (have_k1) {
         const double r = hn / h;
 #pragma unroll
-        for (int i = 0; i < NV; i++) k1[i] *= r;
+        for (int i = 0; i < NV; i++) k1.set(sys, i, k1.get(sys, i) * r);
       }
       h = hn;
       last = true;
@@ -396,10 +405,10 @@ struct Rkck {
 #pragma unroll
       for (int i = 0; i < NV; i++) w[i] = y[i];
     } else {
-      start_stages();
+      start_stages(sys);
     }
   }
-  __device__ __forceinline__ void start_stages() {
+  __device__ __forceinline__ void start_stages(const S &sys) {
     if (++attempts > 1000000) { /* R7 */
       status = ST_MAXSTEPS;
       stage = 0;
@@ -407,11 +416,11 @@ struct Rkck {
     }
     stage = 2;
 #pragma unroll
-    for (int i = 0; i < NV; i++) w[i] = fma(B21, k1[i], y[i]);
+    for (int i = 0; i < NV; i++) w[i] = fma(B21, k1.get(sys, i), y[i]);
   }
 
-  __device__ __forceinline__ void start(const double (&y0)[NV], double t0_, double t1_, double rtol_, double atol_,
-                                        int /*n*/) {
+  __device__ __forceinline__ void start(const S &sys, const double (&y0)[NV], double t0_, double t1_, double rtol_,
+                                        double atol_, int /*n*/) {
 #pragma unroll
     for (int i = 0; i < NV; i++) y[i] = y0[i];
     t = t0_; t1 = t1_; rtol = rtol_; atol = atol_;
@@ -419,7 +428,7 @@ struct Rkck {
     nfe = nacc = nrej = attempts = 0;
     status = ST_OK;
     saw_nonfinite = false;
-    begin_attempt(false);
+    begin_attempt(sys, false);
   }
 
   /* consume f = f(w); returns true when the system has reached t1 (or failed) */
@@ -428,14 +437,15 @@ struct Rkck {
     switch (stage) {
       case 1: /* Eq. 7 */
 #pragma unroll
-        for (int i = 0; i < NV; i++) k1[i] = h * f[i];
-        start_stages();
+        for (int i = 0; i < NV; i++) k1.set(sys, i, h * f[i]);
+        start_stages(sys);
         return stage == 0;
       case 2:
 #pragma unroll
         for (int i = 0; i < NV; i++) {
-          k2[i] = h * f[i];
-          w[i] = fma(B32, k2[i], fma(B31, k1[i], y[i]));
+          const double k2i = h * f[i];
+          k2.set(sys, i, k2i);
+          w[i] = fma(B32, k2i, fma(B31, k1.get(sys, i), y[i]));
         }
         stage = 3;
         return false;
@@ -444,7 +454,7 @@ struct Rkck {
         for (int i = 0; i < NV; i++) {
           const double k3i = h * f[i];
           k3.set(sys, i, k3i);
-          w[i] = fma(B43, k3i, fma(B42, k2[i], fma(B41, k1[i], y[i])));
+          w[i] = fma(B43, k3i, fma(B42, k2.get(sys, i), fma(B41, k1.get(sys, i), y[i])));
         }
         stage = 4;
         return false;
@@ -453,7 +463,7 @@ struct Rkck {
         for (int i = 0; i < NV; i++) {
           const double k4i = h * f[i], k3i = k3.get(sys, i);
           k4.set(sys, i, k4i);
-          w[i] = fma(B54, k4i, fma(B53, k3i, fma(B52, k2[i], fma(B51, k1[i], y[i]))));
+          w[i] = fma(B54, k4i, fma(B53, k3i, fma(B52, k2.get(sys, i), fma(B51, k1.get(sys, i), y[i]))));
         }
         stage = 5;
         return false;
@@ -462,7 +472,7 @@ struct Rkck {
         for (int i = 0; i < NV; i++) {
           const double k5i = h * f[i], k3i = k3.get(sys, i), k4i = k4.get(sys, i);
           k5.set(sys, i, k5i);
-          w[i] = fma(B65, k5i, fma(B64, k4i, fma(B63, k3i, fma(B62, k2[i], fma(B61, k1[i], y[i])))));
+          w[i] = fma(B65, k5i, fma(B64, k4i, fma(B63, k3i, fma(B62, k2.get(sys, i), fma(B61, k1.get(sys, i), y[i])))));
         }
         stage = 6;
         return false;
@@ -475,11 +485,12 @@ struct Rkck {
     for (int i = 0; i < NV; i++) {
       const double k6 = h * f[i];
       const double k3i = k3.get(sys, i), k4i = k4.get(sys, i), k5i = k5.get(sys, i);
-      const double yn = fma(C6, k6, fma(C4, k4i, fma(C3, k3i, fma(C1, k1[i], y[i]))));
-      const double dl = fma(D6, k6, fma(D5, k5i, fma(D4, k4i, fma(D3, k3i, D1 * k1[i]))));
+      const double k1i = k1.get(sys, i);
+      const double yn = fma(C6, k6, fma(C4, k4i, fma(C3, k3i, fma(C1, k1i, y[i]))));
+      const double dl = fma(D6, k6, fma(D5, k5i, fma(D4, k4i, fma(D3, k3i, D1 * k1i))));
       w[i] = yn;
       if (sys.valid(i)) {
-        const double d0 = fma(rtol, fabs(y[i]) + fabs(k1[i]), atol);
+        const double d0 = fma(rtol, fabs(y[i]) + fabs(k1i), atol);
         double e = fabs(dl) / d0;
         if (!isfinite(yn) || isnan(e)) e = __longlong_as_double(0x7ff0000000000000LL); /* +inf */
         errmax = fmax(errmax, e);
@@ -495,7 +506,7 @@ struct Rkck {
       double fac = (errmax > 0.0) ? SAFETY * pow(errmax, -0.2) : 5.0;
       if (fac > 5.0) fac = 5.0; /* P:144 */
       h *= fac;
-      begin_attempt(false);
+      begin_attempt(sys, false);
       return false;
     }
     nrej++;
@@ -508,14 +519,14 @@ struct Rkck {
       saw_nonfinite = true;
     }
 #pragma unroll
-    for (int i = 0; i < NV; i++) k1[i] *= fac; /* R25 */
+    for (int i = 0; i < NV; i++) k1.set(sys, i, k1.get(sys, i) * fac); /* R25 */
     h *= fac;
     const double tmax = fmax(fabs(t), fabs(t1));
     if (!(h > 10.0 * CKB_U * tmax)) { /* R6 */
       status = saw_nonfinite ? ST_NONFINITE : ST_UNDERFLOW;
       return true;
     }
-    begin_attempt(true);
+    begin_attempt(sys, true);
     return stage == 0;
   }
 
@@ -560,8 +571,11 @@ struct Rkc {
 
   double w[NV];                                   /* the next argument of f: y, z (power method), w_{j-1} */
   static constexpr bool XS = (S::L == 1); /* eigenvector estimate v in shared scratch */
-  static constexpr int XDOUBLES = XS ? NV : 0;
-  double y[NV], f0[NV], wjm2[NV];
+  static constexpr bool XSF = XS && (CKB_XS_RKC_F0 != 0); /* f0 and w_{j-2} as well (specialised kernels) */
+  static constexpr int XDOUBLES = XS ? (XSF ? 3 : 1) * NV : 0;
+  double y[NV];
+  XVec<S, 1, XSF> f0;
+  XVec<S, 2, XSF> wjm2;
   XVec<S, 0, XS> v;
   double t, h, t1, Dt, rtol, atol, nd;
   double sigma, err_old, h_old;
@@ -570,8 +584,8 @@ struct Rkc {
   int nfe, nacc, nrej, smax_used, attempts, since_sigma, status, flag;
   bool last, have_prev, saw_nonfinite, sigma_fresh, need_sigma, pm_initial;
 
-  __device__ __forceinline__ void start(const double (&y0)[NV], double t0_, double t1_, double rtol_, double atol_,
-                                        int n) {
+  __device__ __forceinline__ void start(const S & /*sys*/, const double (&y0)[NV], double t0_, double t1_, double rtol_,
+                                        double atol_, int n) {
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       y[i] = y0[i];
@@ -592,7 +606,7 @@ struct Rkc {
   __device__ __forceinline__ void pm_begin(const S &sys, bool have_v, bool initial) {
     if (!have_v) {
 #pragma unroll
-      for (int i = 0; i < NV; i++) v.set(sys, i, f0[i]);
+      for (int i = 0; i < NV; i++) v.set(sys, i, f0.get(sys, i));
     }
     double a = 0.0, b = 0.0;
 #pragma unroll
@@ -667,8 +681,8 @@ struct Rkc {
     const double mh = mut1 * h;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      wjm2[i] = y[i];
-      w[i] = fma(mh, f0[i], y[i]); /* Eq. 19 */
+      wjm2.set(sys, i, y[i]);
+      w[i] = fma(mh, f0.get(sys, i), y[i]); /* Eq. 19 */
     }
     j = 2;
     state = S_STAGE;
@@ -680,7 +694,7 @@ struct Rkc {
     switch (state) {
       case S_F0: {
 #pragma unroll
-        for (int i = 0; i < NV; i++) f0[i] = f[i];
+        for (int i = 0; i < NV; i++) f0.set(sys, i, f[i]);
         pm_begin(sys, false, true);
         return false;
       }
@@ -688,7 +702,7 @@ struct Rkc {
         double dd = 0.0;
 #pragma unroll
         for (int i = 0; i < NV; i++) {
-          const double e = f[i] - f0[i];
+          const double e = f[i] - f0.get(sys, i);
           dd = fma(e, e, dd);
         }
         dd = sqrt(sys.gsum(dd));
@@ -700,7 +714,7 @@ struct Rkc {
           if (dd != 0.0) {
             const double r = pm_d / dd;
 #pragma unroll
-            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0[i], r, y[i]);
+            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0.get(sys, i), r, y[i]);
           } else {
             const int ci = pm_it % (int)nd;
 #pragma unroll
@@ -716,7 +730,7 @@ struct Rkc {
           if (dd != 0.0) {
             const double r = pm_d / dd;
 #pragma unroll
-            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0[i], r, y[i]);
+            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0.get(sys, i), r, y[i]);
           } else {
             const int ci = pm_it % (int)nd;
 #pragma unroll
@@ -734,7 +748,7 @@ struct Rkc {
         /* initial step, Eq. 36-37 (R14, R15): probe f(y + h0 f0) */
         h_old = (sigma > 0.0 && 1.0 / sigma < Dt) ? 1.0 / sigma : Dt; /* h0, parked in h_old */
 #pragma unroll
-        for (int i = 0; i < NV; i++) w[i] = fma(h_old, f0[i], y[i]);
+        for (int i = 0; i < NV; i++) w[i] = fma(h_old, f0.get(sys, i), y[i]);
         state = S_H0;
         return false;
       }
@@ -744,7 +758,7 @@ struct Rkc {
 #pragma unroll
         for (int i = 0; i < NV; i++) {
           if (sys.valid(i)) {
-            const double d0 = h0 * (f[i] - f0[i]);
+            const double d0 = h0 * (f[i] - f0.get(sys, i));
             const double wt = fma(rtol, fabs(y[i]), atol);
             const double q = d0 / wt;
             acc = fma(q, q, acc);
@@ -771,8 +785,8 @@ struct Rkc {
         const double c0 = 1.0 - mu - nu, mh = mut * h, gh = gamt * h;
 #pragma unroll
         for (int i = 0; i < NV; i++) {
-          const double wj = fma(gh, f0[i], fma(mh, f[i], fma(nu, wjm2[i], fma(mu, w[i], c0 * y[i]))));
-          wjm2[i] = w[i];
+          const double wj = fma(gh, f0.get(sys, i), fma(mh, f[i], fma(nu, wjm2.get(sys, i), fma(mu, w[i], c0 * y[i]))));
+          wjm2.set(sys, i, w[i]);
           w[i] = wj;
         }
         if (++j > s) state = S_FINAL;
@@ -786,7 +800,7 @@ struct Rkc {
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       if (sys.valid(i)) {
-        const double del = fma(0.8, y[i] - w[i], 0.4 * h * (f0[i] + f[i]));
+        const double del = fma(0.8, y[i] - w[i], 0.4 * h * (f0.get(sys, i) + f[i]));
         const double wt = fma(rtol, fmax(fabs(y[i]), fabs(w[i])), atol);
         const double q = del / wt;
         acc = fma(q, q, acc);
@@ -805,7 +819,7 @@ struct Rkc {
 #pragma unroll
       for (int i = 0; i < NV; i++) {
         y[i] = w[i];
-        f0[i] = f[i];
+        f0.set(sys, i, f[i]);
       }
       err_old = err;
       h_old = h;
@@ -940,7 +954,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
             const int c = sys.g + L * i;
             y0[i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode[q]] : 0.0;
           }
-          integ[q].start(y0, t0, t0 + dt, rtol, atol, m.n);
+          integ[q].start(sys, y0, t0, t0 + dt, rtol, atol, m.n);
           need_load[q] = false;
         }
       }

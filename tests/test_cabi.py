@@ -130,3 +130,41 @@ def test_product_path_does_not_import_oracle():
     for fn in os.listdir(os.path.join(pkg, "csrc")):
         src = open(os.path.join(pkg, "csrc", fn)).read()
         assert not re.search(r"#include[^\n]*oracle|ora_[a-z]+\s*\(|libckoracle", src), fn
+
+
+def test_codegen_text(L):
+    """ckb_mech_codegen (host only): the straight-line f(y) of a mechanism -- one exp per irreversible reaction
+    with A > 0, every species' thermodynamic polynomials, no table reads; too many unknowns are refused."""
+    mech = synth.make_mechanism(1)
+    src = binding.codegen(mech)
+    assert src.count("ckb_exp(") == mech.n_reactions
+    assert src.count("double cp =") == mech.n_species and src.count("double h =") == mech.n_species
+    assert "f[0][0] =" in src and "tab" not in src and "sR" not in src
+    n_sets = len({tuple(sorted((int(mech.tb_species[e]), float(mech.tb_eff[e]))
+                               for e in range(mech.tb_ptr[r], mech.tb_ptr[r + 1])))
+                  for r in range(len(mech.tb_reaction))})
+    assert src.count("= ctot;") == n_sets + 0
+    toy = synth.toy_mechanism(2, [({0: 2}, {1: 1}, 5.0, 0.0, 0.0), ({1: 1}, {0: 2}, 0.0, 0.0, 0.0)])
+    s2 = binding.codegen(toy)
+    assert s2.count("ckb_exp(") == 1 and "fma(-0x1p+1, q, om" in s2      # A = 0: no rate; nu' = 2 on the reactant
+    with pytest.raises(binding.CkbError):
+        binding.codegen(synth.make_mechanism(3))
+
+
+def test_precompile_fills_cache(L, tmp_path, monkeypatch):
+    """ckb_mech_precompile (host only): NVRTC compiles the generated kernels for sm_100a without a GPU and the
+    second call is served from the on-disk cache."""
+    import ctypes.util
+    import time
+    if not (ctypes.util.find_library("nvrtc") or os.path.exists("/usr/local/cuda/lib64/libnvrtc.so.12")):
+        pytest.skip("NVRTC not installed")
+    monkeypatch.setenv("CKB_JIT_CACHE", str(tmp_path / "jit"))
+    mech = synth.make_mechanism(0)
+    t0 = time.time()
+    binding.precompile(mech)
+    t1 = time.time()
+    files = list((tmp_path / "jit").iterdir())
+    assert len(files) == 1 and files[0].stat().st_size > 10000
+    binding.precompile(mech)
+    assert time.time() - t1 < 0.5 * (t1 - t0) + 0.05
+    assert len(list((tmp_path / "jit").iterdir())) == 1

@@ -22,6 +22,9 @@ def _run_gpu(mech, states, p, dt, method, variant="auto", ld=None, pressure=None
     import torch
     from paper_1309_2710_b200 import binding
     m = binding.mech_load(mech)
+    if variant == "gen":                            # thread-per-ODE with mechanism-specialised kernels
+        m.specialize()
+        variant = "thread"
     n, N = states.shape
     ld = N if ld is None else ld
     buf = torch.full((n, ld), float("nan"), dtype=torch.float64, device="cuda")
@@ -60,6 +63,10 @@ def _compare(gpu, ora, max_flip_frac=2e-3):
     return dict(n=N, flipped=n_flip, relT=float(relT[same].max(initial=0.0)), relY=float(relY[same].max(initial=0.0)))
 
 
+def spec_ok(mech):
+    return mech.n_species + 1 <= 16
+
+
 def _oracle(mech, states, p, dt, method, pressure=None):
     import oracle
     om = oracle.OracleMech(mech)
@@ -75,6 +82,9 @@ CASES = [
     (0, 700, 1e-6, "thread"),
     (2, 300, 1e-6, "warp"),
     (2, 300, 1e-6, "sub8"),
+    (0, 1024, 1e-6, "gen"),
+    (1, 1500, 1e-6, "gen"),
+    (2, 1024, 1e-6, "gen"),
     (0, 700, 1e-6, "sub4"),
     (0, 300, 1e-6, "sub2"),
     (1, 900, 1e-6, "sub4"),
@@ -103,7 +113,8 @@ def test_parity_configs(cfg, N, dt, variant):
 
 
 @pytest.mark.parametrize("cfg,method,variant", [(0, "rkc", "thread"), (2, "rkck", "thread"), (0, "rkc", "warp"),
-                                                (3, "rkck", "warp"), (0, "rkc", "sub4"), (2, "rkck", "sub2")])
+                                                (3, "rkck", "warp"), (0, "rkc", "sub4"), (2, "rkck", "sub2"),
+                                                (0, "rkc", "gen"), (2, "rkck", "gen")])
 def test_parity_other_method(cfg, method, variant):
     """Both integrators on the mechanisms they are not the headline of (RKC on the nonstiff one, RKCK on stiff ones)."""
     mech = synth.make_mechanism(cfg)
@@ -133,7 +144,10 @@ def test_source_term_parity():
         ref = np.stack([om.rhs(states[:, i].copy(), p) for i in range(70)], axis=1)
         m = binding.mech_load(mech)
         st = torch.from_numpy(states).cuda()
-        for v in variants:
+        for v in variants + (("gen",) if spec_ok(mech) else ()):
+            if v == "gen":                          # after the table-driven variants: the switch is per handle
+                m.specialize()
+                v = "thread"
             out = binding.rhs(m, st, p=p, variant=v).cpu().numpy()
             scale = np.abs(ref).max(axis=1, keepdims=True)
             assert (np.abs(out - ref) <= 1e-11 * scale + 1e-13 * np.abs(ref)).all(), (cfg, v)
@@ -181,7 +195,7 @@ def test_full_size_sampled(cfg, n_sample):
     N = {1: 1 << 19, 2: 1 << 18, 3: 1 << 17, 4: 1 << 16}[cfg]
     mech = synth.make_mechanism(cfg)
     states, p = synth.make_states(cfg, N)
-    m = binding.mech_load(mech)
+    m = binding.mech_load(mech, specialize=spec_ok(mech))   # as bench.py: specialised kernels where they apply
     dev = torch.from_numpy(states).cuda()
     stats = torch.zeros((4, N), dtype=torch.int32, device="cuda")
     status = torch.full((N,), -1, dtype=torch.int32, device="cuda")
@@ -332,7 +346,7 @@ def test_degenerate_mechanisms():
         states[1:] = rng.dirichlet(np.ones(K), size=N).T
         for method in ("rkck", "rkc"):
             ora = _oracle(mech, states, synth.P_ATM, 1e-6, method)
-            for variant in ("thread", "warp", "sub8", "sub16", "sub2", "sub4"):
+            for variant in ("thread", "warp", "sub8", "sub16", "sub2", "sub4", "gen"):
                 rep = _compare(_run_gpu(mech, states, synth.P_ATM, 1e-6, method, variant=variant), ora)
                 assert rep["flipped"] <= 1, (name, method, variant, rep)
 
@@ -351,7 +365,7 @@ def test_failure_status_parity():
     states[2] = 1.0 - states[1]
     for method in ("rkck", "rkc"):
         yo, so, to = _oracle(mech, states, synth.P_ATM, 1e-3, method)
-        for variant in ("thread", "warp", "sub4"):
+        for variant in ("thread", "warp", "sub4", "gen"):
             yg, sg, tg = _run_gpu_raw(mech, states, synth.P_ATM, 1e-3, method, variant)
             assert np.array_equal(sg == 0, so == 0), (method, variant, sg, so)
             ok = (so == 0) & (tg == to).all(axis=0)
@@ -363,6 +377,9 @@ def _run_gpu_raw(mech, states, p, dt, method, variant):
     import torch
     from paper_1309_2710_b200 import binding
     m = binding.mech_load(mech)
+    if variant == "gen":
+        m.specialize()
+        variant = "thread"
     N = states.shape[1]
     buf = torch.from_numpy(states).cuda()
     status = torch.full((N,), -7, dtype=torch.int32, device="cuda")
