@@ -48,7 +48,7 @@ struct Launch {
 #define CKB_AUTO_SUB4_MIN_N_RKCK 12288
 #define CKB_AUTO_SUB4_MIN_N_RKC 24576
 #define CKB_AUTO_THREAD_MIN_N 196608
-#define CKB_AUTO_THREAD_MIN_N_SPECIALISED 65536 /* after ckb_mech_specialize(): thread-per-ODE is ~1.5x faster */
+#define CKB_AUTO_THREAD_MIN_N_SPECIALISED 98304 /* after ckb_mech_specialize(): thread-per-ODE is ~1.8x faster at full size */
 
 int choose(const ckb_mech *m, int variant, long long N, int method, Launch *out) {
   const int n = m->K + 1;

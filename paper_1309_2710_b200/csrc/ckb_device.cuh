@@ -32,6 +32,9 @@ namespace ckb {
 #ifndef CKB_XS_RKC_F0
 #define CKB_XS_RKC_F0 0 /* thread-per-ODE RKC: 1 = f0 and w_{j-2} live in the shared scratch too */
 #endif
+#ifndef CKB_BLOCK_LOCKSTEP
+#define CKB_BLOCK_LOCKSTEP 0
+#endif
 #ifndef CKB_UNROLL_SLOTS
 #define CKB_UNROLL_SLOTS 1 /* reaction slots in flight per lane: 2 slots = 4 independent exp chains */
 #endif
@@ -865,7 +868,9 @@ struct Rkc {
  * refill": a lane whose system has finished fetches the next one while its warp neighbours are still
  * sub-stepping, so finished lanes never idle behind a slow neighbour (divergence control).
  * ---------------------------------------------------------------------------------------------- */
+#ifndef CKB_BLOCK
 #define CKB_BLOCK 128
+#endif
 #ifndef CKB_MINB
 #define CKB_MINB 1 /* resident blocks per SM the register allocation must allow (set per instantiation) */
 #endif
@@ -960,6 +965,11 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
       }
       any = any || active[q];
     }
+#if CKB_BLOCK_LOCKSTEP
+    /* the warps of a block enter f(y) together (one instruction stream per block through the instruction caches:
+     * the generated straight-line f(y) is larger than the 32 KB L1.5 I-cache) and leave the loop together */
+    any = __syncthreads_or(any);
+#endif
     if (!any) break;
     /* an idle slot (queue exhausted) keeps evaluating its last argument: harmless, never stored */
     sys.rhs([&](int q, int i) -> double { return integ[q].w[i]; }, f);
