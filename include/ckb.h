@@ -38,7 +38,8 @@ extern "C" {
 #define CKB_METHOD_RKC 1
 
 /* variant: how ODE systems are mapped onto lanes */
-#define CKB_VARIANT_AUTO 0    /* thread-per-ODE for K+1 <= 16 and N >= 40960 (RKC: 65536), else warp   */
+#define CKB_VARIANT_AUTO 0    /* K+1 > 16: warp.  K+1 <= 16: warp for small N, 4 lanes from N = 12288 (RKC:
+                                 24576), thread from N = 196608 (98304 after ckb_mech_specialize)          */
 #define CKB_VARIANT_THREAD 1  /* one thread integrates one system (the paper's mapping)        */
 #define CKB_VARIANT_WARP 2    /* one warp integrates one system; species and reactions over lanes     */
 #define CKB_VARIANT_SUB8 3    /* 8 lanes per system (4 systems per warp)                              */
@@ -130,7 +131,8 @@ const char *ckb_codegen_log(void); /* compiler log of the calling thread's last 
  *   stream           cudaStream_t as void* (NULL = legacy default stream).
  * Asynchronous on `stream`: never synchronises, allocates nothing.  Stateless between calls.
  * N == 0 is a no-op.  Errors: CKB_EINVAL for bad arguments, CKB_EUNSUPPORTED if the variant cannot hold
- * the mechanism (thread-per-ODE needs K+1 <= 16; lane-distributed variants need K+1 <= 4*lanes...),
+ * the mechanism (thread-per-ODE and the 2- / 4-lane variants need K+1 <= 16, the others K+1 <= 4, 7 or 14 times
+ * the lanes per system, see ckb_host.h),
  * CKB_ECUDA if the launch failed.
  */
 int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, double p_uniform,

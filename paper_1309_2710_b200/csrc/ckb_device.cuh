@@ -35,6 +35,9 @@ namespace ckb {
 #ifndef CKB_BLOCK_LOCKSTEP
 #define CKB_BLOCK_LOCKSTEP 0
 #endif
+#ifndef CKB_XS_RKC_Y
+#define CKB_XS_RKC_Y 0 /* ... and y as well */
+#endif
 #ifndef CKB_UNROLL_SLOTS
 #define CKB_UNROLL_SLOTS 1 /* reaction slots in flight per lane: 2 slots = 4 independent exp chains */
 #endif
@@ -91,7 +94,7 @@ __device__ __forceinline__ double ckb_exp(double x, const ExpConst<PIN> &c) {
 template <int L_, int NV_, class TAB, int M_ = 1>
 struct Sys {
   /* M systems share the lanes of a group and are evaluated together: every table word is loaded and decoded
-   * once for all of them, and their (independent) dependency chains interleave -- DESIGN.md 6.5. */
+   * once for all of them, and their (independent) dependency chains interleave -- DESIGN.md 7.4. */
   static constexpr int L = L_, NV = NV_, G = 32 / L_, M = M_;
   /* shared-memory interleave: thread-per-ODE interleaves the 32 systems of a warp element by element (conflict
    * free: all lanes read the same element); lane-distributed mappings give every system a contiguous region */
@@ -533,6 +536,7 @@ struct Rkck {
     return stage == 0;
   }
 
+  __device__ __forceinline__ double y_at(const S &, int i) const { return y[i]; }
   __device__ __forceinline__ void result(int (&st)[4]) const {
     st[0] = nfe; st[1] = nacc; st[2] = nrej; st[3] = 0;
   }
@@ -575,8 +579,9 @@ struct Rkc {
   double w[NV];                                   /* the next argument of f: y, z (power method), w_{j-1} */
   static constexpr bool XS = (S::L == 1); /* eigenvector estimate v in shared scratch */
   static constexpr bool XSF = XS && (CKB_XS_RKC_F0 != 0); /* f0 and w_{j-2} as well (specialised kernels) */
-  static constexpr int XDOUBLES = XS ? (XSF ? 3 : 1) * NV : 0;
-  double y[NV];
+  static constexpr bool XSY = XSF && (CKB_XS_RKC_Y != 0); /* and y */
+  static constexpr int XDOUBLES = XS ? (XSY ? 4 : XSF ? 3 : 1) * NV : 0;
+  XVec<S, 3, XSY> y;
   XVec<S, 1, XSF> f0;
   XVec<S, 2, XSF> wjm2;
   XVec<S, 0, XS> v;
@@ -587,11 +592,11 @@ struct Rkc {
   int nfe, nacc, nrej, smax_used, attempts, since_sigma, status, flag;
   bool last, have_prev, saw_nonfinite, sigma_fresh, need_sigma, pm_initial;
 
-  __device__ __forceinline__ void start(const S & /*sys*/, const double (&y0)[NV], double t0_, double t1_, double rtol_,
+  __device__ __forceinline__ void start(const S &sys, const double (&y0)[NV], double t0_, double t1_, double rtol_,
                                         double atol_, int n) {
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      y[i] = y0[i];
+      y.set(sys, i, y0[i]);
       w[i] = y0[i];
     }
     t = t0_; t1 = t1_; Dt = t1_ - t0_; rtol = rtol_; atol = atol_; nd = (double)n;
@@ -614,7 +619,7 @@ struct Rkc {
     double a = 0.0, b = 0.0;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      a = fma(y[i], y[i], a);
+      a = fma(y.get(sys, i), y.get(sys, i), a);
       const double vi = v.get(sys, i);
       b = fma(vi, vi, b);
     }
@@ -623,11 +628,11 @@ struct Rkc {
       pm_d = ynrm * CKB_SQRTU;
       const double r = pm_d / vnrm;
 #pragma unroll
-      for (int i = 0; i < NV; i++) w[i] = fma(v.get(sys, i), r, y[i]);
+      for (int i = 0; i < NV; i++) w[i] = fma(v.get(sys, i), r, y.get(sys, i));
     } else if (ynrm != 0.0) {
       pm_d = ynrm * CKB_SQRTU;
 #pragma unroll
-      for (int i = 0; i < NV; i++) w[i] = y[i] * (1.0 + CKB_SQRTU);
+      for (int i = 0; i < NV; i++) w[i] = y.get(sys, i) * (1.0 + CKB_SQRTU);
     } else if (vnrm != 0.0) {
       pm_d = CKB_U;
       const double r = pm_d / vnrm;
@@ -684,8 +689,8 @@ struct Rkc {
     const double mh = mut1 * h;
 #pragma unroll
     for (int i = 0; i < NV; i++) {
-      wjm2.set(sys, i, y[i]);
-      w[i] = fma(mh, f0.get(sys, i), y[i]); /* Eq. 19 */
+      wjm2.set(sys, i, y.get(sys, i));
+      w[i] = fma(mh, f0.get(sys, i), y.get(sys, i)); /* Eq. 19 */
     }
     j = 2;
     state = S_STAGE;
@@ -717,12 +722,12 @@ struct Rkc {
           if (dd != 0.0) {
             const double r = pm_d / dd;
 #pragma unroll
-            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0.get(sys, i), r, y[i]);
+            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0.get(sys, i), r, y.get(sys, i));
           } else {
             const int ci = pm_it % (int)nd;
 #pragma unroll
             for (int i = 0; i < NV; i++)
-              if (sys.g + S::L * i == ci) w[i] = y[i] - (w[i] - y[i]);
+              if (sys.g + S::L * i == ci) w[i] = y.get(sys, i) - (w[i] - y.get(sys, i));
           }
           pm_it++;
           return false;
@@ -733,16 +738,16 @@ struct Rkc {
           if (dd != 0.0) {
             const double r = pm_d / dd;
 #pragma unroll
-            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0.get(sys, i), r, y[i]);
+            for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0.get(sys, i), r, y.get(sys, i));
           } else {
             const int ci = pm_it % (int)nd;
 #pragma unroll
             for (int i = 0; i < NV; i++)
-              if (sys.g + S::L * i == ci) w[i] = y[i] - (w[i] - y[i]);
+              if (sys.g + S::L * i == ci) w[i] = y.get(sys, i) - (w[i] - y.get(sys, i));
           }
         }
 #pragma unroll
-        for (int i = 0; i < NV; i++) v.set(sys, i, w[i] - y[i]);
+        for (int i = 0; i < NV; i++) v.set(sys, i, w[i] - y.get(sys, i));
         sigma = 1.2 * pm_sigma; /* R18 */
         sigma_fresh = true;
         need_sigma = false;
@@ -751,7 +756,7 @@ struct Rkc {
         /* initial step, Eq. 36-37 (R14, R15): probe f(y + h0 f0) */
         h_old = (sigma > 0.0 && 1.0 / sigma < Dt) ? 1.0 / sigma : Dt; /* h0, parked in h_old */
 #pragma unroll
-        for (int i = 0; i < NV; i++) w[i] = fma(h_old, f0.get(sys, i), y[i]);
+        for (int i = 0; i < NV; i++) w[i] = fma(h_old, f0.get(sys, i), y.get(sys, i));
         state = S_H0;
         return false;
       }
@@ -762,7 +767,7 @@ struct Rkc {
         for (int i = 0; i < NV; i++) {
           if (sys.valid(i)) {
             const double d0 = h0 * (f[i] - f0.get(sys, i));
-            const double wt = fma(rtol, fabs(y[i]), atol);
+            const double wt = fma(rtol, fabs(y.get(sys, i)), atol);
             const double q = d0 / wt;
             acc = fma(q, q, acc);
           }
@@ -788,7 +793,7 @@ struct Rkc {
         const double c0 = 1.0 - mu - nu, mh = mut * h, gh = gamt * h;
 #pragma unroll
         for (int i = 0; i < NV; i++) {
-          const double wj = fma(gh, f0.get(sys, i), fma(mh, f[i], fma(nu, wjm2.get(sys, i), fma(mu, w[i], c0 * y[i]))));
+          const double wj = fma(gh, f0.get(sys, i), fma(mh, f[i], fma(nu, wjm2.get(sys, i), fma(mu, w[i], c0 * y.get(sys, i)))));
           wjm2.set(sys, i, w[i]);
           w[i] = wj;
         }
@@ -803,8 +808,8 @@ struct Rkc {
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       if (sys.valid(i)) {
-        const double del = fma(0.8, y[i] - w[i], 0.4 * h * (f0.get(sys, i) + f[i]));
-        const double wt = fma(rtol, fmax(fabs(y[i]), fabs(w[i])), atol);
+        const double del = fma(0.8, y.get(sys, i) - w[i], 0.4 * h * (f0.get(sys, i) + f[i]));
+        const double wt = fma(rtol, fmax(fabs(y.get(sys, i)), fabs(w[i])), atol);
         const double q = del / wt;
         acc = fma(q, q, acc);
       }
@@ -821,7 +826,7 @@ struct Rkc {
       fac = fmin(10.0, fmax(0.1, fac)); /* Eq. 33 */
 #pragma unroll
       for (int i = 0; i < NV; i++) {
-        y[i] = w[i];
+        y.set(sys, i, w[i]);
         f0.set(sys, i, f[i]);
       }
       err_old = err;
@@ -852,6 +857,7 @@ struct Rkc {
     return begin_step(sys);
   }
 
+  __device__ __forceinline__ double y_at(const S &sys, int i) const { return y.get(sys, i); }
   __device__ __forceinline__ void result(int (&st)[4]) {
     if (status == ST_OK && flag) status = flag;
     st[0] = nfe; st[1] = nacc; st[2] = nrej; st[3] = smax_used;
@@ -981,7 +987,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
 #pragma unroll
         for (int i = 0; i < NV; i++) {
           const int c = sys.g + L * i;
-          if (c < m.n) states[(size_t)sys.tw(m.o_perm + c) * ld + ode[q]] = integ[q].y[i];
+          if (c < m.n) states[(size_t)sys.tw(m.o_perm + c) * ld + ode[q]] = integ[q].y_at(sys, i);
         }
         if (sys.g == 0) {
           if (status) status[ode[q]] = integ[q].status;
