@@ -205,14 +205,14 @@ class GpuCase:
         self.m.close()
 
 
-def measured_traffic(cfg, N):
+def measured_traffic(cfg, N, specialised=False):
     """dram__bytes_read.sum + dram__bytes_write.sum of the integrate kernel for this workload, from the committed
     ncu --set full capture (profiles/traffic.json, written from the capture named there), per launch; else None."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(path):
         with open(path) as fh:
             for e in json.load(fh).get("captures", []):
-                if e["config"] == cfg and e["N"] == N:
+                if e["config"] == cfg and e["N"] == N and bool(e.get("specialised", False)) == bool(specialised):
                     return e["dram_bytes_read"] + e["dram_bytes_write"]
     return None
 
@@ -221,7 +221,7 @@ def roofline(case, ms, work, peak_tflops, peak_src):
     flops = case.m.flops_per_rhs * work["rhs_calls"]
     ach = flops / (ms * 1e-3) / 1e12
     return {"bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s", "frac": ach / peak_tflops,
-            "traffic": measured_traffic(case.cfg, case.N), "peak_source": peak_src, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
+            "traffic": measured_traffic(case.cfg, case.N, case.specialized), "peak_source": peak_src, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
             "flops_per_rhs": case.m.flops_per_rhs, "rhs_calls_per_launch": work["rhs_calls"],
             "kernel_ms": ms, "hbm_algorithmic_GBps": 2 * 8 * (case.mech.n_species + 1) * case.N / (ms * 1e-3) / 1e9}
 
