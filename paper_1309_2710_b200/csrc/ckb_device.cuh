@@ -41,6 +41,9 @@ namespace ckb {
 #ifndef CKB_RKCK_ALIGN
 #define CKB_RKCK_ALIGN 1 /* thread-per-ODE RKCK: the lanes of a warp stay in the same stage (integrate_kernel): +35 % */
 #endif
+#ifndef CKB_RKC_ALIGN
+#define CKB_RKC_ALIGN 1 /* RKC, several systems per warp: they line up on stage / error-estimate evaluations */
+#endif
 #ifndef CKB_UNROLL_SLOTS
 #define CKB_UNROLL_SLOTS 1 /* reaction slots in flight per lane: 2 slots = 4 independent exp chains */
 #endif
@@ -861,6 +864,10 @@ struct Rkc {
   }
 
   __device__ __forceinline__ double y_at(const S &sys, int i) const { return y.get(sys, i); }
+  /* what the next advance() will do: 3 = error estimate, 2 = last stage of a step, 1 = earlier stage, 0 = other */
+  __device__ __forceinline__ int phase() const {
+    return state == S_FINAL ? 3 : state == S_STAGE ? (j == s ? 2 : 1) : 0;
+  }
   __device__ __forceinline__ void result(int (&st)[4]) {
     if (status == ST_OK && flag) status = flag;
     st[0] = nfe; st[1] = nacc; st[2] = nrej; st[3] = smax_used;
@@ -952,6 +959,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
 #pragma unroll
     for (int i = 0; i < NV; i++) integ[q].w[i] = 1.0; /* finite argument for a slot that never gets a system */
   }
+  bool held_last = false;
   while (true) {
     bool any = false;
 #pragma unroll
@@ -980,16 +988,28 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
     any = __syncthreads_or(any);
 #endif
     if (!any) break;
-    /* Thread-per-ODE RKCK: keep the lanes of a warp in the same stage, so that the stage switch of advance() is
+    /* RKCK with several systems per warp (L < 32): keep the lanes of a warp in the same stage, so that the stage switch of advance() is
      * warp-uniform instead of up to six serialised paths.  Lanes only fall out of step at an attempt boundary:
      * after an accepted step (or a refill) the next evaluation is stage 1 (k1 = f(y)), after a rejection it is
      * stage 2 (k1 rescaled, R25).  When some lane needs stage 1, the stage-2 lanes sit that evaluation out (their
      * argument is evaluated again next time: same values, not counted). */
     bool hold = false;
-    if constexpr (METHOD == 0 && L == 1 && M == 1 && CKB_RKCK_ALIGN != 0) {
+    if constexpr (METHOD == 0 && L < 32 && M == 1 && CKB_RKCK_ALIGN != 0) {
       const bool s1 = active[0] && integ[0].stage == 1;
       const bool any1 = __any_sync(0xffffffffu, s1); /* every lane votes */
       hold = active[0] && !s1 && any1;
+    }
+    /* RKC with several systems per warp: a step with s stages is s - 1 stage evaluations (S_STAGE) and the evaluation of the error
+     * estimate (S_FINAL); with lane refill and the occasional power-method excursion the lanes of a warp drift
+     * into both at once, and advance() then runs both paths one after the other.  A lane in the minority sits one
+     * evaluation out when that lines it up with the majority: S_FINAL lanes wait for lanes that are in their last
+     * stage, last-stage lanes wait for S_FINAL lanes (which start their next step's stages afterwards).  Never
+     * twice in a row, so no lane starves. */
+    if constexpr (METHOD == 1 && L < 32 && M == 1 && CKB_RKC_ALIGN != 0) {
+      const int ph = active[0] ? integ[0].phase() : 0;
+      const int n_last = __popc(__ballot_sync(0xffffffffu, ph == 2)), n_final = __popc(__ballot_sync(0xffffffffu, ph == 3));
+      hold = !held_last && ((ph == 3 && n_last > 0 && n_last >= n_final) || (ph == 2 && n_final > n_last));
+      held_last = hold;
     }
     /* an idle slot (queue exhausted) keeps evaluating its last argument: harmless, never stored */
     sys.rhs([&](int q, int i) -> double { return integ[q].w[i]; }, f);
