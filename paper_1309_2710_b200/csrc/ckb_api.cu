@@ -6,6 +6,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstdio>
 #include <cstring>
 #include <limits>
@@ -266,9 +267,19 @@ int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, doub
     CK(cudaMalloc((void **)&m->ws_stats, (size_t)N * 4 * sizeof(int32_t)));
     m->ws_n_cap = (size_t)N;
   }
-  /* Large batches go through in chunks on internal streams, so that the upload of chunk c+1 and the download of
-   * chunk c-1 overlap the kernel of chunk c (PCIe is full duplex).  The device copy is dense (row stride N). */
-  const int chunks = (N >= 65536) ? CKB_SCRATCH_SLOTS : 1;
+  /* Large RKCK batches go through in chunks on internal streams, so that the upload of chunk c+1 and the download of
+   * chunk c-1 overlap the kernel of chunk c (PCIe is full duplex): there the kernel takes about as long as either
+   * copy (configs[1]: 0.64 ms against 0.8 ms each way).  One stream per chunk: measured faster than one upload, one
+   * compute and one download stream (1.57 against 1.80 ms; concurrent row-wise copies use more copy engines).
+   * RKC batches are stiff problems whose kernel outlasts the copies by one to two orders of magnitude; splitting them
+   * only adds a queue tail per chunk (configs[2]: 80 ms in 3 chunks against 46 ms in one), so they go through whole.
+   * The device copy is dense (row stride N). */
+  static const int max_chunks = [] {
+    const char *e = std::getenv("CKB_HOST_CHUNKS"); /* tuning knob, 1..CKB_SCRATCH_SLOTS */
+    const int v = e ? std::atoi(e) : CKB_SCRATCH_SLOTS;
+    return v < 1 ? 1 : v > CKB_SCRATCH_SLOTS ? CKB_SCRATCH_SLOTS : v;
+  }();
+  const int chunks = (N >= 65536 && method == CKB_METHOD_RKCK) ? max_chunks : 1;
   if (chunks > 1 && !m->hstream[0]) {
     for (int i = 0; i < CKB_SCRATCH_SLOTS; i++) CK(cudaStreamCreateWithFlags(&m->hstream[i], cudaStreamNonBlocking));
     for (int i = 0; i <= CKB_SCRATCH_SLOTS; i++) CK(cudaEventCreateWithFlags(&m->hevent[i], cudaEventDisableTiming));
