@@ -40,6 +40,13 @@ def systems_per_group(L: int, NV: int) -> int:
     return int(os.environ.get("CKB_M32", "1")) if L == 32 else 1
 
 
+def exp_table(L: int) -> int:
+    """1 = exp through the 64-entry 2^(j/64) table in shared memory (12 FP64 instructions + one shared read instead of
+    17 FP64 instructions): pays where the FP64 pipe is the busy unit and the load/store pipe is not."""
+    env = os.environ.get("CKB_EXP_TABLE_MAXL", "0")
+    return 1 if L <= int(env) else 0
+
+
 def min_blocks(L: int, NV: int, method: str = "rkck") -> int:
     """Resident 128-thread blocks per SM that the register allocation of integrate_kernel<L, NV> must allow
     (launch bounds): 4 -> <= 128 registers, 3 -> <= 168, 2 -> <= 255.  Chosen so that no instantiation spills."""
@@ -102,7 +109,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     os.makedirs(OBJ, exist_ok=True)
     flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("CKB_DEFS", "").split()  # tuning knobs
     stamp = os.path.join(OBJ, "stamp")
-    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", "") + os.environ.get("CKB_MINB_L24", "") + os.environ.get("CKB_US_L1", ""))
+    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", "") + os.environ.get("CKB_MINB_L24", "") + os.environ.get("CKB_US_L1", "") + os.environ.get("CKB_EXP_TABLE_MAXL", ""))
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     _embed_sources()
@@ -114,6 +121,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
         obj = os.path.join(OBJ, f"ckb_inst_L{L}_NV{NV}.o")
         jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_MINB={min_blocks(L, NV)}", f"-DCKB_MINB_RKC={min_blocks(L, NV, 'rkc')}",
                            f"-DCKB_UNROLL_SLOTS={int(os.environ.get('CKB_US_L1', '1')) if L == 1 else int(os.environ.get('CKB_US', '1'))}",
+                           f"-DCKB_EXP_TABLE={exp_table(L)}",
                            f"-DCKB_M={systems_per_group(L, NV)}", "-c",
                            os.path.join(CSRC, "ckb_inst.cu"), "-o", obj]))
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
