@@ -144,9 +144,13 @@ def test_codegen_text(L):
                                for e in range(mech.tb_ptr[r], mech.tb_ptr[r + 1])))
                   for r in range(len(mech.tb_reaction))})
     assert src.count("= ctot;") == n_sets + 0
-    toy = synth.toy_mechanism(2, [({0: 2}, {1: 1}, 5.0, 0.0, 0.0), ({1: 1}, {0: 2}, 0.0, 0.0, 0.0)])
+    toy = synth.toy_mechanism(2, [({0: 2}, {1: 1}, 5.0, 0.0, 300.0), ({1: 1}, {0: 2}, 0.0, 0.0, 0.0)])
     s2 = binding.codegen(toy)
     assert s2.count("ckb_exp(") == 1 and "fma(-0x1p+1, q, om" in s2      # A = 0: no rate; nu' = 2 on the reactant
+    assert "lnT, " not in s2                                             # beta = 0: the term is not emitted
+    toy = synth.toy_mechanism(2, [({0: 1}, {1: 1}, 5.0, 0.0, 0.0)])
+    s3 = binding.codegen(toy)
+    assert "ckb_exp(" not in s3 and "double rf = 0x1.4p+2;" in s3        # no temperature dependence: a literal
     with pytest.raises(binding.CkbError):
         binding.codegen(synth.make_mechanism(3))
 

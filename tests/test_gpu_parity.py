@@ -267,7 +267,7 @@ def test_toy_mechanisms_closed_form():
     states[1] = np.linspace(0.1, 1.0, N)
     states[2] = 1.0 - states[1]
     for method in ("rkck", "rkc"):
-        for variant in ("thread", "warp"):
+        for variant in ("thread", "warp", "sub4", "gen"):   # "gen": the rate constant is emitted as a literal
             y, st, _ = _run_gpu(mech, states, synth.P_ATM, 1e-6, method, variant=variant)
             assert (st == 0).all()
             # global error: RKCK (5th order) ~ rtol; RKC (2nd order, ~1e2 steps at rtol 1e-8) ~ 1e2 rtol
