@@ -1023,7 +1023,12 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
 #if CKB_BLOCK_LOCKSTEP
     /* the warps of a block enter f(y) together (one instruction stream per block through the instruction caches:
      * the generated straight-line f(y) is larger than the 32 KB L1.5 I-cache) and leave the loop together */
-    any = __syncthreads_or(any);
+    {
+      const bool mine = any;
+      any = __syncthreads_or(any);
+      /* a warp that has run out of systems only keeps the barrier: the stragglers of the block get its issue slots */
+      if (any && !__any_sync(0xffffffffu, mine)) continue;
+    }
 #endif
     if (!any) break;
     /* RKCK with several systems per warp (L < 32): keep the lanes of a warp in the same stage, so that the stage switch of advance() is
