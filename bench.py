@@ -41,6 +41,7 @@ HEADLINE_N = {0: 1024, 1: 2 ** 19, 2: 2 ** 18, 3: 2 ** 17, 4: 2 ** 16}
 
 
 def parse():
+    global RTOL, ATOL
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
@@ -49,13 +50,17 @@ def parse():
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--n", type=int, default=0, help="override the batch size N")
     ap.add_argument("--dt", type=float, default=0.0)
+    ap.add_argument("--rtol", type=float, default=RTOL, help="relative tolerance (default: BASELINE.json's 1e-8)")
+    ap.add_argument("--atol", type=float, default=ATOL, help="absolute tolerance (default: BASELINE.json's 1e-12)")
     ap.add_argument("--variant", default="auto")
     ap.add_argument("--ordering", default="shuffled", choices=["shuffled", "similar"])
     ap.add_argument("--no-specialize", action="store_true",
                     help="keep the table-driven thread-per-ODE kernels (no runtime-generated mechanism code)")
     ap.add_argument("--no-extra", action="store_true", help="skip the other configs, e2e and cpu_baseline")
     ap.add_argument("--sweep", action="store_true", help="also sweep N over the config's N_list")
-    return ap.parse_args()
+    args = ap.parse_args()
+    RTOL, ATOL = args.rtol, args.atol   # every leg (ours, e2e, oracle) uses the same tolerances
+    return args
 
 
 def workload(cfg, n_override=0, dt=0.0):
