@@ -39,7 +39,8 @@ extern "C" {
 
 /* variant: how ODE systems are mapped onto lanes */
 #define CKB_VARIANT_AUTO 0    /* K+1 > 16: warp.  K+1 <= 16: warp for small N, 4 lanes from N = 12288 (RKC:
-                                 24576), thread from N = 196608 (98304 after ckb_mech_specialize)          */
+                                 24576), thread from N = 131072 (RKC: 196608); after ckb_mech_specialize
+                                 thread from N = 49152 (RKC: 98304)                                     */
 #define CKB_VARIANT_THREAD 1  /* one thread integrates one system (the paper's mapping)        */
 #define CKB_VARIANT_WARP 2    /* one warp integrates one system; species and reactions over lanes     */
 #define CKB_VARIANT_SUB8 3    /* 8 lanes per system (4 systems per warp)                              */

@@ -50,7 +50,8 @@ struct Launch {
 #define CKB_AUTO_SUB4_MIN_N_RKC 24576
 #define CKB_AUTO_THREAD_MIN_N_RKCK 131072
 #define CKB_AUTO_THREAD_MIN_N 196608
-#define CKB_AUTO_THREAD_MIN_N_SPECIALISED 98304 /* after ckb_mech_specialize(): thread-per-ODE is ~1.8x faster at full size */
+#define CKB_AUTO_THREAD_MIN_N_SPECIALISED 98304 /* after ckb_mech_specialize(): thread-per-ODE is ~2x faster at full size */
+#define CKB_AUTO_THREAD_MIN_N_SPECIALISED_RKCK 49152
 
 int choose(const ckb_mech *m, int variant, long long N, int method, Launch *out) {
   const int n = m->K + 1;
@@ -59,7 +60,8 @@ int choose(const ckb_mech *m, int variant, long long N, int method, Launch *out)
     const bool sub4_ok = n <= 16 && m->pk[ckb_host::pack_index(4)].rc == CKB_OK;
     const bool warp_ok = m->pk[ckb_host::pack_index(32)].rc == CKB_OK;
     const long long sub4_min = method == CKB_METHOD_RKC ? CKB_AUTO_SUB4_MIN_N_RKC : CKB_AUTO_SUB4_MIN_N_RKCK;
-    const long long thread_min = m->gen.ok ? CKB_AUTO_THREAD_MIN_N_SPECIALISED
+    const long long thread_min = m->gen.ok ? (method == CKB_METHOD_RKC ? CKB_AUTO_THREAD_MIN_N_SPECIALISED
+                                                                       : CKB_AUTO_THREAD_MIN_N_SPECIALISED_RKCK)
                                            : (method == CKB_METHOD_RKC ? CKB_AUTO_THREAD_MIN_N : CKB_AUTO_THREAD_MIN_N_RKCK);
     if (thread_ok && (N >= thread_min || (!warp_ok && !sub4_ok)))
       variant = CKB_VARIANT_THREAD;
