@@ -60,6 +60,10 @@ def lib():
         L.ora_integrate.argtypes = [C.c_void_p, dp, dp, C.c_double, C.c_int64, C.c_int64, C.c_double,
                                     C.c_double, C.c_double, C.c_double, C.c_int32, ip, ip, C.c_int32]
         L.ora_integrate.restype = C.c_int
+        L.ora_rhs_cv.argtypes = L.ora_rhs.argtypes
+        L.ora_rhs_cv.restype = None
+        L.ora_integrate_cv.argtypes = L.ora_integrate.argtypes
+        L.ora_integrate_cv.restype = C.c_int
         L.ora_rkck_tableau.argtypes = [dp]
         L.ora_rkck_tableau.restype = None
         L.ora_rkck_step.argtypes = [RHS_FN, C.c_void_p, C.c_int, C.c_double, dp, C.c_double, dp, dp]
@@ -134,14 +138,16 @@ class OracleMech:
             _lib.ora_mech_free(self._h)
             self._h = None
 
-    def rhs(self, y, p):
+    def rhs(self, y, p, cv=False):
+        """f(y) at constant pressure p (dyn/cm^2), or with cv=True at constant volume, p = density (g/cm^3)."""
         y = _f64(y)
         out = np.empty_like(y)
-        lib().ora_rhs(self._h, _dp(y), float(p), _dp(out))
+        (lib().ora_rhs_cv if cv else lib().ora_rhs)(self._h, _dp(y), float(p), _dp(out))
         return out
 
-    def integrate(self, states, p, dt, rtol, atol, method, t=0.0, nthreads=0, pressure=None):
-        """states: [(K+1)][N] SoA (copied).  Returns (new_states, status[N], stats[4][N])."""
+    def integrate(self, states, p, dt, rtol, atol, method, t=0.0, nthreads=0, pressure=None, cv=False):
+        """states: [(K+1)][N] SoA (copied).  Returns (new_states, status[N], stats[4][N]).
+        cv=True: constant volume, p / pressure carry the density in g/cm^3 (reading R29)."""
         method = {"rkck": 0, "rkc": 1}.get(method, method)
         st = np.array(states, dtype=np.float64, order="C", copy=True)
         n, N = st.shape
@@ -149,7 +155,8 @@ class OracleMech:
         status = np.zeros(N, dtype=np.int32)
         stats = np.zeros((4, N), dtype=np.int32)
         pr = None if pressure is None else _f64(pressure)
-        rc = lib().ora_integrate(self._h, _dp(st), None if pr is None else _dp(pr), float(p), N, N,
+        fn = lib().ora_integrate_cv if cv else lib().ora_integrate
+        rc = fn(self._h, _dp(st), None if pr is None else _dp(pr), float(p), N, N,
                                  float(t), float(dt), float(rtol), float(atol), int(method),
                                  _ip(status), _ip(stats), int(nthreads))
         if rc != 0:

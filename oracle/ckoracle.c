@@ -551,8 +551,12 @@ int ora_mech_load(const ora_mech_desc *d, ora_mech **out) {
   return ORA_OK;
 }
 
-/* f(y): y = {T, Y_1..Y_K}, constant pressure p (dyn/cm^2).  work: 2K + R doubles. */
-static void chem_rhs(const ora_mech *m, const double *y, double p, double *dydt, double *work) {
+/* f(y): y = {T, Y_1..Y_K}.  work: 2K + R doubles.
+ * cv = 0: constant pressure, p = pressure in dyn/cm^2 (Eq. 6).
+ * cv = 1: constant volume (P:243 mentions the variant without equations; reading R29, the textbook form): p carries
+ *         the density rho in g/cm^3, constant over the call, and the energy equation is
+ *         rho c_v dT/dt = - sum_k u_k omega_k W_k  with  u_k = h_k - Ru T / W_k  and  c_v = c_p - Ru / Wbar. */
+static void chem_rhs(const ora_mech *m, const double *y, double p, double *dydt, double *work, int cv) {
   const int K = m->K, R = m->R;
   const double T = y[0];
   const double *Y = y + 1;
@@ -560,7 +564,7 @@ static void chem_rhs(const ora_mech *m, const double *y, double p, double *dydt,
   /* R9a: ideal gas at constant pressure: rho = p Wbar/(Ru T), 1/Wbar = sum Y_k/W_k; C_k = rho Y_k / W_k */
   double Sum = 0.0;
   for (int k = 0; k < K; k++) Sum += Y[k] / m->W[k];
-  const double rho = p / (ORA_RU * T * Sum);
+  const double rho = cv ? p : p / (ORA_RU * T * Sum);
   for (int k = 0; k < K; k++) C[k] = rho * Y[k] / m->W[k];
   for (int j = 0; j < R; j++) {
     const double kj = m->A[j] * pow(T, m->beta[j]) * exp(-m->E[j] / (ORA_RC * T));   /* Eq. 5, literal */
@@ -591,29 +595,43 @@ static void chem_rhs(const ora_mech *m, const double *y, double p, double *dydt,
     h_sum += hRT * wdot[k];                 /* (h_k W_k)/(Ru T) * omega_k */
   }
   const double cp = ORA_RU * cp_sum;        /* mass-averaged c_p */
-  dydt[0] = -(ORA_RU * T * h_sum) / (rho * cp);                 /* Eq. 6 */
+  if (cv) {                                 /* R29 */
+    double w_sum = 0.0;
+    for (int k = 0; k < K; k++) w_sum += wdot[k];
+    const double cvm = cp - ORA_RU * Sum;   /* c_v = c_p - Ru / Wbar */
+    dydt[0] = -(ORA_RU * T * (h_sum - w_sum)) / (rho * cvm);    /* sum_k (h_k/(Ru T) - 1) omega_k */
+  } else {
+    dydt[0] = -(ORA_RU * T * h_sum) / (rho * cp);               /* Eq. 6 */
+  }
   for (int k = 0; k < K; k++) dydt[1 + k] = m->W[k] * wdot[k] / rho; /* Eq. 2 */
 }
 
 void ora_rhs(const ora_mech *m, const double *y, double p, double *dydt) {
   double *work = (double *)malloc(sizeof(double) * (2 * (size_t)m->K + (size_t)m->R + 1));
-  chem_rhs(m, y, p, dydt, work);
+  chem_rhs(m, y, p, dydt, work, 0);
   free(work);
 }
 
-typedef struct { const ora_mech *m; double p; double *work; } chem_ctx;
+/* constant volume: rho in g/cm^3 */
+void ora_rhs_cv(const ora_mech *m, const double *y, double rho, double *dydt) {
+  double *work = (double *)malloc(sizeof(double) * (2 * (size_t)m->K + (size_t)m->R + 1));
+  chem_rhs(m, y, rho, dydt, work, 1);
+  free(work);
+}
+
+typedef struct { const ora_mech *m; double p; double *work; int cv; } chem_ctx;
 
 static void chem_rhs_cb(double t, const double *y, double *dydt, void *ctx) {
   (void)t;                                   /* autonomous */
   chem_ctx *c = (chem_ctx *)ctx;
-  chem_rhs(c->m, y, c->p, dydt, c->work);
+  chem_rhs(c->m, y, c->p, dydt, c->work, c->cv);
 }
 
 /* Batch entry mirroring the product's integrate(): states are HOST, SoA [(K+1)][ld], updated in place.
  * method 0 = RKCK, 1 = RKC.  status [N] and stats [4][N] may be NULL.  nthreads <= 0 -> OpenMP default. */
-int ora_integrate(const ora_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
-                  int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
-                  int32_t *status, int32_t *stats, int32_t nthreads) {
+static int integrate_closure(const ora_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                             int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                             int32_t *status, int32_t *stats, int32_t nthreads, int cv) {
   if (!m || !states || N < 0 || ld < N || (method != 0 && method != 1) || !(dt > 0.0) || !(rtol > 0.0) ||
       !(atol >= 0.0))
     return ORA_EINVAL;
@@ -630,6 +648,7 @@ int ora_integrate(const ora_mech *m, double *states, const double *pressure, dou
     chem_ctx ctx;
     ctx.m = m;
     ctx.work = work;
+    ctx.cv = cv;
 #pragma omp for schedule(dynamic, 16)
     for (int64_t i = 0; i < N; i++) {
       for (int c = 0; c < n; c++) y[c] = states[(size_t)c * ld + i];
@@ -646,6 +665,19 @@ int ora_integrate(const ora_mech *m, double *states, const double *pressure, dou
     free(work);
   }
   return ORA_OK;
+}
+
+int ora_integrate(const ora_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                  int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                  int32_t *status, int32_t *stats, int32_t nthreads) {
+  return integrate_closure(m, states, pressure, p_uniform, N, ld, t, dt, rtol, atol, method, status, stats, nthreads, 0);
+}
+
+/* constant volume (R29): density[] / rho_uniform in g/cm^3 in place of the pressure */
+int ora_integrate_cv(const ora_mech *m, double *states, const double *density, double rho_uniform, int64_t N,
+                     int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                     int32_t *status, int32_t *stats, int32_t nthreads) {
+  return integrate_closure(m, states, density, rho_uniform, N, ld, t, dt, rtol, atol, method, status, stats, nthreads, 1);
 }
 
 int ora_num_threads(void) {
