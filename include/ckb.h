@@ -151,6 +151,23 @@ int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, doub
                        int32_t variant, int32_t *status, int32_t *stats, void *stream);
 
 /*
+ * Constant-volume closure (the other operator-split chemistry mode; P:243 names it without equations, DESIGN.md
+ * reading R29 takes the textbook form): the density rho of each system is given and constant over the call,
+ *     C_k = rho Y_k / W_k,    dY_k/dt = W_k omega_k / rho                       (Eq. 2-5 unchanged)
+ *     rho c_v dT/dt = - sum_k u_k omega_k W_k,   u_k = h_k - Ru T / W_k,   c_v = c_p - Ru sum_k Y_k / W_k
+ * and the pressure follows from the ideal-gas law.  ckb_integrate_cv / ckb_integrate_host_cv / ckb_rhs_cv are
+ * ckb_integrate / ckb_integrate_host / ckb_rhs with `density` (DEVICE resp. HOST [N], g/cm^3, or NULL to use
+ * rho_uniform > 0) in place of the pressure; every other argument, the layouts, the mapping variants, the
+ * asynchrony and the error behaviour are the same.  The same kernels run (the closure is a launch-uniform flag).
+ */
+int ckb_integrate_cv(const ckb_mech *m, double *states, const double *density, double rho_uniform, int64_t N,
+                     int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
+                     int32_t *status, int32_t *stats, void *stream);
+int ckb_integrate_host_cv(ckb_mech *m, double *states, const double *density, double rho_uniform, int64_t N,
+                          int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                          int32_t variant, int32_t *status, int32_t *stats, void *stream);
+
+/*
  * ckb_rhs: evaluate the source term f(y) (Eq. 2-6) once for each of N systems, without integrating;
  * dydt DEVICE [(K+1)][ld] receives (dT/dt, dY_k/dt).  Same layout and mapping variants as
  * ckb_integrate.  Used by the parity tests of the source term and by the roofline measurement.
@@ -158,6 +175,8 @@ int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, doub
  */
 int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, double p_uniform, int64_t N,
             int64_t ld, double *dydt, int32_t variant, int32_t repeat, void *stream);
+int ckb_rhs_cv(const ckb_mech *m, const double *states, const double *density, double rho_uniform, int64_t N,
+               int64_t ld, double *dydt, int32_t variant, int32_t repeat, void *stream);
 
 /*
  * ckb_fp64_probe: roofline denominator.  Runs a register-resident kernel of independent DFMA chains on

@@ -22,7 +22,8 @@ ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
 # every symbol include/ckb.h declares
 EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "ckb_integrate_host",
            "ckb_rhs", "ckb_fp64_probe", "ckb_mech_pack_stats", "ckb_strerror", "ckb_last_cuda_error",
-           "ckb_mech_specialize", "ckb_mech_precompile", "ckb_mech_codegen", "ckb_codegen_log")
+           "ckb_mech_specialize", "ckb_mech_precompile", "ckb_mech_codegen", "ckb_codegen_log",
+           "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv")
 
 
 class CkbError(RuntimeError):
@@ -74,6 +75,12 @@ def lib():
     L.ckb_integrate_host.restype = C.c_int
     L.ckb_rhs.argtypes = [vp, vp, vp, dbl, i64, i64, vp, i32, i32, vp]
     L.ckb_rhs.restype = C.c_int
+    L.ckb_integrate_cv.argtypes = integ
+    L.ckb_integrate_cv.restype = C.c_int
+    L.ckb_integrate_host_cv.argtypes = integ
+    L.ckb_integrate_host_cv.restype = C.c_int
+    L.ckb_rhs_cv.argtypes = L.ckb_rhs.argtypes
+    L.ckb_rhs_cv.restype = C.c_int
     L.ckb_fp64_probe.argtypes = [i32, i64, C.POINTER(dbl), vp]
     L.ckb_fp64_probe.restype = C.c_int
     L.ckb_mech_pack_stats.argtypes = [C.POINTER(_Desc), i32, C.POINTER(i32)]
@@ -212,10 +219,11 @@ def mech_load(mech, specialize=False) -> Mech:
 
 
 def integrate(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None, pressure=None,
-              variant="auto", status=None, stats=None, stream=None):
+              variant="auto", status=None, stats=None, stream=None, cv=False):
     """ckb_integrate: advance states (CUDA float64 tensor [(K+1)][ld], in place) over one global step dt.
 
     p: uniform pressure (dyn/cm^2) or pressure: CUDA tensor [N].  status: int32 CUDA [N]; stats: int32 CUDA [4][N].
+    cv=True calls ckb_integrate_cv: constant volume, p / pressure carry the density in g/cm^3.
     Asynchronous on the current (or given) torch stream.
     """
     import torch
@@ -223,7 +231,7 @@ def integrate(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None,
         raise ValueError("states must be [(K+1)][ld]")
     ld = int(states.shape[1])
     N = ld if N is None else int(N)
-    rc = lib().ckb_integrate(
+    rc = (lib().ckb_integrate_cv if cv else lib().ckb_integrate)(
         m._h, _dev_ptr(states, torch.float64, "states"), _dev_ptr(pressure, torch.float64, "pressure"),
         float(0.0 if p is None else p), N, ld, float(t), float(dt), float(rtol), float(atol),
         int(METHODS.get(method, method)), int(VARIANTS.get(variant, variant)),
@@ -233,8 +241,8 @@ def integrate(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None,
 
 
 def integrate_host(m: Mech, states, dt, rtol, atol, method, *, t=0.0, p=None, pressure=None, variant="auto",
-                   status=None, stats=None, stream=None):
-    """ckb_integrate_host: the same call on HOST buffers (numpy float64 [(K+1)][N] C-contiguous, or a pinned
+                   status=None, stats=None, stream=None, cv=False):
+    """ckb_integrate_host (cv=True: ckb_integrate_host_cv): the same call on HOST buffers (numpy float64 [(K+1)][N] C-contiguous, or a pinned
     CPU torch tensor), host<->device copies inside the call; returns after the stream has been synchronised."""
     def hp(a, dtype):
         if a is None:
@@ -246,7 +254,7 @@ def integrate_host(m: Mech, states, dt, rtol, atol, method, *, t=0.0, p=None, pr
     n, N = int(states.shape[0]), int(states.shape[1])
     if n != m.K + 1:
         raise ValueError("states must be [(K+1)][N]")
-    rc = lib().ckb_integrate_host(
+    rc = (lib().ckb_integrate_host_cv if cv else lib().ckb_integrate_host)(
         m._h, hp(states, np.float64), hp(pressure, np.float64), float(0.0 if p is None else p), N, N, float(t),
         float(dt), float(rtol), float(atol), int(METHODS.get(method, method)), int(VARIANTS.get(variant, variant)),
         hp(status, np.int32), hp(stats, np.int32), _stream_ptr(stream))
@@ -254,18 +262,35 @@ def integrate_host(m: Mech, states, dt, rtol, atol, method, *, t=0.0, p=None, pr
     return states
 
 
-def rhs(m: Mech, states, *, p=None, pressure=None, variant="auto", repeat=1, out=None, N=None, stream=None):
-    """ckb_rhs: f(y) for every system; returns dydt [(K+1)][ld] (CUDA float64)."""
+def rhs(m: Mech, states, *, p=None, pressure=None, variant="auto", repeat=1, out=None, N=None, stream=None,
+        cv=False):
+    """ckb_rhs (cv=True: ckb_rhs_cv, p / pressure carry the density): f(y) for every system; returns dydt
+    [(K+1)][ld] (CUDA float64)."""
     import torch
     ld = int(states.shape[1])
     N = ld if N is None else int(N)
     if out is None:
         out = torch.empty_like(states)
-    rc = lib().ckb_rhs(m._h, _dev_ptr(states, torch.float64, "states"), _dev_ptr(pressure, torch.float64, "pressure"),
+    rc = (lib().ckb_rhs_cv if cv else lib().ckb_rhs)(m._h, _dev_ptr(states, torch.float64, "states"), _dev_ptr(pressure, torch.float64, "pressure"),
                        float(0.0 if p is None else p), N, ld, _dev_ptr(out, torch.float64, "out"),
                        int(VARIANTS.get(variant, variant)), int(repeat), _stream_ptr(stream))
     _check(rc, "ckb_rhs")
     return out
+
+
+def integrate_cv(m: Mech, states, dt, rtol, atol, method, **kw):
+    """ckb_integrate_cv: constant-volume closure (R29); p= / pressure= carry the density in g/cm^3."""
+    return integrate(m, states, dt, rtol, atol, method, cv=True, **kw)
+
+
+def integrate_host_cv(m: Mech, states, dt, rtol, atol, method, **kw):
+    """ckb_integrate_host_cv."""
+    return integrate_host(m, states, dt, rtol, atol, method, cv=True, **kw)
+
+
+def rhs_cv(m: Mech, states, **kw):
+    """ckb_rhs_cv."""
+    return rhs(m, states, cv=True, **kw)
 
 
 def fp64_probe(kind="dfma", iters=1 << 16, stream=None) -> float:

@@ -191,7 +191,7 @@ int ckb_mech_info(const ckb_mech *m, int32_t *n_species, int32_t *n_reactions, i
 static int integrate_impl(const ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
                           int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
                           int32_t variant, int32_t *status, int32_t *stats, cudaStream_t stream, int slot,
-                          int64_t n_choice) {
+                          int64_t n_choice, int cv) {
   if (!m || N < 0 || (method != CKB_METHOD_RKCK && method != CKB_METHOD_RKC)) return CKB_EINVAL;
   if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(t) || !(rtol > 0.0) || !(atol >= 0.0)) return CKB_EINVAL;
   if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
@@ -201,7 +201,7 @@ static int integrate_impl(const ckb_mech *m, double *states, const double *press
   if (N == 0) return CKB_OK;
   if (!states || ld < N) return CKB_EINVAL;
   ckb_host::IntegrateArgs a{states, pressure, p_uniform, (long long)N, (long long)ld, t, dt, rtol, atol,
-                            status, stats, stream, nullptr};
+                            status, stats, stream, nullptr, cv};
   /* queue order: hottest systems first (row 0 of states = T); pointless when every system starts at once */
   if (N >= 4096) {
     if (l.L <= 4 && method == CKB_METHOD_RKC && m->pk[0].rc == CKB_OK) {
@@ -211,7 +211,7 @@ static int integrate_impl(const ckb_mech *m, double *states, const double *press
       rc = ckb_host::queue_scratch(m, slot, N);
       if (rc) return rc;
       ckb_host::ProxyArgs pa{states, pressure, p_uniform, (long long)N, (long long)ld, 1e-3 * dt, rtol, atol,
-                             m->osc[slot].d_keys, stream};
+                             m->osc[slot].d_keys, stream, cv};
       rc = dispatch_proxy(m, l1, pa);
       if (rc) return rc;
       rc = ckb_host::make_queue_order(m, slot, 1, m->osc[slot].d_keys, N, a.stream, &a.order);
@@ -227,11 +227,18 @@ int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, dou
                   int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
                   int32_t *status, int32_t *stats, void *stream) {
   return integrate_impl(m, states, pressure, p_uniform, N, ld, t, dt, rtol, atol, method, variant, status, stats,
-                        (cudaStream_t)stream, 0, N);
+                        (cudaStream_t)stream, 0, N, 0);
 }
 
-int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, double p_uniform, int64_t N,
-            int64_t ld, double *dydt, int32_t variant, int32_t repeat, void *stream) {
+int ckb_integrate_cv(const ckb_mech *m, double *states, const double *density, double rho_uniform, int64_t N,
+                     int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
+                     int32_t *status, int32_t *stats, void *stream) {
+  return integrate_impl(m, states, density, rho_uniform, N, ld, t, dt, rtol, atol, method, variant, status, stats,
+                        (cudaStream_t)stream, 0, N, 1);
+}
+
+static int rhs_impl(const ckb_mech *m, const double *states, const double *pressure, double p_uniform, int64_t N,
+                    int64_t ld, double *dydt, int32_t variant, int32_t repeat, void *stream, int cv) {
   if (!m || N < 0 || repeat < 1) return CKB_EINVAL;
   if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
   Launch l;
@@ -239,16 +246,26 @@ int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, dou
   if (rc) return rc;
   if (N == 0) return CKB_OK;
   if (!states || !dydt || ld < N) return CKB_EINVAL;
-  ckb_host::RhsArgs a{states, pressure, p_uniform, (long long)N, (long long)ld, dydt, repeat, (cudaStream_t)stream};
+  ckb_host::RhsArgs a{states, pressure, p_uniform, (long long)N, (long long)ld, dydt, repeat, (cudaStream_t)stream, cv};
   return dispatch_rhs(m, l, a);
 }
 
-int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
-                       int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
-                       int32_t variant, int32_t *status, int32_t *stats, void *stream) {
+int ckb_rhs(const ckb_mech *m, const double *states, const double *pressure, double p_uniform, int64_t N,
+            int64_t ld, double *dydt, int32_t variant, int32_t repeat, void *stream) {
+  return rhs_impl(m, states, pressure, p_uniform, N, ld, dydt, variant, repeat, stream, 0);
+}
+
+int ckb_rhs_cv(const ckb_mech *m, const double *states, const double *density, double rho_uniform, int64_t N,
+               int64_t ld, double *dydt, int32_t variant, int32_t repeat, void *stream) {
+  return rhs_impl(m, states, density, rho_uniform, N, ld, dydt, variant, repeat, stream, 1);
+}
+
+static int integrate_host_impl(ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                               int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                               int32_t variant, int32_t *status, int32_t *stats, void *stream, int cv) {
   if (!m || N < 0) return CKB_EINVAL;
-  if (N == 0) return ckb_integrate(m, nullptr, nullptr, p_uniform, 0, 0, t, dt, rtol, atol, method, variant,
-                                   nullptr, nullptr, stream);
+  if (N == 0) return integrate_impl(m, nullptr, nullptr, p_uniform, 0, 0, t, dt, rtol, atol, method, variant,
+                                    nullptr, nullptr, (cudaStream_t)stream, 0, 0, cv);
   if (!states || ld < N) return CKB_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
   const int n = m->K + 1;
@@ -296,7 +313,7 @@ int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, doub
     if (pressure) CK(cudaMemcpyAsync(m->ws_pressure + c0, pressure + c0, (size_t)nc * 8, cudaMemcpyHostToDevice, cs));
     int rc = integrate_impl(m, m->ws_states + c0, pressure ? m->ws_pressure + c0 : nullptr, p_uniform, nc, N, t, dt,
                             rtol, atol, method, variant, status ? m->ws_status + c0 : nullptr,
-                            stats ? m->ws_stats + 4 * c0 : nullptr, cs, c, N);
+                            stats ? m->ws_stats + 4 * c0 : nullptr, cs, c, N, cv);
     if (rc) return rc;
     CK(cudaMemcpy2DAsync(states + c0, (size_t)ld * 8, m->ws_states + c0, (size_t)N * 8, (size_t)nc * 8, (size_t)n,
                          cudaMemcpyDeviceToHost, cs));
@@ -311,6 +328,20 @@ int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, doub
   }
   CK(cudaStreamSynchronize(s));
   return CKB_OK;
+}
+
+int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                       int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                       int32_t variant, int32_t *status, int32_t *stats, void *stream) {
+  return integrate_host_impl(m, states, pressure, p_uniform, N, ld, t, dt, rtol, atol, method, variant, status, stats,
+                             stream, 0);
+}
+
+int ckb_integrate_host_cv(ckb_mech *m, double *states, const double *density, double rho_uniform, int64_t N,
+                          int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
+                          int32_t variant, int32_t *status, int32_t *stats, void *stream) {
+  return integrate_host_impl(m, states, density, rho_uniform, N, ld, t, dt, rtol, atol, method, variant, status, stats,
+                             stream, 1);
 }
 
 const char *ckb_strerror(int code) {

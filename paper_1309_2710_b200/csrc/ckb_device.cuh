@@ -132,8 +132,11 @@ __device__ __forceinline__ double ckb_exp(double x, const ExpConst<PIN> &c) {
  * Sys<L, NV, TAB>: one ODE system on L lanes with NV register slots per lane; tables from the kernel
  * parameter bank (ParamTab) or global/L1 (GlobalTab).
  * ---------------------------------------------------------------------------------------------- */
-template <int L_, int NV_, class TAB, int M_ = 1>
+template <int L_, int NV_, class TAB, int M_ = 1, int CV_ = 0>
 struct Sys {
+  /* closure (compile time, so that the constant-pressure kernels carry none of it): false = constant pressure
+   * (Eq. 6), true = constant volume (R29: the "pressure" argument carries the density rho) */
+  static constexpr bool CV = CV_ != 0;
   /* M systems share the lanes of a group and are evaluated together: every table word is loaded and decoded
    * once for all of them, and their (independent) dependency chains interleave -- DESIGN.md 7.4. */
   static constexpr int L = L_, NV = NV_, G = 32 / L_, M = M_;
@@ -161,8 +164,13 @@ struct Sys {
   __device__ __forceinline__ unsigned long long tw(int i) const { return tab.ld(i); }
   __device__ __forceinline__ double td(int i) const { return __longlong_as_double((long long)tab.ld(i)); }
   __device__ __forceinline__ void set_pressure(int q, double p) {
-    pR[q] = p / CKB_RU;
-    Rp[q] = CKB_RU / p;
+    if (CV) { /* R29, constant volume: p carries the density rho (constant over the call) */
+      pR[q] = p;
+      Rp[q] = 1.0 / p;
+    } else {
+      pR[q] = p / CKB_RU;
+      Rp[q] = CKB_RU / p;
+    }
   }
 
   __device__ __forceinline__ void gsync() const {
@@ -227,6 +235,7 @@ struct Sys {
           h = fma(h, T[q], hc[k]);
         }
         h = fma(hc[5], invT[q], h);
+        if (CV) h -= 1.0; /* R29: u_k W_k/(Ru T) = h_k W_k/(Ru T) - 1 */
         const double v = Y(q, i) * iw; /* Y_k / W_k */
         if (L == 1) {
           sH[i * GI] = h;
@@ -246,13 +255,14 @@ struct Sys {
         s2[q] += __shfl_xor_sync(mask, s2[q], o);
       }
     }
-    /* R9a: ideal gas at constant pressure: rho = p / (Ru T sum_k Y_k/W_k), C_k = rho Y_k / W_k */
+    /* R9a: ideal gas at constant pressure: rho = p / (Ru T sum_k Y_k/W_k), C_k = rho Y_k / W_k;
+     * R29: constant volume: rho given, C_tot = rho sum_k Y_k/W_k */
     double ctot[M], invrho[M];
 #pragma unroll
     for (int q = 0; q < M; q++) {
-      ctot[q] = pR[q] * invT[q];
-      const double rho = ctot[q] * (1.0 / s1[q]);
-      invrho[q] = s1[q] * T[q] * Rp[q];
+      ctot[q] = CV ? pR[q] * s1[q] : pR[q] * invT[q];
+      const double rho = CV ? pR[q] : ctot[q] * (1.0 / s1[q]);
+      invrho[q] = CV ? Rp[q] : s1[q] * T[q] * Rp[q];
 #pragma unroll
       for (int i = 0; i < NV; i++) {
         const int c = g + L * i;
@@ -359,10 +369,11 @@ struct Sys {
 #pragma unroll
       for (int q = 0; q < M; q++) s3[q] += __shfl_xor_sync(mask, s3[q], o);
     }
-    /* Eq. 6: dT/dt = -(Ru T sum_k (h_k/RT) omega_k) / (rho cp), cp = Ru sum_k Y_k (cp_k/R) / W_k */
+    /* Eq. 6: dT/dt = -(Ru T sum_k (h_k/RT) omega_k) / (rho cp), cp = Ru sum_k Y_k (cp_k/R) / W_k;
+     * R29: dT/dt = -(Ru T sum_k (h_k/RT - 1) omega_k) / (rho c_v), c_v = cp - Ru sum_k Y_k / W_k */
     if (g == 0) {
 #pragma unroll
-      for (int q = 0; q < M; q++) f[q][0] = -(T[q] * s3[q] * invrho[q]) / s2[q];
+      for (int q = 0; q < M; q++) f[q][0] = -(T[q] * s3[q] * invrho[q]) / (CV ? s2[q] - s1[q] : s2[q]);
     }
   }
 };
@@ -969,14 +980,14 @@ struct IntegratorOf { typedef Rkck<S> type; };
 template <class S>
 struct IntegratorOf<S, 1> { typedef Rkc<S> type; };
 
-template <int L, int NV, class TAB, int METHOD, int M>
+template <int L, int NV, class TAB, int METHOD, int M, int CV = 0>
 __global__ void __launch_bounds__(CKB_BLOCK, METHOD == 0 ? CKB_MINB : CKB_MINB_RKC)
 integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, double *__restrict__ states,
                  const double *__restrict__ pressure, double p_uniform, long long N, long long ld, double t0,
                  double dt, double rtol, double atol, int *__restrict__ status, int *__restrict__ stats,
                  unsigned long long *__restrict__ counter, const int *__restrict__ order) {
   extern __shared__ double smem[];
-  typedef Sys<L, NV, TAB, M> S;
+  typedef Sys<L, NV, TAB, M, CV> S;
   S sys(m, tab);
   sys_setup(sys, m, smem, IntegratorOf<S, METHOD>::type::XDOUBLES + S::HDOUBLES);
   constexpr int G = S::G;
@@ -1084,13 +1095,13 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
   }
 }
 
-template <int L, int NV, class TAB>
+template <int L, int NV, class TAB, int CV = 0>
 __global__ void __launch_bounds__(CKB_BLOCK)
 rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, const double *__restrict__ states,
            const double *__restrict__ pressure, double p_uniform, long long N, long long ld,
            double *__restrict__ dydt, int repeat) {
   extern __shared__ double smem[];
-  typedef Sys<L, NV, TAB, 1> S;
+  typedef Sys<L, NV, TAB, 1, CV> S;
   S sys(m, tab);
   sys_setup(sys, m, smem, S::HDOUBLES);
   const long long ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * S::G + (threadIdx.x & 31) / L;
@@ -1122,13 +1133,13 @@ rhs_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, c
  *     key_i = || (f(y + h f(y)) - f(y)) / (h wt) ||_rms,   wt = atol + rtol |y|
  * (two evaluations of f, a fraction of a percent of the integration) orders the queue far better than T does
  * (rank correlation with the true cost 0.79 against 0.27 on configs[2]). */
-template <int L, int NV, class TAB>
+template <int L, int NV, class TAB, int CV = 0>
 __global__ void __launch_bounds__(CKB_BLOCK)
 cost_proxy_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab,
                   const double *__restrict__ states, const double *__restrict__ pressure, double p_uniform,
                   long long N, long long ld, double h, double rtol, double atol, double *__restrict__ key) {
   extern __shared__ double smem[];
-  typedef Sys<L, NV, TAB, 1> S;
+  typedef Sys<L, NV, TAB, 1, CV> S;
   S sys(m, tab);
   sys_setup(sys, m, smem, S::HDOUBLES);
   const long long ode = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * S::G + (threadIdx.x & 31) / L;

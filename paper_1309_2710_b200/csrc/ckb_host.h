@@ -67,7 +67,7 @@ namespace ckb_host {
 /* mechanism-specialised thread-per-ODE kernels (ckb_gen.cu): integrate RKCK, integrate RKC, rhs, cost proxy */
 struct GenKernels {
   cudaLibrary_t lib = nullptr;
-  cudaKernel_t k[4] = {};
+  cudaKernel_t k[8] = {}; /* [4..7]: the constant-volume instantiations */
   int NV = 0, resident[2] = {0, 0};
   size_t smem[2] = {0, 0};
   bool ok = false;
@@ -103,6 +103,7 @@ struct IntegrateArgs {
   double *states; const double *pressure; double p_uniform; long long N, ld;
   double t, dt, rtol, atol; int *status, *stats; cudaStream_t stream;
   const int *order; /* queue order (device) or NULL */
+  int cv = 0;       /* 1: constant volume (pressure / p_uniform carry the density) */
 };
 
 /* mode 0: keys are temperatures (hottest first); mode 1: keys are cost proxies (largest first, log-spaced bins) */
@@ -113,10 +114,12 @@ int queue_scratch(const ckb_mech *m, int slot, long long N);
 struct ProxyArgs {
   const double *states; const double *pressure; double p_uniform; long long N, ld; double h, rtol, atol;
   double *key; cudaStream_t stream;
+  int cv = 0;
 };
 struct RhsArgs {
   const double *states; const double *pressure; double p_uniform; long long N, ld; double *dydt; int repeat;
   cudaStream_t stream;
+  int cv = 0;
 };
 
 /* the instantiation list: (lanes per system L, register slots per lane NV); a system needs K+1 <= L*NV */

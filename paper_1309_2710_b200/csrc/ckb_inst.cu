@@ -31,6 +31,7 @@ typedef ckb::GlobalTab Tab;
 
 static const Packed &pack_of(const ckb_mech *m) { return m->pk[pack_index(L)]; }
 
+
 static size_t smem_bytes(const ckb_mech *m, int M, int xdoubles) {
   const ckb::DevMech &dm = pack_of(m).dm;
   return (size_t)(ckb::region_doubles(dm) + xdoubles) * (32 / L) * M * (CKB_BLOCK / 32) * sizeof(double);
@@ -51,9 +52,9 @@ static long long n_blocks(long long N, int M) {
   return (N + per_block - 1) / per_block;
 }
 
-template <int METHOD>
+template <int METHOD, int CV>
 static int launch(const ckb_mech *m, const IntegrateArgs &a) {
-  auto kern = ckb::integrate_kernel<L, NV, Tab, METHOD, CKB_M>;
+  auto kern = ckb::integrate_kernel<L, NV, Tab, METHOD, CKB_M, CV>;
   const size_t smem = smem_bytes(m, CKB_M, ckb::IntegratorOf<ckb::Sys<L, NV, Tab, CKB_M>, METHOD>::type::XDOUBLES + ckb::Sys<L, NV, Tab, CKB_M>::HDOUBLES);
   int rc = prep(kern, smem);
   if (rc) return rc;
@@ -83,11 +84,12 @@ static int launch(const ckb_mech *m, const IntegrateArgs &a) {
 }  // namespace
 
 int CKB_CAT(integrate_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, int method, const IntegrateArgs &a) {
-  return method == 0 ? launch<0>(m, a) : launch<1>(m, a);
+  if (a.cv) return method == 0 ? launch<0, 1>(m, a) : launch<1, 1>(m, a);
+  return method == 0 ? launch<0, 0>(m, a) : launch<1, 0>(m, a);
 }
 
 int CKB_CAT(rhs_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const RhsArgs &a) {
-  auto kern = ckb::rhs_kernel<L, NV, Tab>;
+  auto kern = a.cv ? ckb::rhs_kernel<L, NV, Tab, 1> : ckb::rhs_kernel<L, NV, Tab, 0>;
   const size_t smem = smem_bytes(m, 1, ckb::Sys<L, NV, Tab, 1>::HDOUBLES);
   int rc = prep(kern, smem);
   if (rc) return rc;
@@ -103,7 +105,7 @@ int CKB_CAT(rhs_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const RhsArgs &a) {
 
 int CKB_CAT(proxy_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const ProxyArgs &a) {
 #if CKB_L == 1
-  auto kern = ckb::cost_proxy_kernel<L, NV, Tab>;
+  auto kern = a.cv ? ckb::cost_proxy_kernel<L, NV, Tab, 1> : ckb::cost_proxy_kernel<L, NV, Tab, 0>;
   const size_t smem = smem_bytes(m, 1, ckb::Sys<L, NV, Tab, 1>::HDOUBLES);
   int rc = prep(kern, smem);
   if (rc) return rc;

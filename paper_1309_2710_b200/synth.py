@@ -355,6 +355,14 @@ def make_states(cfg: int, N: int, seed: int = 0, stream: int = 1, ordering: str 
     return np.ascontiguousarray(states), P_ATM
 
 
+def make_densities(mech: "Mechanism", states: np.ndarray, p: float = P_ATM) -> np.ndarray:
+    """Densities (g/cm^3) for the constant-volume inputs: the density each system of `states` has at pressure p
+    (ideal gas, rho = p / (Ru T sum_k Y_k/W_k)) -- i.e. the same 1 atm initial conditions as the constant-pressure
+    workload, then held at their own volume.  Input recipe only; no method arithmetic."""
+    w = np.asarray(mech.mol_weight, dtype=np.float64)
+    return p / (_RU * states[0] * (states[1:] / w[:, None]).sum(axis=0))
+
+
 def toy_mechanism(K, reactions, W=None, nasa=None, third_body=None, name="toy") -> Mechanism:
     """Hand-built mechanism for closed-form tests.
 
