@@ -64,6 +64,18 @@ def min_blocks(L: int, NV: int, method: str = "rkck") -> int:
     return 2
 
 
+def tmem_tables(L: int, NV: int) -> int:
+    """1 = the object also carries warp-per-ODE integrate kernels that read the reaction-slot table from tensor memory
+    (tcgen05.ld) instead of global memory / L1: one block of 512 threads per SM then owns the SM's
+    512 TMEM columns, so only where 128 registers per thread are enough (NV = 2, the 53-species class)."""
+    return int(os.environ.get("CKB_TMEM", "1")) if (L == 32 and NV == 2) else 0
+
+
+def block_threads(L: int, NV: int) -> int:
+    """Threads per block of the table-driven kernels (CKB_BLOCK)."""
+    return int(os.environ.get("CKB_BLOCK_L32", "128")) if L == 32 else 128
+
+
 def _digest(extra: str) -> str:
     h = hashlib.sha256(extra.encode())
     h.update(open(os.path.abspath(__file__), "rb").read())  # the per-instantiation knobs live in this file
@@ -109,7 +121,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     os.makedirs(OBJ, exist_ok=True)
     flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("CKB_DEFS", "").split()  # tuning knobs
     stamp = os.path.join(OBJ, "stamp")
-    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", "") + os.environ.get("CKB_MINB_L24", "") + os.environ.get("CKB_US_L1", "") + os.environ.get("CKB_EXP_TABLE_MAXL", ""))
+    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", "") + os.environ.get("CKB_MINB_L24", "") + os.environ.get("CKB_US_L1", "") + os.environ.get("CKB_EXP_TABLE_MAXL", "") + os.environ.get("CKB_BLOCK_L32", "") + os.environ.get("CKB_TMEM", ""))
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     _embed_sources()
@@ -119,7 +131,10 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
         jobs.append((obj, [NVCC, *flags, "-c", os.path.join(CSRC, src), "-o", obj]))
     for (L, NV) in instantiations():
         obj = os.path.join(OBJ, f"ckb_inst_L{L}_NV{NV}.o")
-        jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_MINB={min_blocks(L, NV)}", f"-DCKB_MINB_RKC={min_blocks(L, NV, 'rkc')}",
+        bt = block_threads(L, NV)
+        jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_BLOCK={bt}",
+                           f"-DCKB_MINB={max(1, min_blocks(L, NV) * 128 // bt)}", f"-DCKB_MINB_RKC={max(1, min_blocks(L, NV, 'rkc') * 128 // bt)}",
+                           f"-DCKB_TMEM={tmem_tables(L, NV)}",
                            f"-DCKB_UNROLL_SLOTS={int(os.environ.get('CKB_US_L1', '1')) if L == 1 else int(os.environ.get('CKB_US', '1'))}",
                            f"-DCKB_EXP_TABLE={exp_table(L)}",
                            f"-DCKB_M={systems_per_group(L, NV)}", "-c",

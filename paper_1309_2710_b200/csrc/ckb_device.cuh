@@ -128,6 +128,79 @@ __device__ __forceinline__ double ckb_exp(double x, const ExpConst<PIN> &c) {
 }
 #endif
 
+/* N exponentials advanced in lock step (same arithmetic per chain as ckb_exp, non-table form): the N dependency
+ * chains are emitted interleaved, step by step, so that a warp has N DFMAs in flight instead of one (the compiler
+ * keeps the emission order; left to itself it runs the chains one after the other). */
+template <int N, bool PIN>
+__device__ __forceinline__ void ckb_exp_n(const double (&x)[N], double (&out)[N], const ExpConst<PIN> &c) {
+  double t[N], r[N], p[N];
+#pragma unroll
+  for (int u = 0; u < N; u++) t[u] = fma(x[u], c.log2e, 6755399441055744.0);
+#pragma unroll
+  for (int u = 0; u < N; u++) r[u] = fma(t[u] - 6755399441055744.0, c.ln2hi, x[u]);
+#pragma unroll
+  for (int u = 0; u < N; u++) r[u] = fma(t[u] - 6755399441055744.0, c.ln2lo, r[u]);
+#pragma unroll
+  for (int u = 0; u < N; u++) p[u] = c.q[9];
+#pragma unroll
+  for (int i = 8; i >= 0; i--) {
+#pragma unroll
+    for (int u = 0; u < N; u++) p[u] = fma(p[u], r[u], c.q[i]);
+  }
+#pragma unroll
+  for (int u = 0; u < N; u++) p[u] = fma(p[u], r[u], 1.0);
+#pragma unroll
+  for (int u = 0; u < N; u++) p[u] = fma(p[u], r[u], 1.0);
+#pragma unroll
+  for (int u = 0; u < N; u++) {
+    int k = __double2loint(t[u]);
+    k = max(-1022, min(1023, k));
+    out[u] = __hiloint2double(__double2hiint(p[u]) + (k << 20), __double2loint(p[u]));
+  }
+}
+
+#ifndef CKB_TMEM
+#define CKB_TMEM 0 /* warp-per-ODE integrate kernels: 1 = the reaction-slot table is read from tensor memory */
+#endif
+#if CKB_TMEM
+/* Tensor memory as a table store.  The warp-per-ODE kernels are bound by the L1/shared data pipe
+ * (ncu: LSU wavefronts at 82 % of peak), and half of those wavefronts are the coalesced loads of the slot table --
+ * the same 8 words per lane every evaluation of f(y).  TMEM (512 columns x 128 lanes x 32 bit per SM) is read with
+ * tcgen05.ld over its own datapath: lane g of warp w owns TMEM lane 32 (w mod 4) + g, and the 8 table words of slot
+ * round r sit in 16 consecutive columns -- ONE tcgen05.ld.32x32b.x16 per slot instead of 8 LDG.64. */
+#define CKB_TMEM_COLS 512
+__device__ __forceinline__ void tm_alloc(unsigned *holder_smem) {
+  const unsigned dst = (unsigned)__cvta_generic_to_shared(holder_smem);
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst), "r"(CKB_TMEM_COLS) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tm_dealloc(unsigned base) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(CKB_TMEM_COLS) : "memory");
+}
+__device__ __forceinline__ void tm_fence_sync_fence() {
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+}
+__device__ __forceinline__ void tm_st16(unsigned addr, const unsigned (&v)[16]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+               ::"r"(addr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
+               "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_ld16(unsigned addr, unsigned (&v)[16]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+                 "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+               : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+#ifndef CKB_TMEM_SLOTS
+#define CKB_TMEM_SLOTS 1 /* reaction slots in flight per lane in the TMEM slot loop (2 slots = 4 exp chains in lock step:
+                            measured slower, the registers they take cost more than the overlap gives) */
+#endif
+#endif
+
 /* ------------------------------------------------------------------------------------------------
  * Sys<L, NV, TAB>: one ODE system on L lanes with NV register slots per lane; tables from the kernel
  * parameter bank (ParamTab) or global/L1 (GlobalTab).
@@ -159,6 +232,10 @@ struct Sys {
   int g;           /* lane within the group */
   int src0;        /* warp lane that holds component 0 (T) */
   double pR[M], Rp[M]; /* p / Ru and Ru / p (R24: pressure constant over the call) */
+#if CKB_TMEM
+  bool tm_on = false;  /* slot table resident in tensor memory (set by integrate_kernel) */
+  unsigned tm_addr = 0;/* TMEM address of this warp's lane quarter, column of slot round 0 */
+#endif
 
   __device__ __forceinline__ Sys(const DevMech &m_, const TAB &tab_) : m(m_), tab(tab_) {}
   __device__ __forceinline__ unsigned long long tw(int i) const { return tab.ld(i); }
@@ -293,6 +370,45 @@ struct Sys {
     gsync();
     /* Eq. 4-5: q_s = [M] (k_f prod C_reactants - k_r prod C_products); absent molecules point at C_0 = 1, an
      * absent third body at a 1.0.  The 16-bit fields are BYTE offsets into the system's region. */
+#if CKB_TMEM
+    if (L == 32 && M == 1 && tm_on) { /* warp-uniform: slot table in tensor memory, U slots per lane in flight */
+      constexpr int U = CKB_TMEM_SLOTS;
+      const ExpConst<true> ec;
+      double *qp = sR + qoff + g;
+      const char *c = reinterpret_cast<const char *>(sR);
+      const int last = m.NSR - 1;
+      for (int r = 0; r < m.NSR; r += U, qp += U * L) {
+        unsigned v[U][16];
+#pragma unroll
+        for (int u = 0; u < U; u++) tm_ld16(tm_addr + (unsigned)(r + u < last ? r + u : last) * 16u, v[u]);
+        tm_wait_ld();
+        double xf[U], xr[U], pf[U], pr[U], mt[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#define CKB_TD(x) __hiloint2double((int)v[u][2 * (x) + 1], (int)v[u][2 * (x)])
+          xf[u] = fma(-CKB_TD(CKB_SL_THF), invT[0], fma(CKB_TD(CKB_SL_BF), lnT[0], CKB_TD(CKB_SL_LNAF)));
+          xr[u] = fma(-CKB_TD(CKB_SL_THR), invT[0], fma(CKB_TD(CKB_SL_BR), lnT[0], CKB_TD(CKB_SL_LNAR)));
+#undef CKB_TD
+          const unsigned alo = v[u][2 * CKB_SL_IDXA], ahi = v[u][2 * CKB_SL_IDXA + 1];
+          const unsigned blo = v[u][2 * CKB_SL_IDXB], bhi = v[u][2 * CKB_SL_IDXB + 1];
+#define CKB_AT(off) (*reinterpret_cast<const double *>(c + (off)))
+          pf[u] = CKB_AT(alo & 0xFFFFu) * CKB_AT(alo >> 16) * CKB_AT(ahi & 0xFFFFu);
+          pr[u] = CKB_AT(blo & 0xFFFFu) * CKB_AT(blo >> 16) * CKB_AT(bhi & 0xFFFFu);
+          mt[u] = CKB_AT(ahi >> 16);
+#undef CKB_AT
+        }
+        double xs[2 * U], ks[2 * U], res[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) { xs[2 * u] = xf[u]; xs[2 * u + 1] = xr[u]; }
+        ckb_exp_n<2 * U>(xs, ks, ec);
+#pragma unroll
+        for (int u = 0; u < U; u++) res[u] = (ks[2 * u] * pf[u] - ks[2 * u + 1] * pr[u]) * mt[u];
+#pragma unroll
+        for (int u = 0; u < U; u++)
+          if (u == 0 || r + u <= last) qp[u * L] = res[u];
+      }
+    } else
+#endif
     {
       constexpr int US = CKB_UNROLL_SLOTS;
       const ExpConst<(L > 1)> ec;
@@ -300,9 +416,13 @@ struct Sys {
       double *qp = sR + qoff + g * GI;
 #pragma unroll US
       for (int r = 0; r < m.NSR; r++, b += CKB_SL_WORDS * L, qp += L * GI) {
-        const double lnAf = td(b + CKB_SL_LNAF * L), bf = td(b + CKB_SL_BF * L), thf = td(b + CKB_SL_THF * L);
-        const double lnAr = td(b + CKB_SL_LNAR * L), br = td(b + CKB_SL_BR * L), thr = td(b + CKB_SL_THR * L);
-        const unsigned long long wa = tw(b + CKB_SL_IDXA * L), wb = tw(b + CKB_SL_IDXB * L);
+        double lnAf, bf, thf, lnAr, br, thr;
+        unsigned long long wa, wb;
+        {
+          lnAf = td(b + CKB_SL_LNAF * L), bf = td(b + CKB_SL_BF * L), thf = td(b + CKB_SL_THF * L);
+          lnAr = td(b + CKB_SL_LNAR * L), br = td(b + CKB_SL_BR * L), thr = td(b + CKB_SL_THR * L);
+          wa = tw(b + CKB_SL_IDXA * L), wb = tw(b + CKB_SL_IDXB * L);
+        }
         const unsigned alo = (unsigned)wa, ahi = (unsigned)(wa >> 32), blo = (unsigned)wb, bhi = (unsigned)(wb >> 32);
         const unsigned a0 = alo & 0xFFFFu, a1 = alo >> 16, a2 = ahi & 0xFFFFu, tb = ahi >> 16;
         const unsigned b0 = blo & 0xFFFFu, b1 = blo >> 16, b2 = bhi & 0xFFFFu;
@@ -943,7 +1063,9 @@ struct Rkc {
 template <class S>
 __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem, int xdoubles) {
   constexpr int L = S::L, G = S::G, M = S::M;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  /* a one-warp block (CKB_BLOCK == 32) has its shared region at a compile-time address: every runtime-indexed
+   * shared read is then [offset + immediate], without the add of a per-warp base */
+  const int lane = threadIdx.x & 31, warp = (CKB_BLOCK == 32) ? 0 : (threadIdx.x >> 5);
   const int grp = lane / L;
   sys.g = lane % L;
   sys.src0 = grp * L;
@@ -980,8 +1102,13 @@ struct IntegratorOf { typedef Rkck<S> type; };
 template <class S>
 struct IntegratorOf<S, 1> { typedef Rkc<S> type; };
 
-template <int L, int NV, class TAB, int METHOD, int M, int CV = 0>
-__global__ void __launch_bounds__(CKB_BLOCK, METHOD == 0 ? CKB_MINB : CKB_MINB_RKC)
+#ifndef CKB_TMEM_BLOCK
+#define CKB_TMEM_BLOCK 512 /* TM = 1: one block per SM owns the SM's tensor memory; 512 threads x 128 registers */
+#endif
+
+/* TM = 1 (only where the object is compiled with CKB_TMEM): the slot table is read from tensor memory. */
+template <int L, int NV, class TAB, int METHOD, int M, int CV = 0, int TM = 0>
+__global__ void __launch_bounds__(TM ? CKB_TMEM_BLOCK : CKB_BLOCK, TM ? 1 : (METHOD == 0 ? CKB_MINB : CKB_MINB_RKC))
 integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB tab, double *__restrict__ states,
                  const double *__restrict__ pressure, double p_uniform, long long N, long long ld, double t0,
                  double dt, double rtol, double atol, int *__restrict__ status, int *__restrict__ stats,
@@ -991,9 +1118,38 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
   S sys(m, tab);
   sys_setup(sys, m, smem, IntegratorOf<S, METHOD>::type::XDOUBLES + S::HDOUBLES);
   constexpr int G = S::G;
+  constexpr int BLOCK = TM ? CKB_TMEM_BLOCK : CKB_BLOCK;
+#if CKB_TMEM
+  /* slot table -> tensor memory: warp 0 allocates the SM's 512 columns (one block per SM: the launch bounds fill the
+   * register file), warps 0..3 copy the table into their lane quarter, every warp then reads its own quarter */
+  __shared__ unsigned tm_holder;
+  unsigned tm_base = 0;
+  sys.tm_on = (TM != 0) && (L == 32) && m.NSR * 16 <= CKB_TMEM_COLS;
+  if (sys.tm_on) {
+    const int warp = threadIdx.x >> 5;
+    if (warp == 0) tm_alloc(&tm_holder);
+    tm_fence_sync_fence();
+    tm_base = *reinterpret_cast<volatile unsigned *>(&tm_holder);
+    sys.tm_addr = tm_base + ((unsigned)((warp & 3) * 32) << 16);
+    if (warp < 4) {
+      for (int r = 0; r < m.NSR; r++) {
+        unsigned v[16];
+#pragma unroll
+        for (int x = 0; x < CKB_SL_WORDS; x++) {
+          const unsigned long long w = sys.tw(m.o_sl + (r * CKB_SL_WORDS + x) * L + sys.g);
+          v[2 * x] = (unsigned)w;
+          v[2 * x + 1] = (unsigned)(w >> 32);
+        }
+        tm_st16(sys.tm_addr + (unsigned)r * 16u, v);
+      }
+      tm_wait_st();
+    }
+    tm_fence_sync_fence();
+  }
+#endif
   /* queue positions: every group starts with M of its own, then pulls from the counter */
-  const long long n_static = (long long)gridDim.x * (CKB_BLOCK / 32) * G * M;
-  const long long grp_id = ((long long)blockIdx.x * (CKB_BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L;
+  const long long n_static = (long long)gridDim.x * (BLOCK / 32) * G * M;
+  const long long grp_id = ((long long)blockIdx.x * (BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L;
   typename IntegratorOf<S, METHOD>::type integ[M];
   long long qi[M], ode[M];
   bool need_load[M], active[M];
@@ -1093,6 +1249,12 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
       }
     }
   }
+#if CKB_TMEM
+  if (sys.tm_on) {
+    tm_fence_sync_fence(); /* every warp has left the loop */
+    if ((threadIdx.x >> 5) == 0) tm_dealloc(tm_base);
+  }
+#endif
 }
 
 template <int L, int NV, class TAB, int CV = 0>

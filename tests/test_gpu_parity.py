@@ -452,3 +452,40 @@ def _run_gpu_raw(mech, states, p, dt, method, variant):
     torch.cuda.synchronize()
     m.close()
     return buf.cpu().numpy(), status.cpu().numpy(), stats.cpu().numpy()
+
+
+@pytest.mark.parametrize("method,cv", [("rkc", False), ("rkck", False), ("rkc", True)])
+def test_tensor_memory_slot_table_bitwise(method, cv):
+    """Warp-per-ODE batches of >= 2368 systems on the 53-species class read the reaction-slot table from tensor
+    memory (tcgen05.ld); smaller batches read it from global memory.  Same arithmetic per system, so
+    one batch of 2600 (TMEM kernel) must equal the same systems integrated as two batches of 1300 (plain kernel) bit
+    for bit -- and both are compared with the oracle on a sample."""
+    import torch
+    from paper_1309_2710_b200 import binding
+    mech = synth.make_mechanism(3)
+    N = 2600
+    states, p = synth.make_states(3, N)
+    arg = synth.make_densities(mech, states, p) if cv else None
+    m = binding.mech_load(mech)
+
+    def run(cols):
+        buf = torch.from_numpy(np.ascontiguousarray(states[:, cols])).cuda()
+        st = torch.full((len(cols),), -7, dtype=torch.int32, device="cuda")
+        sts = torch.full((4, len(cols)), -7, dtype=torch.int32, device="cuda")
+        pr = None if arg is None else torch.from_numpy(np.ascontiguousarray(arg[cols])).cuda()
+        binding.integrate(m, buf, 1e-6, RTOL, ATOL, method, p=0.0 if cv else p, pressure=pr, variant="warp",
+                          status=st, stats=sts, cv=cv)
+        torch.cuda.synchronize()
+        return buf.cpu().numpy(), st.cpu().numpy(), sts.cpu().numpy()
+
+    whole = run(np.arange(N))
+    a, b = run(np.arange(N // 2)), run(np.arange(N // 2, N))
+    m.close()
+    assert np.array_equal(whole[0], np.concatenate([a[0], b[0]], axis=1))
+    assert np.array_equal(whole[1], np.concatenate([a[1], b[1]]))
+    assert np.array_equal(whole[2], np.concatenate([a[2], b[2]], axis=1))
+    idx = np.random.default_rng(11).choice(N, 48, replace=False)
+    import oracle
+    ora = oracle.OracleMech(mech).integrate(states[:, idx].copy(), 0.0 if cv else p, 1e-6, RTOL, ATOL, method,
+                                            pressure=None if arg is None else arg[idx].copy(), cv=cv)
+    _compare((whole[0][:, idx], whole[1][idx], whole[2][:, idx]), ora)
