@@ -67,8 +67,14 @@ def min_blocks(L: int, NV: int, method: str = "rkck") -> int:
 def tmem_tables(L: int, NV: int) -> int:
     """1 = the object also carries warp-per-ODE integrate kernels that read the reaction-slot table from tensor memory
     (tcgen05.ld) instead of global memory / L1: one block of 512 threads per SM then owns the SM's
-    512 TMEM columns, so only where 128 registers per thread are enough (NV = 2, the 53-species class)."""
-    return int(os.environ.get("CKB_TMEM", "1")) if (L == 32 and NV == 2) else 0
+    512 TMEM columns, sized by tmem_block()."""
+    return int(os.environ.get("CKB_TMEM", "1")) if (L == 32 and NV in (2, 4)) else 0
+
+
+def tmem_block(L: int, NV: int) -> int:
+    """Threads of the one block per SM of the TMEM kernels: what the registers allow (128 per thread for NV = 2, 168
+    for NV = 4, the 111-species class)."""
+    return 512 if NV <= 2 else 384
 
 
 def block_threads(L: int, NV: int) -> int:
@@ -134,7 +140,8 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
         bt = block_threads(L, NV)
         jobs.append((obj, [NVCC, *flags, f"-DCKB_L={L}", f"-DCKB_NV={NV}", f"-DCKB_BLOCK={bt}",
                            f"-DCKB_MINB={max(1, min_blocks(L, NV) * 128 // bt)}", f"-DCKB_MINB_RKC={max(1, min_blocks(L, NV, 'rkc') * 128 // bt)}",
-                           f"-DCKB_TMEM={tmem_tables(L, NV)}",
+                           f"-DCKB_TMEM={tmem_tables(L, NV)}", f"-DCKB_TMEM_BLOCK={tmem_block(L, NV)}",
+                           f"-DCKB_TMEM_MIN_N={148 * tmem_block(L, NV) // 32}",
                            f"-DCKB_UNROLL_SLOTS={int(os.environ.get('CKB_US_L1', '1')) if L == 1 else int(os.environ.get('CKB_US', '1'))}",
                            f"-DCKB_EXP_TABLE={exp_table(L)}",
                            f"-DCKB_M={systems_per_group(L, NV)}", "-c",
