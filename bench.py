@@ -123,7 +123,7 @@ class GpuCase:
 
     specialize = True   # class-wide switch (--no-specialize)
 
-    def __init__(self, cfg, N, dt, variant="auto", ordering="shuffled", device=0):
+    def __init__(self, cfg, N, dt, variant="auto", ordering="shuffled", device=0, cv=False):
         import torch
         from paper_1309_2710_b200 import binding
         self.torch, self.binding = torch, binding
@@ -141,6 +141,9 @@ class GpuCase:
             except binding.CkbError as e:
                 self.specialize_error = str(e)[:200]
         st, self.p = synth.make_states(cfg, N, ordering=ordering)
+        # constant-volume closure: the same states, each held at the density it has at 1 atm
+        self.cv = cv
+        self.density = torch.from_numpy(synth.make_densities(self.mech, st, self.p)).cuda() if cv else None
         self.host0 = st
         self.states0 = torch.from_numpy(st).cuda()
         self.states = torch.empty_like(self.states0)
@@ -149,7 +152,8 @@ class GpuCase:
         self.flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
     def step(self, want_stats=False):
-        self.binding.integrate(self.m, self.states, self.dt, RTOL, ATOL, self.spec.method, p=self.p,
+        self.binding.integrate(self.m, self.states, self.dt, RTOL, ATOL, self.spec.method,
+                               p=0.0 if self.cv else self.p, pressure=self.density, cv=self.cv,
                                variant=self.variant, status=self.status if want_stats else None,
                                stats=self.stats if want_stats else None)
 
@@ -226,7 +230,7 @@ def roofline(case, ms, work, peak_tflops, peak_src):
     flops = case.m.flops_per_rhs * work["rhs_calls"]
     ach = flops / (ms * 1e-3) / 1e12
     return {"bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s", "frac": ach / peak_tflops,
-            "traffic": measured_traffic(case.cfg, case.N, case.specialized), "peak_source": peak_src, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
+            "traffic": None if getattr(case, "cv", False) else measured_traffic(case.cfg, case.N, case.specialized), "peak_source": peak_src, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
             "flops_per_rhs": case.m.flops_per_rhs, "rhs_calls_per_launch": work["rhs_calls"],
             "kernel_ms": ms, "hbm_algorithmic_GBps": 2 * 8 * (case.mech.n_species + 1) * case.N / (ms * 1e-3) / 1e9}
 
@@ -364,6 +368,20 @@ def run_ours(args):
                     del cs
                 except Exception as ex:  # pragma: no cover
                     extra[f"cfg{c}_{var}"] = {"error": str(ex)}
+        # constant-volume closure (ckb_integrate_cv) on the headline workload and on configs[3]
+        for c in (1, 3):
+            try:
+                s2, N2, dt2 = workload(c)
+                cs = GpuCase(c, N2, dt2, "auto", cv=True)
+                wk = cs.work()
+                m2 = cs.timed_steps(3, 3)
+                extra[f"cv_cfg{c}_{s2.method}_auto_N{N2}"] = {
+                    "odes_per_s": N2 / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)), "work": wk,
+                    "roofline": roofline(cs, float(np.mean(m2)), wk, peak_flops / 1e12, "measured DFMA probe")}
+                cs.close()
+                del cs
+            except Exception as ex:  # pragma: no cover
+                extra[f"cv_cfg{c}"] = {"error": str(ex)}
         # the paper's "similar neighbours" experiment: the same systems sorted by T
         try:
             cs = GpuCase(args.config, N, dt, args.variant, "similar")
