@@ -167,3 +167,44 @@ def test_cv_argument_checks():
     with pytest.raises(binding.CkbError):
         binding.rhs_cv(m, st, p=-1.0)
     m.close()
+
+
+@pytest.mark.parametrize("cfg,N,n_sample,specialize", [(2, 40000, 400, False), (2, 120000, 400, True), (1, 1 << 19, 2000, True),
+                                                       (3, 4096, 64, False)])
+def test_cv_at_size_sampled(cfg, N, n_sample, specialize):
+    """Constant volume in the launch configurations a user gets at size (AUTO: 4 lanes per system with the cost-proxy
+    queue order of the cv kernels at mid sizes, the specialised thread-per-ODE kernels at full size, the tensor-memory
+    warp-per-ODE kernel on the 53-species class): sampled systems against the oracle one by one."""
+    import torch
+    from paper_1309_2710_b200 import binding
+    spec = synth.CONFIGS[cfg]
+    mech = synth.make_mechanism(cfg)
+    states, p = synth.make_states(cfg, N)
+    rho = synth.make_densities(mech, states, p)
+    m = binding.mech_load(mech, specialize=specialize)
+    dev = torch.from_numpy(states).cuda()
+    stats = torch.zeros((4, N), dtype=torch.int32, device="cuda")
+    status = torch.full((N,), -1, dtype=torch.int32, device="cuda")
+    binding.integrate_cv(m, dev, 1e-6, RTOL, ATOL, spec.method, pressure=torch.from_numpy(rho).cuda(), status=status,
+                         stats=stats)
+    torch.cuda.synchronize()
+    y, st, stt = dev.cpu().numpy(), status.cpu().numpy(), stats.cpu().numpy()
+    m.close()
+    assert np.isin(st, (0, 4)).all() and np.isfinite(y).all() and (stt[0] > 0).all()
+    pick = np.random.default_rng(23 + cfg).choice(N, size=n_sample, replace=False)
+    ora = _oracle_cv(mech, np.ascontiguousarray(states[:, pick]), 0.0, 1e-6, spec.method, density=rho[pick].copy())
+    rep = _compare((y[:, pick], st[pick], stt[:, pick]), ora, max_flip_frac=5e-3)
+    print(f"cv at size cfg{cfg} N={N}: {rep}")
+
+
+@pytest.mark.parametrize("cfg,N,dt,rtol,atol", [(1, 2048, 1e-8, 1e-10, 1e-40), (2, 1024, 1e-6, 1e-6, 1e-10),
+                                               (3, 128, 1e-6, 1e-6, 1e-10)])
+def test_parity_cv_paper_settings(cfg, N, dt, rtol, atol):
+    """The paper's own tolerances and global steps at constant volume."""
+    spec = synth.CONFIGS[cfg]
+    mech = synth.make_mechanism(cfg)
+    states, p = synth.make_states(cfg, N)
+    rho = synth.make_densities(mech, states, p)
+    ora = _oracle_cv(mech, states, 0.0, dt, spec.method, density=rho, rtol=rtol, atol=atol)
+    gpu = _run_gpu_cv(mech, states, 0.0, dt, spec.method, density=rho, rtol=rtol, atol=atol)
+    _compare(gpu, ora, max_flip_frac=5e-3)

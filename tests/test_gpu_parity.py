@@ -279,6 +279,30 @@ def test_full_size_sampled(cfg, n_sample):
     print(f"full size cfg{cfg} N={N}: {rep}")
 
 
+def test_cfg4_larger_global_step_tensor_memory_kernel():
+    """configs[4]'s second global step (1e-5 s) at its smallest batch size (N = 8192): the 384-thread tensor-memory
+    kernel of the 111-species class (batches >= 1776), sampled against the oracle."""
+    import torch
+    from paper_1309_2710_b200 import binding
+    mech = synth.make_mechanism(4)
+    N = 8192
+    states, p = synth.make_states(4, N)
+    m = binding.mech_load(mech)
+    dev = torch.from_numpy(states).cuda()
+    stats = torch.zeros((4, N), dtype=torch.int32, device="cuda")
+    status = torch.full((N,), -1, dtype=torch.int32, device="cuda")
+    binding.integrate(m, dev, 1e-5, RTOL, ATOL, "rkc", p=p, status=status, stats=stats)
+    torch.cuda.synchronize()
+    y, st, stt = dev.cpu().numpy(), status.cpu().numpy(), stats.cpu().numpy()
+    m.close()
+    assert np.isin(st, (0, 4)).all() and np.isfinite(y).all()
+    assert np.abs(y[1:].sum(0) - 1.0).max() < 1e-11
+    pick = np.random.default_rng(41).choice(N, size=24, replace=False)
+    ora = _oracle(mech, np.ascontiguousarray(states[:, pick]), p, 1e-5, "rkc")
+    rep = _compare((y[:, pick], st[pick], stt[:, pick]), ora, max_flip_frac=0.05)
+    print(f"cfg4 dt=1e-5 N={N}: {rep}")
+
+
 @pytest.mark.parametrize("cfg,N,n_sample", [(1, 50000, 1500), (2, 40000, 600)])
 def test_mid_size_auto_sampled(cfg, N, n_sample):
     """Batch sizes at which AUTO maps small mechanisms onto 4 lanes per system (and orders the RKC queue by the
