@@ -60,6 +60,8 @@ def lib():
         L.ora_integrate.argtypes = [C.c_void_p, dp, dp, C.c_double, C.c_int64, C.c_int64, C.c_double,
                                     C.c_double, C.c_double, C.c_double, C.c_int32, ip, ip, C.c_int32]
         L.ora_integrate.restype = C.c_int
+        L.ora_mech_set_thermo2.argtypes = [C.c_void_p, dp, dp]
+        L.ora_mech_set_thermo2.restype = C.c_int
         L.ora_rhs_cv.argtypes = L.ora_rhs.argtypes
         L.ora_rhs_cv.restype = None
         L.ora_integrate_cv.argtypes = L.ora_integrate.argtypes
@@ -132,6 +134,12 @@ class OracleMech:
         if rc != 0:
             raise ValueError(f"ora_mech_load failed: {rc}")
         self._h = h
+        # optional second temperature range of the NASA fits (reading R30)
+        if getattr(mech, "nasa_high", None) is not None:
+            hi, tm = _f64(mech.nasa_high), _f64(mech.T_mid)
+            assert hi.shape == (self.K, 7) and tm.shape == (self.K,)
+            if lib().ora_mech_set_thermo2(self._h, _dp(hi), _dp(tm)) != 0:
+                raise ValueError("ora_mech_set_thermo2 failed")
 
     def __del__(self):
         if getattr(self, "_h", None) and _lib is not None:

@@ -492,6 +492,7 @@ typedef struct ora_mech {
   int32_t *tb_of; /* [R] index of the reaction's third-body row, or -1 */
   double *alpha;  /* [R3][K] dense third-body efficiencies (1 where not listed) */
   int R3;
+  double *nasa_hi, *T_mid; /* optional second temperature range (ora_mech_set_thermo2), else NULL */
 } ora_mech;
 
 static void *dup_mem(const void *src, size_t bytes) {
@@ -506,7 +507,19 @@ void ora_mech_free(ora_mech *m) {
   free(m->reac_ptr); free(m->reac_sp); free(m->reac_nu);
   free(m->prod_ptr); free(m->prod_sp); free(m->prod_nu);
   free(m->tb_of); free(m->alpha);
+  free(m->nasa_hi); free(m->T_mid);
   free(m);
+}
+
+/* Two temperature ranges for the NASA fits ("thermodynamic properties are typically fitted as
+ * polynomials across different temperature ranges"; reading R30, the Chemkin convention): species k uses nasa_high[k]
+ * where T > T_mid[k] and the coefficients given at load (the low range) where T <= T_mid[k].  Arrays are copied. */
+int ora_mech_set_thermo2(ora_mech *m, const double *nasa_high, const double *T_mid) {
+  if (!m || !nasa_high || !T_mid) return ORA_EINVAL;
+  free(m->nasa_hi); free(m->T_mid);
+  m->nasa_hi = (double *)dup_mem(nasa_high, sizeof(double) * 7 * (size_t)m->K);
+  m->T_mid = (double *)dup_mem(T_mid, sizeof(double) * (size_t)m->K);
+  return (m->nasa_hi && m->T_mid) ? ORA_OK : ORA_ENOMEM;
 }
 
 int ora_mech_load(const ora_mech_desc *d, ora_mech **out) {
@@ -589,6 +602,7 @@ static void chem_rhs(const ora_mech *m, const double *y, double p, double *dydt,
   const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
   for (int k = 0; k < K; k++) {
     const double *a = m->nasa + 7 * (size_t)k;
+    if (m->T_mid && T > m->T_mid[k]) a = m->nasa_hi + 7 * (size_t)k; /* R30: the high range above T_mid */
     const double cpR = a[0] + a[1] * T + a[2] * T2 + a[3] * T3 + a[4] * T4;
     const double hRT = a[0] + a[1] * T / 2.0 + a[2] * T2 / 3.0 + a[3] * T3 / 4.0 + a[4] * T4 / 5.0 + a[5] / T;
     cp_sum += Y[k] * cpR / m->W[k];

@@ -50,6 +50,8 @@ class Mechanism:
     tb_eff: np.ndarray           # [nnz_tb] alpha_jk
     rate_factor: float = 1.0     # calibration factor already folded into arr_A
     meta: dict = field(default_factory=dict)
+    nasa_high: np.ndarray = None # [K][7] optional second (high) temperature range, used where T > T_mid[k]
+    T_mid: np.ndarray = None     # [K] K
 
     @property
     def n_species(self) -> int:
@@ -361,6 +363,33 @@ def make_densities(mech: "Mechanism", states: np.ndarray, p: float = P_ATM) -> n
     workload, then held at their own volume.  Input recipe only; no method arithmetic."""
     w = np.asarray(mech.mol_weight, dtype=np.float64)
     return p / (_RU * states[0] * (states[1:] / w[:, None]).sum(axis=0))
+
+
+def with_two_range_thermo(mech: "Mechanism", T_range, seed: int = 0) -> "Mechanism":
+    """The same mechanism with two-range NASA fits: `mech.nasa` stays the low range, a high range is
+    drawn beside it, and each species switches at its own T_mid drawn inside `T_range` (so that a batch of states
+    straddles the switch and systems cross it while they react).  Like real fits, c_p and h are continuous at T_mid:
+    a2..a5 of the high range are drawn (a flatter polynomial), a1 and a6 follow from the two continuity conditions.
+    Input recipe only; the source term itself is in neither library's interest here."""
+    import copy
+    rng = _rng(seed, 900, int(mech.n_species))
+    K = mech.n_species
+    lo = np.asarray(mech.nasa, dtype=np.float64)
+    Tm = rng.uniform(T_range[0] + 0.25 * (T_range[1] - T_range[0]), T_range[1] - 0.25 * (T_range[1] - T_range[0]), size=K)
+    hi = np.zeros_like(lo)
+    hi[:, 1] = lo[:, 1] * rng.uniform(0.3, 0.8, size=K)
+    hi[:, 2] = lo[:, 2] * rng.uniform(0.3, 0.8, size=K)
+    hi[:, 3] = lo[:, 3] * rng.uniform(0.3, 0.8, size=K)
+    hi[:, 4] = lo[:, 4] * rng.uniform(0.3, 0.8, size=K)
+    pw = np.stack([Tm ** i for i in range(5)], axis=1)                       # [K][5]: 1, T, T^2, T^3, T^4
+    hi[:, 0] = (lo[:, :5] * pw).sum(1) - (hi[:, 1:5] * pw[:, 1:]).sum(1)    # c_p/R continuous
+    H = lambda a: (a[:, :5] * pw * Tm[:, None] / np.arange(1, 6)).sum(1)     # T (a1 + a2 T/2 + ... + a5 T^4/5)
+    hi[:, 5] = lo[:, 5] + H(lo) - H(hi)                                       # h/R continuous
+    hi[:, 6] = lo[:, 6]
+    out = copy.copy(mech)
+    out.nasa_high, out.T_mid = np.ascontiguousarray(hi), np.ascontiguousarray(Tm)
+    out.name = mech.name + "+2range"
+    return out
 
 
 def toy_mechanism(K, reactions, W=None, nasa=None, third_body=None, name="toy") -> Mechanism:
