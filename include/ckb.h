@@ -93,6 +93,18 @@ typedef struct ckb_mech ckb_mech; /* opaque; owns the packed tables in device me
 int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out);
 void ckb_mech_free(ckb_mech *m);
 
+/*
+ * ckb_mech_load2: ckb_mech_load for NASA fits with two temperature ranges ("thermodynamic properties are
+ * typically fitted as polynomials across different temperature ranges"; reading R30, the Chemkin convention):
+ *   nasa_high HOST [K][7]  a1..a7 of the high range; d->nasa is the low range
+ *   T_mid     HOST [K]     species k uses nasa_high[k] where T > T_mid[k] and d->nasa[k] where T <= T_mid[k]
+ * Both NULL: identical to ckb_mech_load.  The switch is taken per species and per evaluation of f(y), from the
+ * temperature of the argument (a system may cross T_mid while it reacts); it is a select between two table rows, not a
+ * branch.  Everything else (packing, limits, ownership, errors) as ckb_mech_load; ckb_mech_specialize generates both
+ * ranges.  ckb_mech_precompile / ckb_mech_codegen / ckb_mech_pack_stats describe the one-range mechanism of `d`.
+ */
+int ckb_mech_load2(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, ckb_mech **out);
+
 /* number of species / reactions / fused reaction slots / algorithmic flops per f(y) */
 int ckb_mech_info(const ckb_mech *m, int32_t *n_species, int32_t *n_reactions, int32_t *n_slots,
                   double *flops_per_rhs);

@@ -23,7 +23,7 @@ ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
 EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "ckb_integrate_host",
            "ckb_rhs", "ckb_fp64_probe", "ckb_mech_pack_stats", "ckb_strerror", "ckb_last_cuda_error",
            "ckb_mech_specialize", "ckb_mech_precompile", "ckb_mech_codegen", "ckb_codegen_log",
-           "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv")
+           "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv", "ckb_mech_load2")
 
 
 class CkbError(RuntimeError):
@@ -64,6 +64,8 @@ def lib():
     vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
     L.ckb_mech_load.argtypes = [C.POINTER(_Desc), C.POINTER(vp)]
     L.ckb_mech_load.restype = C.c_int
+    L.ckb_mech_load2.argtypes = [C.POINTER(_Desc), vp, vp, C.POINTER(vp)]
+    L.ckb_mech_load2.restype = C.c_int
     L.ckb_mech_free.argtypes = [vp]
     L.ckb_mech_free.restype = None
     L.ckb_mech_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
@@ -192,7 +194,14 @@ class Mech:
         for k, v in keep.items():
             setattr(d, k, v.ctypes.data)
         self._h = C.c_void_p()
-        _check(lib().ckb_mech_load(C.byref(d), C.byref(self._h)), "ckb_mech_load")
+        if getattr(mech, "nasa_high", None) is not None:    # two temperature ranges (ckb_mech_load2)
+            hi, tm = _f64(mech.nasa_high), _f64(mech.T_mid)
+            if hi.shape != (d.n_species, 7) or tm.shape != (d.n_species,):
+                raise ValueError("nasa_high must be [K][7] and T_mid [K]")
+            _check(lib().ckb_mech_load2(C.byref(d), C.c_void_p(hi.ctypes.data), C.c_void_p(tm.ctypes.data),
+                                        C.byref(self._h)), "ckb_mech_load2")
+        else:
+            _check(lib().ckb_mech_load(C.byref(d), C.byref(self._h)), "ckb_mech_load")
         ks, rs, ns, fl = C.c_int32(), C.c_int32(), C.c_int32(), C.c_double()
         _check(lib().ckb_mech_info(self._h, C.byref(ks), C.byref(rs), C.byref(ns), C.byref(fl)), "ckb_mech_info")
         self.K, self.R, self.n_slots, self.flops_per_rhs = ks.value, rs.value, ns.value, fl.value

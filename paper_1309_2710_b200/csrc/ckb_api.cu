@@ -125,14 +125,16 @@ int dispatch_rhs(const ckb_mech *m, const Launch &l, const ckb_host::RhsArgs &a)
  * ---------------------------------------------------------------------------------------------- */
 extern "C" {
 
-int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out) {
+int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out) { return ckb_mech_load2(d, nullptr, nullptr, out); }
+
+int ckb_mech_load2(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, ckb_mech **out) {
   if (!d || !out) return CKB_EINVAL;
   *out = nullptr;
   ckb_mech *m = new (std::nothrow) ckb_mech();
   if (!m) return CKB_ENOMEM;
   int rc;
   try {
-    rc = ckb_host::load_packings(d, m);
+    rc = ckb_host::load_packings(d, nasa_high, T_mid, m);
   } catch (const std::bad_alloc &) {
     rc = CKB_ENOMEM;
   }

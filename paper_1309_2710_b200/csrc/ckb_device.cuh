@@ -298,10 +298,17 @@ struct Sys {
       const int b = m.o_sp + i * CKB_SP_WORDS * L + g;
       /* R8a: cp_k/R = a1 + a2 T + ... + a5 T^4;  h_k/(RT) = a1 + a2 T/2 + ... + a5 T^4/5 + a6/T */
       double cc[5], hc[6];
+      /* R30 (two temperature ranges, ckb_mech_load2): this lane's species takes its coefficients from the second
+       * species table where T > T_mid -- a select between two table rows, per species and per evaluation */
+      int bt = b;
+      if (m.o_sp2) { /* launch-uniform */
+        const int b2 = m.o_sp2 + i * CKB_SP_WORDS * L + g;
+        if (T[0] > td(b2 + CKB_SP_INVW * L)) bt = b2;
+      }
 #pragma unroll
-      for (int k = 0; k < 5; k++) cc[k] = td(b + (CKB_SP_CP + k) * L);
+      for (int k = 0; k < 5; k++) cc[k] = td(bt + (CKB_SP_CP + k) * L);
 #pragma unroll
-      for (int k = 0; k < 6; k++) hc[k] = td(b + (CKB_SP_H + k) * L);
+      for (int k = 0; k < 6; k++) hc[k] = td(bt + (CKB_SP_H + k) * L);
       const double iw = td(b + CKB_SP_INVW * L);
 #pragma unroll
       for (int q = 0; q < M; q++) {

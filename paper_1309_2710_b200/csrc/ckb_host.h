@@ -44,6 +44,7 @@ struct Rx {
 struct Parsed {
   int K = 0, R = 0;
   std::vector<double> W, nasa;                                  /* [K], [K][7] */
+  std::vector<double> nasa_hi, Tmid;                            /* [K][7], [K]: second temperature range, or empty */
   std::vector<double> A, beta, E;                               /* [R] */
   std::vector<Rx> rx;                                           /* [R] */
   std::vector<std::vector<std::pair<int, double>>> sets;        /* third-body sets: (species, alpha) */
@@ -56,7 +57,7 @@ struct Parsed {
 void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<int> &comp_of_sp);
 int parse_mechanism(const ckb_mech_desc *d, Parsed &P);
 int pack_for(const Parsed &P, int L, Packed &out);
-int load_packings(const ckb_mech_desc *d, ckb_mech *m);
+int load_packings(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, ckb_mech *m);
 #define CKB_NPACK 6
 inline int pack_index(int L) { return L == 1 ? 0 : L == 8 ? 1 : L == 16 ? 2 : L == 32 ? 3 : L == 2 ? 4 : 5; }
 }  // namespace ckb_host

@@ -433,6 +433,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   m.o_glen = take(NV);
   m.o_rflag = off; off += NSR;
   m.o_perm = off; off += n;
+  m.o_sp2 = P.nasa_hi.empty() ? 0 : take((size_t)NV * CKB_SP_WORDS * L);
   m.s_tab = s_tab;
   m.o_rkc = off; off += s_tab - 1;
   m.o_rkcs = off; off += 4 * (s_tab - 1) * s_tab / 2;
@@ -448,6 +449,19 @@ int pack_for(const Parsed &P, int L, Packed &out) {
       const double *a = &P.nasa[7 * (size_t)k];
       putd(base + CKB_SP_INVW * L, 1.0 / P.W[k]);
       putd(base + CKB_SP_W * L, P.W[k]);
+      for (int q = 0; q < 5; q++) {
+        putd(base + (CKB_SP_CP + q) * L, a[q]);
+        putd(base + (CKB_SP_H + q) * L, a[q] / (double)(q + 1));
+      }
+      putd(base + (CKB_SP_H + 5) * L, a[5]);
+    }
+  }
+  if (m.o_sp2) { /* R30: the high range, chosen on the device where T > T_mid (rows of T and padding: zeros) */
+    for (int c = 1; c < n; c++) {
+      const int i = c / L, g = c % L, base = m.o_sp2 + i * CKB_SP_WORDS * L + g;
+      const int k = sp_of_comp[c];
+      const double *a = &P.nasa_hi[7 * (size_t)k];
+      putd(base + CKB_SP_INVW * L, P.Tmid[k]);
       for (int q = 0; q < 5; q++) {
         putd(base + (CKB_SP_CP + q) * L, a[q]);
         putd(base + (CKB_SP_H + q) * L, a[q] / (double)(q + 1));
@@ -567,11 +581,21 @@ int pack_for(const Parsed &P, int L, Packed &out) {
 
 /* parse once, pack for every lanes-per-system value; the thread-per-ODE packing must fit the kernel
  * parameter space (CKB_PARAM_WORDS) */
-int load_packings(const ckb_mech_desc *d, ckb_mech *m) {
+int load_packings(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, ckb_mech *m) {
   m->parsed = std::make_shared<Parsed>();
   Parsed &P = *m->parsed;
   int rc = parse_mechanism(d, P);
   if (rc != CKB_OK) return rc;
+  if ((nasa_high == nullptr) != (T_mid == nullptr)) return CKB_EINVAL;
+  if (nasa_high) {
+    for (int k = 0; k < P.K; k++) {
+      if (!std::isfinite(T_mid[k])) return CKB_EINVAL;
+      for (int q = 0; q < 7; q++)
+        if (!std::isfinite(nasa_high[7 * (size_t)k + q])) return CKB_EINVAL;
+    }
+    P.nasa_hi.assign(nasa_high, nasa_high + 7 * (size_t)P.K);
+    P.Tmid.assign(T_mid, T_mid + P.K);
+  }
   m->K = P.K;
   m->R = P.R;
   m->NS = (int)P.slots.size();

@@ -78,6 +78,8 @@ struct DevMech {
   int s_tab;
   int words;
   int o_perm;        /* [n] original state row (0 = T, 1 + species index) of component c                    */
+  int o_sp2;         /* [NV][13][L] second species table: the high temperature range of the NASA fits, with
+                        T_mid in the CKB_SP_INVW word (W word unused); 0 = the mechanism has one range       */
 };
 
 /* doubles of shared memory per system: C region, [M] region, q region */
