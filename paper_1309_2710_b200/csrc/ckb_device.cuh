@@ -469,17 +469,20 @@ struct Sys {
           for (int q = 0; q < M; q++)
             acc0[q] = fma(coef, *reinterpret_cast<const double *>(reinterpret_cast<const char *>(sQ + q * RS) + o), acc0[q]);
         }
-      } else { /* two entries per word: (int16 coefficient << 16) | q offset */
+      } else { /* two entries per word: (coefficient +1 / -1 << 16) | q offset.  The coefficient is applied by XOR-ing
+                  its sign (bit 31 of the entry) into q: no int -> double conversion, an add instead of an FMA
+                  (exactly fma(+-1, q, acc)); a stoichiometric coefficient |nu| > 1 is entered |nu| times, an idle
+                  entry reads one of the 0.0 slots behind the q region */
         for (int t = 0; t < len; t++, gp += L) {
           const unsigned long long w = tw(gp);
           const unsigned lo = (unsigned)w, hi = (unsigned)(w >> 32);
-          const double c0 = (double)((int)lo >> 16), c1 = (double)((int)hi >> 16);
           const unsigned o0 = lo & 0xFFFFu, o1 = hi & 0xFFFFu;
 #pragma unroll
           for (int q = 0; q < M; q++) {
             const char *qb = reinterpret_cast<const char *>(sQ + q * RS);
-            acc0[q] = fma(c0, *reinterpret_cast<const double *>(qb + o0), acc0[q]);
-            acc1[q] = fma(c1, *reinterpret_cast<const double *>(qb + o1), acc1[q]);
+            const double q0 = *reinterpret_cast<const double *>(qb + o0), q1 = *reinterpret_cast<const double *>(qb + o1);
+            acc0[q] += __hiloint2double(__double2hiint(q0) ^ (int)(lo & 0x80000000u), __double2loint(q0));
+            acc1[q] += __hiloint2double(__double2hiint(q1) ^ (int)(hi & 0x80000000u), __double2loint(q1));
           }
         }
       }
@@ -1098,6 +1101,12 @@ __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem
     for (int q = 0; q < M; q++) {
       sys.sR[q * sys.RS] = 1.0;                          /* "absent molecule" concentration */
       sys.sR[q * sys.RS + (m.n + m.NTB) * GI] = 1.0;     /* "no third body" */
+    }
+  }
+  if (L > 1 && sys.g < CKB_ZERO_SLOTS) { /* the operands of idle gather entries (a group has >= 2 lanes: loop) */
+    for (int z = sys.g; z < CKB_ZERO_SLOTS; z += L) {
+#pragma unroll
+      for (int q = 0; q < M; q++) sys.sR[q * sys.RS + sys.qoff + m.NSR * L + z] = 0.0;
     }
   }
 #endif

@@ -409,7 +409,14 @@ int pack_for(const Parsed &P, int L, Packed &out) {
     for (int g = 0; g < L; g++) {
       const int c = g + L * i;
       if (c < 1 || c >= n) continue;
-      for (auto &sc : P.rows[sp_of_comp[c]]) rows[g].push_back(GEntry{pos_of_slot[sc.first], sc.second});
+      for (auto &sc : P.rows[sp_of_comp[c]]) {
+        if (L == 1) {
+          rows[g].push_back(GEntry{pos_of_slot[sc.first], sc.second});
+        } else { /* lane-distributed mappings apply the coefficient as a sign: |nu| > 1 is entered |nu| times */
+          for (int rep = 0; rep < std::abs(sc.second); rep++)
+            rows[g].push_back(GEntry{pos_of_slot[sc.first], sc.second > 0 ? 1 : -1});
+        }
+      }
     }
     sched[i] = colour_gather(rows, L, optimise);
     glen[i] = (L == 1) ? (int)sched[i].size() : ((int)sched[i].size() + 1) / 2;
@@ -526,7 +533,8 @@ int pack_for(const Parsed &P, int L, Packed &out) {
         for (int g = 0; g < L; g++) {
           GEntry e = t < (int)sched[i].size() ? sched[i][t][g] : GEntry{-1, 0};
           if (e.pos < 0) {
-            e.coef = 0;
+            const bool zero_slot = L > 1; /* idle: + 0.0 from the zero slot of a bank pair nobody else reads */
+            e.coef = zero_slot ? 1 : 0;
             e.pos = g % 16;
             if (L >= 16 && t < (int)sched[i].size()) {
               bool busy[16] = {false};
@@ -539,6 +547,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
               for (int r0 = 0; r0 < 16; r0++)
                 if (!busy[r0]) { e.pos = r0; break; }
             }
+            if (zero_slot) e.pos = NSR * L + ((e.pos - NSR * L) % 16 + 16) % 16; /* same bank pair, behind the q region */
           }
           if (L >= 16) addr[g] = e.pos;
           if (L == 1) { /* double coefficient with the q offset in its 16 lowest mantissa bits */

@@ -13,6 +13,7 @@
  *   [0, n)            C_c, concentration of component c; C_0 = 1.0 stands for "no molecule"
  *   [n, n+NTB+1)      [M]_t per third-body efficiency set; the last one = 1.0 stands for "no third body"
  *   [n+NTB+1, +NSR*L) q_s, net rate of progress of reaction slot s
+ *   L > 1: then 16 doubles of 0.0 (one per bank pair), the operand of an idle entry of the Eq. 3 gather
  */
 #pragma once
 #ifndef __CUDACC__
@@ -70,8 +71,9 @@ struct DevMech {
   int o_rflag;       /* [NSR]              round flags: 1 = a third molecule is read, 2 = a third body is read   */
   int o_tb;          /* [NTBR][TBE][2][L]  (alpha-1, region byte offset of the species)                        */
   int o_glen;        /* [NV]               64-bit words per lane of gather level i (uniform over lanes)   */
-  int o_gat;         /* [sum glen][L]      gather entries.  L > 1: two per word, (int16 coefficient << 16) |
-                                           BYTE offset (x G) of q_s inside the q region; L = 1: one
+  int o_gat;         /* [sum glen][L]      gather entries.  L > 1: two per word, (int16 coefficient +1 / -1 << 16) |
+                                           BYTE offset (x G) of q_s inside the q region (bit 31 = sign of the
+                                           coefficient; |nu| > 1 is entered nu times; idle: a 0.0 slot); L = 1: one
                                            per word, double coefficient with the offset in its low 16 bits */
   int o_rkc;         /* RKC coefficients for s = 2..s_tab: [s-2] -> mu~_1; stages at o_rkcs               */
   int o_rkcs;        /* [(s-2)(s-1)/2 + (j-2)][4] = mu_j, nu_j, mu~_j, gamma~_j, j = 2..s                  */
@@ -83,6 +85,9 @@ struct DevMech {
 };
 
 /* doubles of shared memory per system: C region, [M] region, q region */
-__host__ __device__ __forceinline__ int region_doubles(const DevMech &m) { return m.n + m.NTB + 1 + m.NSR * m.L; }
+#define CKB_ZERO_SLOTS 16 /* L > 1: 0.0 in every bank pair behind the q region, read by idle gather entries */
+__host__ __device__ __forceinline__ int region_doubles(const DevMech &m) {
+  return m.n + m.NTB + 1 + m.NSR * m.L + (m.L > 1 ? CKB_ZERO_SLOTS : 0);
+}
 
 }  // namespace ckb

@@ -207,4 +207,4 @@ def test_parity_cv_paper_settings(cfg, N, dt, rtol, atol):
     rho = synth.make_densities(mech, states, p)
     ora = _oracle_cv(mech, states, 0.0, dt, spec.method, density=rho, rtol=rtol, atol=atol)
     gpu = _run_gpu_cv(mech, states, 0.0, dt, spec.method, density=rho, rtol=rtol, atol=atol)
-    _compare(gpu, ora, max_flip_frac=5e-3)
+    _compare(gpu, ora, max_flip_frac=5e-3, rtol=rtol, atol=atol)

@@ -42,7 +42,7 @@ def _run_gpu(mech, states, p, dt, method, variant="auto", ld=None, pressure=None
     return out[:, :N].copy(), status.cpu().numpy(), stats.cpu().numpy()
 
 
-def _compare(gpu, ora, max_flip_frac=2e-3, y_cut=Y_CUT):
+def _compare(gpu, ora, max_flip_frac=2e-3, y_cut=Y_CUT, rtol=RTOL, atol=ATOL):
     (yg, sg, tg), (yo, so, to) = gpu, ora
     N = yg.shape[1]
     assert np.isfinite(yg).all()
@@ -56,10 +56,12 @@ def _compare(gpu, ora, max_flip_frac=2e-3, y_cut=Y_CUT):
     n_flip = int((~same).sum())
     assert n_flip <= max(2, int(max_flip_frac * N)), f"{n_flip} of {N} systems took different decisions"
     if n_flip:
-        # a flipped system is still a valid integration: agrees to the integrator's own accuracy
-        assert relT[~same].max() <= 1e-6
+        # a flipped system is still a valid integration (R28: a different, equally correct step sequence):
+        # it agrees to the integrator's own accuracy, which scales with the requested tolerances -- 100 rtol on T,
+        # 1000 rtol |Y| + 1000 atol on Y (1e-6, 1e-5 and 1e-9 at BASELINE.json's rtol = 1e-8, atol = 1e-12)
+        assert relT[~same].max() <= 100.0 * rtol
         absY = np.abs(Yg - Yo)[:, ~same]
-        assert (absY <= 1e-5 * np.abs(Yo[:, ~same]) + 1e-9).all()
+        assert (absY <= 1e3 * rtol * np.abs(Yo[:, ~same]) + 1e3 * atol).all()
     return dict(n=N, flipped=n_flip, relT=float(relT[same].max(initial=0.0)), relY=float(relY[same].max(initial=0.0)))
 
 
@@ -139,7 +141,7 @@ def test_parity_paper_settings(cfg, N, dt, rtol, atol, variant):
     states, p = synth.make_states(cfg, N)
     ora = _oracle(mech, states, p, dt, spec.method, rtol=rtol, atol=atol)
     gpu = _run_gpu(mech, states, p, dt, spec.method, variant=variant, rtol=rtol, atol=atol)
-    rep = _compare(gpu, ora, max_flip_frac=5e-3)
+    rep = _compare(gpu, ora, max_flip_frac=5e-3, rtol=rtol, atol=atol)
     print(f"paper settings cfg{cfg} {spec.method} {variant} dt={dt} rtol={rtol}: {rep}, stages max {ora[2][3].max()}")
     assert np.isin(ora[1], (0, 4)).all()
 
