@@ -172,3 +172,22 @@ def test_precompile_fills_cache(L, tmp_path, monkeypatch):
     binding.precompile(mech)
     assert time.time() - t1 < 0.5 * (t1 - t0) + 0.05
     assert len(list((tmp_path / "jit").iterdir())) == 1
+
+
+def test_mech_load2_rejects_bad_input(L):
+    """ckb_mech_load2 validates the second temperature range before any CUDA call (same codes with or without a GPU)."""
+    mech = synth.with_two_range_thermo(synth.make_mechanism(0), synth.CONFIGS[0].T_range)
+    d, keep = binding._make_desc(mech)
+    h = C.c_void_p()
+    hi = np.ascontiguousarray(mech.nasa_high)
+    tm = np.ascontiguousarray(mech.T_mid)
+    vp = lambda a: C.c_void_p(a.ctypes.data)
+    assert L.ckb_mech_load2(C.byref(d), vp(hi), None, C.byref(h)) == binding.EINVAL      # one array without the other
+    assert L.ckb_mech_load2(C.byref(d), None, vp(tm), C.byref(h)) == binding.EINVAL
+    bad = tm.copy()
+    bad[2] = np.inf
+    assert L.ckb_mech_load2(C.byref(d), vp(hi), vp(bad), C.byref(h)) == binding.EINVAL
+    bad_hi = hi.copy()
+    bad_hi[1, 3] = np.nan
+    assert L.ckb_mech_load2(C.byref(d), vp(bad_hi), vp(tm), C.byref(h)) == binding.EINVAL
+    assert L.ckb_mech_load2(None, vp(hi), vp(tm), C.byref(h)) == binding.EINVAL
