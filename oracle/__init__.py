@@ -62,6 +62,8 @@ def lib():
         L.ora_integrate.restype = C.c_int
         L.ora_mech_set_thermo2.argtypes = [C.c_void_p, dp, dp]
         L.ora_mech_set_thermo2.restype = C.c_int
+        L.ora_mech_set_falloff.argtypes = [C.c_void_p, C.c_int32, ip, dp, dp]
+        L.ora_mech_set_falloff.restype = C.c_int
         L.ora_rhs_cv.argtypes = L.ora_rhs.argtypes
         L.ora_rhs_cv.restype = None
         L.ora_integrate_cv.argtypes = L.ora_integrate.argtypes
@@ -140,6 +142,13 @@ class OracleMech:
             assert hi.shape == (self.K, 7) and tm.shape == (self.K,)
             if lib().ora_mech_set_thermo2(self._h, _dp(hi), _dp(tm)) != 0:
                 raise ValueError("ora_mech_set_thermo2 failed")
+
+        # optional fall-off reactions (reading R31): fo_reaction [n], fo_low [n][3], fo_troe [n][4]
+        if getattr(mech, "fo_reaction", None) is not None and len(mech.fo_reaction):
+            fr, lo, tr = _i32(mech.fo_reaction), _f64(mech.fo_low), _f64(mech.fo_troe)
+            assert lo.shape == (len(fr), 3) and tr.shape == (len(fr), 4)
+            if lib().ora_mech_set_falloff(self._h, len(fr), _ip(fr), _dp(lo), _dp(tr)) != 0:
+                raise ValueError("ora_mech_set_falloff failed")
 
     def __del__(self):
         if getattr(self, "_h", None) and _lib is not None:

@@ -493,6 +493,8 @@ typedef struct ora_mech {
   double *alpha;  /* [R3][K] dense third-body efficiencies (1 where not listed) */
   int R3;
   double *nasa_hi, *T_mid; /* optional second temperature range (ora_mech_set_thermo2), else NULL */
+  int32_t *fo_of;          /* optional fall-off reactions (ora_mech_set_falloff): [R] row of the reaction or -1 */
+  double *fo_low, *fo_troe;/* [n_fo][3] A_0, beta_0, E_0;  [n_fo][4] a, T***, T*, T** (a = NaN: Lindemann) */
 } ora_mech;
 
 static void *dup_mem(const void *src, size_t bytes) {
@@ -508,7 +510,31 @@ void ora_mech_free(ora_mech *m) {
   free(m->prod_ptr); free(m->prod_sp); free(m->prod_nu);
   free(m->tb_of); free(m->alpha);
   free(m->nasa_hi); free(m->T_mid);
+  free(m->fo_of); free(m->fo_low); free(m->fo_troe);
   free(m);
+}
+
+/* Pressure-dependent (fall-off) reactions (P:80 refers to the Chemkin manual for the formulation;
+ * reading R31, that manual's form): for a reaction listed here the Arrhenius parameters given at load are the
+ * high-pressure limit k_inf, (A_0, beta_0, E_0) the low-pressure limit k_0, and
+ *     P_r = k_0 [M] / k_inf,   k = k_inf (P_r / (1 + P_r)) F,   rate of progress = k prod C  (no further [M] factor),
+ * [M] = sum_k alpha_k C_k with the reaction's third-body efficiencies if it is also listed as a third-body reaction,
+ * else all alpha = 1.  Lindemann: F = 1.  Troe: log10 F = log10 F_cent / (1 + ((log10 P_r + c)/(n - 0.14 (log10 P_r + c)))^2),
+ * c = -0.4 - 0.67 log10 F_cent, n = 0.75 - 1.27 log10 F_cent, F_cent = (1-a) exp(-T/T***) + a exp(-T/T*) + exp(-T** / T)
+ * (the last term is left out where T** is not finite).  troe[i][0] = NaN marks a Lindemann reaction. */
+int ora_mech_set_falloff(ora_mech *m, int32_t n_fo, const int32_t *reaction, const double *low3, const double *troe4) {
+  if (!m || n_fo < 0 || (n_fo > 0 && (!reaction || !low3 || !troe4))) return ORA_EINVAL;
+  free(m->fo_of); free(m->fo_low); free(m->fo_troe);
+  m->fo_of = (int32_t *)malloc(sizeof(int32_t) * (size_t)(m->R ? m->R : 1));
+  m->fo_low = (double *)dup_mem(low3, sizeof(double) * 3 * (size_t)n_fo);
+  m->fo_troe = (double *)dup_mem(troe4, sizeof(double) * 4 * (size_t)n_fo);
+  if (!m->fo_of || !m->fo_low || !m->fo_troe) return ORA_ENOMEM;
+  for (int j = 0; j < m->R; j++) m->fo_of[j] = -1;
+  for (int i = 0; i < n_fo; i++) {
+    if (reaction[i] < 0 || reaction[i] >= m->R || m->fo_of[reaction[i]] >= 0) return ORA_EINVAL;
+    m->fo_of[reaction[i]] = i;
+  }
+  return ORA_OK;
 }
 
 /* Two temperature ranges for the NASA fits ("thermodynamic properties are typically fitted as
@@ -582,7 +608,28 @@ static void chem_rhs(const ora_mech *m, const double *y, double p, double *dydt,
   for (int j = 0; j < R; j++) {
     const double kj = m->A[j] * pow(T, m->beta[j]) * exp(-m->E[j] / (ORA_RC * T));   /* Eq. 5, literal */
     double rate = kj;
-    if (m->tb_of[j] >= 0) {                 /* R22: [M]_j = sum_k alpha_jk C_k */
+    if (m->fo_of && m->fo_of[j] >= 0) {     /* R31: fall-off, kj is k_inf */
+      const double *lo = m->fo_low + 3 * (size_t)m->fo_of[j], *tr = m->fo_troe + 4 * (size_t)m->fo_of[j];
+      double M = 0.0;
+      if (m->tb_of[j] >= 0) {
+        const double *al = m->alpha + (size_t)m->tb_of[j] * K;
+        for (int k = 0; k < K; k++) M += al[k] * C[k];
+      } else {
+        for (int k = 0; k < K; k++) M += C[k];
+      }
+      const double k0 = lo[0] * pow(T, lo[1]) * exp(-lo[2] / (ORA_RC * T));
+      const double Pr = k0 * M / kj;
+      double F = 1.0;                       /* Lindemann */
+      if (tr[0] == tr[0]) {                 /* Troe (a is not NaN) */
+        double Fcent = (1.0 - tr[0]) * exp(-T / tr[1]) + tr[0] * exp(-T / tr[2]);
+        if (isfinite(tr[3])) Fcent += exp(-tr[3] / T);
+        const double lF = log10(Fcent), lP = log10(Pr);
+        const double c = -0.4 - 0.67 * lF, nn = 0.75 - 1.27 * lF;
+        const double x = (lP + c) / (nn - 0.14 * (lP + c));
+        F = pow(10.0, lF / (1.0 + x * x));
+      }
+      rate = kj * (Pr / (1.0 + Pr)) * F;
+    } else if (m->tb_of[j] >= 0) {          /* R22: [M]_j = sum_k alpha_jk C_k */
       const double *al = m->alpha + (size_t)m->tb_of[j] * K;
       double M = 0.0;
       for (int k = 0; k < K; k++) M += al[k] * C[k];

@@ -194,6 +194,9 @@ class Mech:
         for k, v in keep.items():
             setattr(d, k, v.ctypes.data)
         self._h = C.c_void_p()
+        if getattr(mech, "fo_reaction", None) is not None and len(mech.fo_reaction):
+            # no silent degradation: the C ABI has no entry for fall-off reactions yet
+            raise NotImplementedError("fall-off (pressure-dependent) reactions are not supported by the CUDA library")
         if getattr(mech, "nasa_high", None) is not None:    # two temperature ranges (ckb_mech_load2)
             hi, tm = _f64(mech.nasa_high), _f64(mech.T_mid)
             if hi.shape != (d.n_species, 7) or tm.shape != (d.n_species,):

@@ -52,6 +52,9 @@ class Mechanism:
     meta: dict = field(default_factory=dict)
     nasa_high: np.ndarray = None # [K][7] optional second (high) temperature range, used where T > T_mid[k]
     T_mid: np.ndarray = None     # [K] K
+    fo_reaction: np.ndarray = None  # [n_fo] int32: fall-off reactions (arr_A/beta/E are then the high-pressure limit)
+    fo_low: np.ndarray = None       # [n_fo][3] A_0, beta_0, E_0 of the low-pressure limit
+    fo_troe: np.ndarray = None      # [n_fo][4] a, T***, T*, T** (a = NaN: Lindemann; T** = inf: three-parameter form)
 
     @property
     def n_species(self) -> int:
