@@ -105,6 +105,25 @@ void ckb_mech_free(ckb_mech *m);
  */
 int ckb_mech_load2(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, ckb_mech **out);
 
+/*
+ * ckb_mech_load3: ckb_mech_load2 (nasa_high / T_mid may both be NULL) plus pressure-dependent "fall-off" reactions
+ * (P:80 refers to the Chemkin manual for the formulation; reading R31 takes that manual's form):
+ *   n_falloff            number of fall-off reactions (0: identical to ckb_mech_load2)
+ *   fo_reaction HOST [n] reaction index; its arr_A / arr_beta / arr_E are then the HIGH-pressure limit k_inf (A > 0)
+ *   fo_low      HOST [n][3] A_0 (> 0), beta_0, E_0 (cal/mol) of the low-pressure limit k_0
+ *   fo_troe     HOST [n][4] a, T***, T*, T** of Troe's broadening; a = NaN: Lindemann (F = 1); T** = +inf: the
+ *                        three-parameter form (no exp(-T** / T) term); T***, T* > 0 (+inf allowed)
+ *     P_r = k_0 [M] / k_inf,   k = k_inf (P_r / (1 + P_r)) F,   rate of progress = k prod C   (no further [M] factor)
+ *     log10 F = log10 F_cent / (1 + ((log10 P_r + c) / (n - 0.14 (log10 P_r + c)))^2),  c = -0.4 - 0.67 log10 F_cent,
+ *     n = 0.75 - 1.27 log10 F_cent,  F_cent = (1 - a) exp(-T/T***) + a exp(-T/T*) + exp(-T** / T)
+ * [M] uses the reaction's third-body efficiencies if it is also listed in tb_reaction, else all alpha = 1.  On the
+ * device the factor P_r/(1+P_r) F takes the place of the reaction's third-body concentration (it is a per-reaction
+ * multiplier of the same kind), so the reaction loop is unchanged.  CKB_EINVAL: a reaction listed twice or out of range,
+ * non-positive A_0 or A_inf, non-finite parameters.
+ */
+int ckb_mech_load3(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, int32_t n_falloff,
+                   const int32_t *fo_reaction, const double *fo_low, const double *fo_troe, ckb_mech **out);
+
 /* number of species / reactions / fused reaction slots / algorithmic flops per f(y) */
 int ckb_mech_info(const ckb_mech *m, int32_t *n_species, int32_t *n_reactions, int32_t *n_slots,
                   double *flops_per_rhs);

@@ -23,7 +23,7 @@ ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
 EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "ckb_integrate_host",
            "ckb_rhs", "ckb_fp64_probe", "ckb_mech_pack_stats", "ckb_strerror", "ckb_last_cuda_error",
            "ckb_mech_specialize", "ckb_mech_precompile", "ckb_mech_codegen", "ckb_codegen_log",
-           "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv", "ckb_mech_load2")
+           "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv", "ckb_mech_load2", "ckb_mech_load3")
 
 
 class CkbError(RuntimeError):
@@ -66,6 +66,8 @@ def lib():
     L.ckb_mech_load.restype = C.c_int
     L.ckb_mech_load2.argtypes = [C.POINTER(_Desc), vp, vp, C.POINTER(vp)]
     L.ckb_mech_load2.restype = C.c_int
+    L.ckb_mech_load3.argtypes = [C.POINTER(_Desc), vp, vp, i32, vp, vp, vp, C.POINTER(vp)]
+    L.ckb_mech_load3.restype = C.c_int
     L.ckb_mech_free.argtypes = [vp]
     L.ckb_mech_free.restype = None
     L.ckb_mech_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
@@ -194,10 +196,17 @@ class Mech:
         for k, v in keep.items():
             setattr(d, k, v.ctypes.data)
         self._h = C.c_void_p()
-        if getattr(mech, "fo_reaction", None) is not None and len(mech.fo_reaction):
-            # no silent degradation: the C ABI has no entry for fall-off reactions yet
-            raise NotImplementedError("fall-off (pressure-dependent) reactions are not supported by the CUDA library")
-        if getattr(mech, "nasa_high", None) is not None:    # two temperature ranges (ckb_mech_load2)
+        if getattr(mech, "fo_reaction", None) is not None and len(mech.fo_reaction):   # fall-off reactions
+            fr, lo, tr = _i32(mech.fo_reaction), _f64(mech.fo_low), _f64(mech.fo_troe)
+            if lo.shape != (len(fr), 3) or tr.shape != (len(fr), 4):
+                raise ValueError("fo_low must be [n][3] and fo_troe [n][4]")
+            hi = tm = None
+            if getattr(mech, "nasa_high", None) is not None:
+                hi, tm = _f64(mech.nasa_high), _f64(mech.T_mid)
+            p_ = lambda a: None if a is None else C.c_void_p(a.ctypes.data)
+            _check(lib().ckb_mech_load3(C.byref(d), p_(hi), p_(tm), len(fr), p_(fr), p_(lo), p_(tr), C.byref(self._h)),
+                   "ckb_mech_load3")
+        elif getattr(mech, "nasa_high", None) is not None:    # two temperature ranges (ckb_mech_load2)
             hi, tm = _f64(mech.nasa_high), _f64(mech.T_mid)
             if hi.shape != (d.n_species, 7) or tm.shape != (d.n_species,):
                 raise ValueError("nasa_high must be [K][7] and T_mid [K]")

@@ -128,13 +128,19 @@ extern "C" {
 int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out) { return ckb_mech_load2(d, nullptr, nullptr, out); }
 
 int ckb_mech_load2(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, ckb_mech **out) {
-  if (!d || !out) return CKB_EINVAL;
+  return ckb_mech_load3(d, nasa_high, T_mid, 0, nullptr, nullptr, nullptr, out);
+}
+
+int ckb_mech_load3(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, int32_t n_falloff,
+                   const int32_t *fo_reaction, const double *fo_low, const double *fo_troe, ckb_mech **out) {
+  if (!d || !out || n_falloff < 0) return CKB_EINVAL;
+  const ckb_host::FoDesc fo{n_falloff, fo_reaction, fo_low, fo_troe};
   *out = nullptr;
   ckb_mech *m = new (std::nothrow) ckb_mech();
   if (!m) return CKB_ENOMEM;
   int rc;
   try {
-    rc = ckb_host::load_packings(d, nasa_high, T_mid, m);
+    rc = ckb_host::load_packings(d, nasa_high, T_mid, n_falloff > 0 ? &fo : nullptr, m);
   } catch (const std::bad_alloc &) {
     rc = CKB_ENOMEM;
   }

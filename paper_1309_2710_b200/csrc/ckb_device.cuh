@@ -369,6 +369,29 @@ struct Sys {
           Mc[q] = fma(am1, *reinterpret_cast<const double *>(reinterpret_cast<const char *>(sR + q * RS) + off), Mc[q]);
       }
       const int t = r * L + g;
+      if (m.o_fo) { /* launch-uniform: the mechanism has fall-off reactions (R31) */
+        const int fb = m.o_fo + r * 8 * L + g;
+        const int kind = (int)td(fb);
+        if (kind > 0) { /* this set belongs to a fall-off reaction: "[M]" becomes P_r/(1+P_r) F, k_j stays k_inf */
+          const ExpConst<false> fec;
+          const double dlnA = td(fb + L), dbeta = td(fb + 2 * L), dtheta = td(fb + 3 * L);
+#pragma unroll
+          for (int q = 0; q < M; q++) {
+            const double Pr = Mc[q] * ckb_exp(fma(-dtheta, invT[q], fma(dbeta, lnT[q], dlnA)), fec);
+            double B = Pr / (1.0 + Pr);
+            if (kind >= 2) { /* Troe */
+              const double a = td(fb + 4 * L);
+              double Fc = (1.0 - a) * ckb_exp(-T[q] * td(fb + 5 * L), fec) + a * ckb_exp(-T[q] * td(fb + 6 * L), fec);
+              if (kind == 2) Fc += ckb_exp(-td(fb + 7 * L) * invT[q], fec);
+              const double lF = log10(Fc), lP = log10(Pr);
+              const double c = -0.4 - 0.67 * lF, nn = 0.75 - 1.27 * lF;
+              const double x = (lP + c) / (nn - 0.14 * (lP + c));
+              B *= exp(2.302585092994046 * (lF / (1.0 + x * x)));
+            }
+            Mc[q] = B;
+          }
+        }
+      }
       if (t < m.NTB) {
 #pragma unroll
         for (int q = 0; q < M; q++) sR[q * RS + (n + t) * GI] = Mc[q];

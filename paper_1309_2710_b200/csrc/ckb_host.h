@@ -48,6 +48,10 @@ struct Parsed {
   std::vector<double> A, beta, E;                               /* [R] */
   std::vector<Rx> rx;                                           /* [R] */
   std::vector<std::vector<std::pair<int, double>>> sets;        /* third-body sets: (species, alpha) */
+  /* fall-off reactions (R31): each owns one efficiency set; fo[t] describes set t (kind 0: an ordinary set).
+   * kind 1 Lindemann, 2 Troe with the T** term, 3 Troe without it */
+  struct Fo { int kind = 0; double dlnA = 0, dbeta = 0, dtheta = 0, a = 0, invT3 = 0, invT1 = 0, T2 = 0; };
+  std::vector<Fo> fo;                                           /* [sets.size()] or empty */
   struct Slot { int f, r; };
   std::vector<Slot> slots;                                      /* fused forward/reverse pairs */
   std::vector<std::vector<std::pair<int, int>>> rows;           /* [K] gather rows: (slot, net coefficient) */
@@ -55,9 +59,10 @@ struct Parsed {
 };
 /* components: 0 = T, then species by decreasing gather-row length (ckb_tables.h) */
 void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<int> &comp_of_sp);
-int parse_mechanism(const ckb_mech_desc *d, Parsed &P);
+struct FoDesc { int n; const int32_t *reaction; const double *low3, *troe4; };
+int parse_mechanism(const ckb_mech_desc *d, Parsed &P, const FoDesc *fo = nullptr);
 int pack_for(const Parsed &P, int L, Packed &out);
-int load_packings(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, ckb_mech *m);
+int load_packings(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, const FoDesc *fo, ckb_mech *m);
 #define CKB_NPACK 6
 inline int pack_index(int L) { return L == 1 ? 0 : L == 8 ? 1 : L == 16 ? 2 : L == 32 ? 3 : L == 2 ? 4 : 5; }
 }  // namespace ckb_host

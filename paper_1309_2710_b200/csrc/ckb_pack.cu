@@ -27,7 +27,7 @@ inline unsigned long long dbits(double x) {
 
 }  // namespace
 
-int parse_mechanism(const ckb_mech_desc *d, Parsed &P) {
+int parse_mechanism(const ckb_mech_desc *d, Parsed &P, const FoDesc *fo) {
   const int K = d->n_species, R = d->n_reactions, R3 = d->n_third_body;
   if (K < 1 || R < 0 || R3 < 0) return CKB_EINVAL;
   if (!d->mol_weight || !d->nasa) return CKB_EINVAL;
@@ -92,6 +92,41 @@ int parse_mechanism(const ckb_mech_desc *d, Parsed &P) {
     }
     rx[j].tbset = it->second;
   }
+  /* R31: a fall-off reaction owns an efficiency set (its third-body efficiencies if it has them, else all 1), whose
+   * "[M]" the kernels replace by the blending factor P_r/(1+P_r) F -- a per-reaction multiplier like [M] itself */
+  if (fo && fo->n > 0) {
+    if (!fo->reaction || !fo->low3 || !fo->troe4) return CKB_EINVAL;
+    std::vector<char> seen(R, 0);
+    for (int i = 0; i < fo->n; i++) {
+      const int j = fo->reaction[i];
+      if (j < 0 || j >= R || seen[j]) return CKB_EINVAL;
+      seen[j] = 1;
+      const double A0 = fo->low3[3 * i], b0 = fo->low3[3 * i + 1], E0 = fo->low3[3 * i + 2];
+      const double *tr = fo->troe4 + 4 * (size_t)i;
+      if (!(A0 > 0.0) || !std::isfinite(A0) || !std::isfinite(b0) || !std::isfinite(E0) || !(d->arr_A[j] > 0.0))
+        return CKB_EINVAL;
+      Parsed::Fo f;
+      f.dlnA = std::log(A0) - std::log(d->arr_A[j]);
+      f.dbeta = b0 - d->arr_beta[j];
+      f.dtheta = (E0 - d->arr_E[j]) / RC_CAL;
+      if (tr[0] != tr[0]) {
+        f.kind = 1;
+      } else {
+        if (!std::isfinite(tr[0]) || !(tr[1] > 0.0) || !(tr[2] > 0.0) || tr[3] != tr[3]) return CKB_EINVAL;
+        f.kind = std::isfinite(tr[3]) ? 2 : 3;
+        f.a = tr[0];
+        f.invT3 = 1.0 / tr[1]; /* 1/inf = 0: exp(-T/inf) = 1 */
+        f.invT1 = 1.0 / tr[2];
+        f.T2 = std::isfinite(tr[3]) ? tr[3] : 0.0;
+      }
+      std::vector<std::pair<int, double>> key;
+      if (rx[j].tbset >= 0) key = P.sets[rx[j].tbset];
+      rx[j].tbset = (int)P.sets.size();
+      P.sets.push_back(key);
+      P.fo.resize(P.sets.size());
+      P.fo.back() = f;
+    }
+  }
   if (P.sets.size() > 65000) return CKB_EUNSUPPORTED;
 
   /* fuse forward / reverse reactions over the same species (and the same third body) into one slot */
@@ -132,6 +167,10 @@ int parse_mechanism(const ckb_mech_desc *d, Parsed &P) {
   }
   for (int r = 0; r < R3; r++) F += 2.0 * (d->tb_ptr[r + 1] - d->tb_ptr[r]) + 1.0; /* P:80 */
   F += 27.0 * K + 46.0 + 3.0 * 36.0; /* thermo, Eq. 2, Eq. 6, rho, ln T, 1/T */
+  for (auto &f : P.fo) {             /* R31: k_0 (one exp), P_r, P_r/(1+P_r); Troe: F_cent, two log10, 10^x */
+    if (f.kind >= 1) F += 4.0 + 30.0 + 2.0 + 36.0;
+    if (f.kind >= 2) F += (f.kind == 2 ? 3.0 : 2.0) * 32.0 + 2.0 * 46.0 + 12.0 + 36.0 + 36.0 + 30.0;
+  }
   P.flops_per_rhs = F;
   return CKB_OK;
 }
@@ -441,6 +480,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   m.o_rflag = off; off += NSR;
   m.o_perm = off; off += n;
   m.o_sp2 = P.nasa_hi.empty() ? 0 : take((size_t)NV * CKB_SP_WORDS * L);
+  m.o_fo = P.fo.empty() ? 0 : take((size_t)NTBR * 8 * L);
   m.s_tab = s_tab;
   m.o_rkc = off; off += s_tab - 1;
   m.o_rkcs = off; off += 4 * (s_tab - 1) * s_tab / 2;
@@ -508,6 +548,14 @@ int pack_for(const Parsed &P, int L, Packed &out) {
     if (pl.slot >= 0) {
       if (pl.a[2] || pl.b[2]) b[(size_t)m.o_rflag + r] |= 1ull;
       if (P.rx[P.slots[pl.slot].f].tbset >= 0) b[(size_t)m.o_rflag + r] |= 2ull;
+    }
+  }
+  if (m.o_fo) { /* R31: per efficiency set, zeros (kind 0) for ordinary and padding sets */
+    for (int t = 0; t < (int)P.fo.size(); t++) {
+      const int r = t / L, g = t % L, base = m.o_fo + r * 8 * L + g;
+      const Parsed::Fo &f = P.fo[t];
+      const double w8[8] = {(double)f.kind, f.dlnA, f.dbeta, f.dtheta, f.a, f.invT3, f.invT1, f.T2};
+      for (int x = 0; x < 8; x++) putd(base + x * L, w8[x]);
     }
   }
   for (int t = 0; t < NTBR * L; t++) { /* third-body sets, padded with (alpha - 1) = 0 on C_0 */
@@ -590,10 +638,10 @@ int pack_for(const Parsed &P, int L, Packed &out) {
 
 /* parse once, pack for every lanes-per-system value; the thread-per-ODE packing must fit the kernel
  * parameter space (CKB_PARAM_WORDS) */
-int load_packings(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, ckb_mech *m) {
+int load_packings(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, const FoDesc *fo, ckb_mech *m) {
   m->parsed = std::make_shared<Parsed>();
   Parsed &P = *m->parsed;
-  int rc = parse_mechanism(d, P);
+  int rc = parse_mechanism(d, P, fo);
   if (rc != CKB_OK) return rc;
   if ((nasa_high == nullptr) != (T_mid == nullptr)) return CKB_EINVAL;
   if (nasa_high) {

@@ -80,6 +80,9 @@ struct DevMech {
   int s_tab;
   int words;
   int o_perm;        /* [n] original state row (0 = T, 1 + species index) of component c                    */
+  int o_fo;          /* [NTBR][8][L] fall-off description of efficiency set t (R31): kind (0 none, 1 Lindemann,
+                        2 Troe, 3 Troe without T**), ln A_0 - ln A_inf, beta_0 - beta_inf, (E_0 - E_inf)/R_c,
+                        a, 1/T***, 1/T*, T**; 0 = the mechanism has no fall-off reaction                     */
   int o_sp2;         /* [NV][13][L] second species table: the high temperature range of the NASA fits, with
                         T_mid in the CKB_SP_INVW word (W word unused); 0 = the mechanism has one range       */
 };

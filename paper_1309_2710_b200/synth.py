@@ -395,6 +395,35 @@ def with_two_range_thermo(mech: "Mechanism", T_range, seed: int = 0) -> "Mechani
     return out
 
 
+def with_falloff(mech: "Mechanism", seed: int = 0) -> "Mechanism":
+    """The same mechanism with some reactions turned into pressure-dependent (fall-off) reactions:
+    every second third-body reaction (they keep their efficiencies for [M]) and three reactions without a third body.
+    The listed Arrhenius parameters become the high-pressure limit; the low-pressure limit is drawn so that the reduced
+    pressure P_r = k_0 [M]/k_inf spans about 1e-2..1e2 at 1 atm (A_0 = A_inf 10^U(-1.5, 1.5) / C_ref with C_ref the molar
+    density at 1 atm and 1200 K, beta_0 = beta_inf - U(0, 1), E_0 = E_inf + U(-3, 3) kcal/mol) -- the fall-off regime, as
+    for the real mechanisms' (+M) reactions at atmospheric pressure.  One half Lindemann, one quarter Troe with four and
+    one quarter with three parameters (a ~ U(0.3, 0.8), T*** ~ U(50, 500), T* ~ U(800, 3000), T** ~ U(2000, 6000) K)."""
+    import copy
+    rng = _rng(seed, 901, int(mech.n_reactions))
+    tb = [int(j) for j in mech.tb_reaction[::2]]
+    plain = [j for j in range(mech.n_reactions) if j not in set(int(x) for x in mech.tb_reaction)][:3]
+    pick = np.array(sorted(tb + plain), dtype=np.int32)
+    n = len(pick)
+    c_ref = P_ATM / (_RU * 1200.0)
+    low = np.stack([mech.arr_A[pick] * 10.0 ** rng.uniform(-1.5, 1.5, size=n) / c_ref,
+                    mech.arr_beta[pick] - rng.uniform(0.0, 1.0, size=n),
+                    mech.arr_E[pick] + rng.uniform(-3000.0, 3000.0, size=n)], axis=1)
+    troe = np.full((n, 4), np.nan)
+    for i in range(n):
+        if i % 2 == 1:
+            troe[i] = (rng.uniform(0.3, 0.8), rng.uniform(50.0, 500.0), rng.uniform(800.0, 3000.0),
+                       rng.uniform(2000.0, 6000.0) if i % 4 == 1 else np.inf)
+    out = copy.copy(mech)
+    out.fo_reaction, out.fo_low, out.fo_troe = pick, np.ascontiguousarray(low), np.ascontiguousarray(troe)
+    out.name = mech.name + "+falloff"
+    return out
+
+
 def toy_mechanism(K, reactions, W=None, nasa=None, third_body=None, name="toy") -> Mechanism:
     """Hand-built mechanism for closed-form tests.
 

@@ -1,6 +1,5 @@
 """Pins for the oracle's fall-off reactions (reading R31: the Chemkin-manual form the paper refers to,
-P:80).  The CUDA library does not take fall-off reactions yet (binding refuses them); the oracle and its pins are committed
-first, as for every other part of the path.
+P:80).  The oracle and its pins were committed before the CUDA path (ckb_mech_load3; parity in tests/test_gpu_falloff.py).
 
 The pins reduce the fall-off rate to paths pinned elsewhere (third-body and plain reactions, test_oracle_chem.py) in its
 two limits, and fix the constants of the blending function at the points where it has closed-form values:
@@ -138,9 +137,3 @@ def test_only_listed_reactions_change_and_integration_runs():
         assert np.allclose(a.rhs(states[:, i].copy(), p), b.rhs(states[:, i].copy(), p), rtol=1e-12, atol=0)
     y1, st, _ = a.integrate(states, p, 1e-6, 1e-8, 1e-12, "rkck")
     assert (st == 0).all() and np.abs(y1[1:].sum(0) - 1.0).max() < 1e-12
-
-
-def test_cuda_binding_refuses_falloff_loudly():
-    from paper_1309_2710_b200 import binding
-    with pytest.raises(NotImplementedError):
-        binding.Mech(_mech())
