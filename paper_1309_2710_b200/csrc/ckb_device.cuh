@@ -369,15 +369,23 @@ struct Sys {
           Mc[q] = fma(am1, *reinterpret_cast<const double *>(reinterpret_cast<const char *>(sR + q * RS) + off), Mc[q]);
       }
       const int t = r * L + g;
-      if (m.o_fo) { /* launch-uniform: the mechanism has fall-off reactions (R31) */
-        const int fb = m.o_fo + r * 8 * L + g;
+      if (t < m.NTB) {
+#pragma unroll
+        for (int q = 0; q < M; q++) sR[q * RS + (n + t) * GI] = Mc[q];
+      }
+    }
+    if (m.o_fo) { /* launch-uniform: the mechanism has fall-off reactions (R31).  A second pass, so that mechanisms without
+                     them keep the loop above as it was: the set of a fall-off reaction has its [M] replaced by
+                     P_r/(1+P_r) F (k_j stays k_inf); each lane revisits the sets it wrote itself */
+      for (int r = 0; r < m.NTBR; r++) {
+        const int t = r * L + g, fb = m.o_fo + r * 8 * L + g;
         const int kind = (int)td(fb);
-        if (kind > 0) { /* this set belongs to a fall-off reaction: "[M]" becomes P_r/(1+P_r) F, k_j stays k_inf */
+        if (kind > 0 && t < m.NTB) {
           const ExpConst<false> fec;
           const double dlnA = td(fb + L), dbeta = td(fb + 2 * L), dtheta = td(fb + 3 * L);
 #pragma unroll
           for (int q = 0; q < M; q++) {
-            const double Pr = Mc[q] * ckb_exp(fma(-dtheta, invT[q], fma(dbeta, lnT[q], dlnA)), fec);
+            const double Pr = sR[q * RS + (n + t) * GI] * ckb_exp(fma(-dtheta, invT[q], fma(dbeta, lnT[q], dlnA)), fec);
             double B = Pr / (1.0 + Pr);
             if (kind >= 2) { /* Troe */
               const double a = td(fb + 4 * L);
@@ -388,13 +396,9 @@ struct Sys {
               const double x = (lP + c) / (nn - 0.14 * (lP + c));
               B *= exp(2.302585092994046 * (lF / (1.0 + x * x)));
             }
-            Mc[q] = B;
+            sR[q * RS + (n + t) * GI] = B;
           }
         }
-      }
-      if (t < m.NTB) {
-#pragma unroll
-        for (int q = 0; q < M; q++) sR[q * RS + (n + t) * GI] = Mc[q];
       }
     }
     gsync();
