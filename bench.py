@@ -123,13 +123,15 @@ class GpuCase:
 
     specialize = True   # class-wide switch (--no-specialize)
 
-    def __init__(self, cfg, N, dt, variant="auto", ordering="shuffled", device=0, cv=False):
+    def __init__(self, cfg, N, dt, variant="auto", ordering="shuffled", device=0, cv=False, f1=False):
         import torch
         from paper_1309_2710_b200 import binding
         self.torch, self.binding = torch, binding
         self.spec = synth.CONFIGS[cfg]
         self.cfg, self.N, self.dt, self.variant = cfg, N, dt, variant
         self.mech = synth.make_mechanism(cfg)
+        if f1:   # two-range NASA fits and fall-off reactions on the same mechanism (ckb_mech_load3)
+            self.mech = synth.with_falloff(synth.with_two_range_thermo(self.mech, self.spec.T_range))
         self.m = binding.mech_load(self.mech)
         # mechanism-specialised thread-per-ODE kernels (ckb_mech_specialize) where the mapping applies; if the
         # runtime compiler is missing the table-driven kernels stay in place and the bench line says so
@@ -382,6 +384,24 @@ def run_ours(args):
                 del cs
             except Exception as ex:  # pragma: no cover
                 extra[f"cv_cfg{c}"] = {"error": str(ex)}
+        # two-range thermodynamics + fall-off reactions (ckb_mech_load3) on the same workloads
+        for c in (1, 3):
+            try:
+                s2, N2, dt2 = workload(c)
+                if c == 3:
+                    N2 //= 4   # the fall-off variant of 53/634 needs 7x the f evaluations per system: a quarter batch
+                cs = GpuCase(c, N2, dt2, "auto", f1=True)
+                wk = cs.work()
+                m2 = cs.timed_steps(3, 3)
+                rf = roofline(cs, float(np.mean(m2)), wk, peak_flops / 1e12, "measured DFMA probe")
+                rf["traffic"] = None
+                extra[f"f1_cfg{c}_{s2.method}_auto_N{N2}"] = {
+                    "odes_per_s": N2 / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)), "work": wk, "roofline": rf,
+                    "n_falloff": int(len(cs.mech.fo_reaction))}
+                cs.close()
+                del cs
+            except Exception as ex:  # pragma: no cover
+                extra[f"f1_cfg{c}"] = {"error": str(ex)}
         # the paper's "similar neighbours" experiment: the same systems sorted by T
         try:
             cs = GpuCase(args.config, N, dt, args.variant, "similar")
