@@ -77,6 +77,10 @@ def lib():
         L.ora_rkck_generic.restype = C.c_int
         L.ora_rkc_generic.argtypes = L.ora_rkck_generic.argtypes
         L.ora_rkc_generic.restype = C.c_int
+        L.ora_rkck_trace.argtypes = L.ora_rkck_generic.argtypes + [dp, C.c_int64, C.POINTER(C.c_int64)]
+        L.ora_rkck_trace.restype = C.c_int
+        L.ora_rkc_trace.argtypes = L.ora_rkck_trace.argtypes
+        L.ora_rkc_trace.restype = C.c_int
         L.ora_rkc_coeffs.argtypes = [C.c_int, dp, dp, dp, dp, dp, dp, dp, dp, dp]
         L.ora_rkc_coeffs.restype = C.c_int
         L.ora_rkc_step.argtypes = [RHS_FN, C.c_void_p, C.c_int, C.c_double, dp, C.c_double, C.c_int, dp, dp]
@@ -229,6 +233,32 @@ def rkck_generic(fn, y, t0, t1, rtol, atol):
 
 def rkc_generic(fn, y, t0, t1, rtol, atol):
     return _generic(lib().ora_rkc_generic, fn, y, t0, t1, rtol, atol)
+
+
+TRACE_COLS = ("t", "h", "err", "accepted", "s", "sigma_refreshed", "sigma", "est0")
+
+
+def _trace(entry, fn, y, t0, t1, rtol, atol, cap):
+    y = np.array(y, dtype=np.float64, copy=True)
+    n = len(y)
+    stats = np.zeros(4, dtype=np.int32)
+    rows = np.zeros((cap, len(TRACE_COLS)))
+    nrows = C.c_int64()
+    status = entry(wrap_rhs(fn, n), None, n, _dp(y), float(t0), float(t1), float(rtol), float(atol), _ip(stats),
+                   _dp(rows), cap, C.byref(nrows))
+    assert nrows.value <= cap, "trace buffer too small"
+    tr = rows[: nrows.value]
+    return y, int(status), stats, {k: tr[:, i] for i, k in enumerate(TRACE_COLS)}
+
+
+def rkck_trace(fn, y, t0, t1, rtol, atol, cap=100000):
+    """ora_rkck_generic with its step trace: one entry per attempt (t, h, errmax, accepted, ...)."""
+    return _trace(lib().ora_rkck_trace, fn, y, t0, t1, rtol, atol, cap)
+
+
+def rkc_trace(fn, y, t0, t1, rtol, atol, cap=100000):
+    """ora_rkc_generic with its step trace: one entry per attempt (t, h, err, accepted, s, sigma_refreshed, sigma, est0)."""
+    return _trace(lib().ora_rkc_trace, fn, y, t0, t1, rtol, atol, cap)
 
 
 def spectral_radius(fn, t, y, v=None):

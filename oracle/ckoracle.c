@@ -18,15 +18,23 @@
  *   ora_rkck_step            : y'=lambda y closed form R(z), R*(z); measured order 5 / 4 on y'=-y^2
  *   ora_rkc_coeffs/_step     : stage closed form a_j + b_j T_j(w0 + w1 z) for s = 2..200; Chebyshev bound
  *                              |P_s(z)| <= 1 on [-beta(s), 0]; measured order 2; c_1 = c_2/T_2'(w0)
- *   ora_spectral_radius      : linear operators with known spectrum; FD-Jacobian eigenvalues on chemistry
+ *   ora_spectral_radius      : linear operators with known spectrum; on the 9/13/53-species chemistry: same value and
+ *                              same evaluation count as a textbook power iteration on an explicit central-difference
+ *                              Jacobian, and the distribution of (returned value)/rho(J)
  *   ora_rhs                  : A->B, A->B->C (Bateman), A+B->C+D, A+M->B+M closed forms; Arrhenius in mpmath;
  *                              Sum Y and element mass invariants
  *   ora_rkck/rkc drivers     : tolerance proportionality, brute-force fixed-step reference, RKCK-vs-RKC
- *                              cross-check, linear invariants.
- *   PARITY UNPINNED (builder's reading, nothing in the paper or the mathematics fixes them):
+ *                              cross-check, linear invariants; and from the step traces (ora_rkck_trace /
+ *                              ora_rkc_trace, tests/test_oracle_controllers.py): Eq. 16-17 with both exponents, S and
+ *                              both limits; Eq. 30-32 against the closed form on y' = lambda y; Eq. 33-35
+ *                              incl. the orientation of Eq. 34's memory term and the [0.1, 10] clamp; Eq. 36-38 by
+ *                              hand; Eq. 39 truncated with dt sigma inside the stability interval; the 25-step /
+ *                              after-rejection refresh of sigma.
+ *   PARITY UNPINNED (builder's reading, nothing in the paper or the mathematics fixes them; the traces pin that the
+ *   code does what the reading says, not that the reading is the only possible one):
  *   R4 (RKCK first trial step), R5 (end-of-interval clipping), R6/R7 (failure codes), R10 (b_1 = b_2 for
  *   nonlinear f), R13 (controller memory dropped after a rejection), R14/R15 (initial-step weights and cap),
- *   R16 (sigma refresh rule), R17/R18 (power-method details and its 1.2 safety factor).
+ *   R16 (sigma refreshed after a rejection only when stale), R17/R18 (power-method details and its 1.2 safety factor).
  */
 #include <math.h>
 #include <stdint.h>
@@ -132,8 +140,26 @@ static int all_finite(const double *v, int n) {
  * RKCK driver.  Integrates y from t0 to t1 in place.
  * stats[0]=RHS evaluations, [1]=accepted steps, [2]=rejected steps, [3]=0.  Returns a status code.
  * ---------------------------------------------------------------------------------------------- */
-int ora_rkck_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol,
-                     double atol, int32_t *stats) {
+/* Step trace (test-only; the pins of the step-size controllers read it): one row of ORA_TRACE_COLS doubles per
+ * step ATTEMPT, in order:  [0] t at the start of the attempt, [1] the step size attempted (after the R5 clip / the
+ * R12 cap), [2] the error measure of the attempt (RKCK: errmax of Eq. 17; RKC: ||err|| of Eq. 31), [3] 1 accepted /
+ * 0 rejected, [4] RKC: stages s of the attempt (RKCK: 6), [5] RKC: 1 if the spectral radius was re-estimated for
+ * this attempt (the initial estimate counts for attempt 0), [6] RKC: sigma in use, [7] RKC, attempt 0 only: the
+ * ||est|| of Eq. 37 that produced the first step (else 0).  Recording changes nothing in the arithmetic. */
+#define ORA_TRACE_COLS 8
+typedef struct { double *rows; int64_t cap, n; } ora_trace;
+static void trace_row(ora_trace *tr, double t, double h, double err, int acc, int s, int refreshed, double sigma,
+                      double est0) {
+  if (!tr) return;
+  if (tr->n < tr->cap) {
+    double *r = tr->rows + ORA_TRACE_COLS * (size_t)tr->n;
+    r[0] = t; r[1] = h; r[2] = err; r[3] = acc; r[4] = s; r[5] = refreshed; r[6] = sigma; r[7] = est0;
+  }
+  tr->n++;
+}
+
+static int rkck_driver(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol,
+                       double atol, int32_t *stats, ora_trace *tr) {
   const double S = 0.9;
   const double u = 2.220446049250313e-16;     /* 2^-52 */
   double *buf = (double *)malloc(sizeof(double) * (size_t)n * 9);
@@ -170,6 +196,7 @@ int ora_rkck_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, doubl
       double e = fabs(delta[c]) / d0;
       if (!(e <= errmax)) errmax = e;          /* NaN propagates into errmax */
     }
+    trace_row(tr, t, h, errmax, finite && errmax <= 1.0, 6, 0, 0.0, 0.0);
     if (finite && errmax <= 1.0) {             /* P:139 accept */
       nacc++;
       for (int c = 0; c < n; c++) y[c] = ynew[c];
@@ -202,6 +229,20 @@ int ora_rkck_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, doubl
   if (stats) { stats[0] = nfe; stats[1] = nacc; stats[2] = nrej; stats[3] = 0; }
   free(buf);
   return status;
+}
+
+int ora_rkck_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol,
+                     double atol, int32_t *stats) {
+  return rkck_driver(f, ctx, n, y, t0, t1, rtol, atol, stats, NULL);
+}
+
+/* test entry: the same driver, recording up to cap attempts into rows[cap][ORA_TRACE_COLS]; *n_rows = attempts made */
+int ora_rkck_trace(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol, double atol,
+                   int32_t *stats, double *rows, int64_t cap, int64_t *n_rows) {
+  ora_trace tr = {rows, cap, 0};
+  const int st = rkck_driver(f, ctx, n, y, t0, t1, rtol, atol, stats, &tr);
+  if (n_rows) *n_rows = tr.n;
+  return st;
 }
 
 /* ------------------------------------------------------------------------------------------------
@@ -361,8 +402,8 @@ double ora_spectral_radius(ora_rhs_fn f, void *ctx, int n, double t, const doubl
  * RKC driver: Eq. 30-39 and P:233.  Integrates y from t0 to t1 in place.
  * stats[0]=RHS evaluations, [1]=accepted, [2]=rejected, [3]=largest stage count used.
  * ---------------------------------------------------------------------------------------------- */
-int ora_rkc_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol,
-                    double atol, int32_t *stats) {
+static int rkc_driver(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol,
+                      double atol, int32_t *stats, ora_trace *tr) {
   const double u = 2.220446049250313e-16;
   const double Dt = t1 - t0;
   /* R12: round-off cap on the stage count, s_max = max(2, round(sqrt(rtol/(10 u)))) */
@@ -382,7 +423,7 @@ int ora_rkc_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double
   int sigma_fresh = 1, need_sigma = 0, since_sigma = 0;
 
   /* initial step: Eq. 36-38, R14 weights atol + rtol |y_0|, R15 caps at the global step */
-  double h;
+  double h, est0;
   {
     double h0 = (sigma > 0.0 && 1.0 / sigma < Dt) ? 1.0 / sigma : Dt;      /* Eq. 36 */
     double *z = pw, *g = pw + nn;
@@ -396,6 +437,7 @@ int ora_rkc_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double
       acc += (d0 / wt) * (d0 / wt);
     }
     double est = sqrt(acc / (double)n);                                    /* Eq. 31 */
+    est0 = est;
     h = Dt;
     if (est > 0.0) {
       double h1 = 0.1 * h0 / sqrt(est);                                    /* Eq. 38 */
@@ -409,10 +451,12 @@ int ora_rkc_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double
   int saw_nonfinite = 0;
   while (1) {
     int last = 0;
+    int refreshed = (attempts == 0);
     if (1.1 * h >= t1 - t) { h = t1 - t; last = 1; }                       /* R5 */
     if (need_sigma) {                                                      /* P:233, R16 */
       sigma = spectral_radius(f, ctx, n, t, y, f0, v, 1, &nfe, &flag, pw);
       sigma_fresh = 1; need_sigma = 0; since_sigma = 0;
+      refreshed = 1;
     }
     int s = 1 + (int)floor(sqrt(1.0 + 1.54 * h * sigma));                  /* Eq. 39, R12 truncation */
     if (s < 2) s = 2;
@@ -435,6 +479,7 @@ int ora_rkc_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double
       acc += (del / wt) * (del / wt);
     }
     double err = sqrt(acc / (double)n);
+    trace_row(tr, t, h, err, err <= 1.0, s, refreshed, sigma, attempts == 1 ? est0 : 0.0);
     if (err <= 1.0) {                                                      /* accept */
       nacc++;
       double fac;
@@ -471,6 +516,20 @@ int ora_rkc_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double
   if (stats) { stats[0] = nfe; stats[1] = nacc; stats[2] = nrej; stats[3] = smax_used; }
   free(buf);
   return status;
+}
+
+int ora_rkc_generic(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol,
+                    double atol, int32_t *stats) {
+  return rkc_driver(f, ctx, n, y, t0, t1, rtol, atol, stats, NULL);
+}
+
+/* test entry: the same driver with the step trace (see ora_rkck_trace) */
+int ora_rkc_trace(ora_rhs_fn f, void *ctx, int n, double *y, double t0, double t1, double rtol, double atol,
+                  int32_t *stats, double *rows, int64_t cap, int64_t *n_rows) {
+  ora_trace tr = {rows, cap, 0};
+  const int st = rkc_driver(f, ctx, n, y, t0, t1, rtol, atol, stats, &tr);
+  if (n_rows) *n_rows = tr.n;
+  return st;
 }
 
 /* ================================================================================================

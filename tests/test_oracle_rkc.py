@@ -186,3 +186,115 @@ def test_driver_tolerance_proportionality():
 def test_driver_nonfinite_fails_cleanly():
     y, status, st = oracle.rkc_generic(lambda t, y: np.array([np.nan]), [1.0], 0.0, 1.0, 1e-6, 1e-12)
     assert status in (3, 4) and y[0] == 1.0 and st[1] == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# Power method on chemistry (SURVEY C7 "Power method" row).  Harness only: a central-difference Jacobian of the
+# oracle's source term and numpy's dense eigenvalues / matrix products.
+# ------------------------------------------------------------------------------------------------
+def _fd_jacobian(om, y0, p):
+    n = len(y0)
+    J = np.empty((n, n))
+    for c in range(n):
+        h = 1e-6 * max(abs(y0[c]), 1e-3)
+        yp, ym = y0.copy(), y0.copy()
+        yp[c] += h
+        ym[c] -= h
+        J[:, c] = (om.rhs(yp, p) - om.rhs(ym, p)) / (2.0 * h)
+    return J
+
+
+def _textbook_power_iteration(J, f0):
+    """Plain power iteration on the MATRIX J from the start vector f(y): sigma_k = ||J v||, v <- J v / sigma_k, stopped
+    when two successive values agree to 1 % (k >= 2) or after 50 products; what the nonlinear method of [48] reduces to
+    when f is replaced by its linearisation.  Returns (1.2 sigma, k, converged, distance of the closest call to 1 %)."""
+    v = f0 / np.linalg.norm(f0)
+    sig, margin = 0.0, np.inf
+    for k in range(1, 51):
+        w = J @ v
+        prev, sig = sig, np.linalg.norm(w)
+        if k >= 2:
+            margin = min(margin, abs(abs(sig - prev) / sig - 0.01))
+            if abs(sig - prev) <= 0.01 * sig:
+                return 1.2 * sig, k, True, margin
+        v = w / sig
+    return 1.2 * sig, 50, False, margin
+
+
+@pytest.mark.parametrize("cfg,N", [(0, 48), (2, 64), (3, 6)])
+def test_power_method_on_chemistry_is_power_iteration_on_the_fd_jacobian(cfg, N):
+    """The nonlinear power method (finite displacement d = ||y|| sqrt(u) along v, sigma = ||f(z) - f(y)|| / d, R17) on
+    the chemistry source term gives the same value after the same number of evaluations as the textbook iteration on an
+    explicitly formed Jacobian -- an independent route to the same numbers: a wrong displacement, norm, stopping rule,
+    iteration count or safety factor (R18) shows up here."""
+    from paper_1309_2710_b200 import synth
+    mech = synth.make_mechanism(cfg)
+    om = oracle.OracleMech(mech)
+    states, p = synth.make_states(cfg, N)
+    compared = 0
+    for i in range(N):
+        y0 = states[:, i].copy()
+        J = _fd_jacobian(om, y0, p)
+        sig, v, nfe, flag = oracle.spectral_radius(lambda t, y: om.rhs(y, p), 0.0, y0)
+        ref, k, conv, margin = _textbook_power_iteration(J, om.rhs(y0, p))
+        if margin < 6e-4:
+            continue                       # a stopping decision within 0.06 % of the 1 % threshold may fall either way
+        compared += 1
+        assert nfe == k and (flag == 4) == (not conv), (i, nfe, k, flag, conv)
+        assert abs(sig / ref - 1.0) < 2e-3, (i, sig, ref)
+    assert compared >= 0.6 * N
+
+
+@pytest.mark.parametrize("cfg,N,frac_in,lo_bound", [(1, 160, 0.93, 0.3), (2, 160, 0.75, 0.05)])
+def test_power_method_on_chemistry_against_the_spectral_radius(cfg, N, frac_in, lo_bound):
+    """Returned value / rho(J) on the 9- and 13-species mechanisms.  Measured (seed 0): the median is the safety factor
+    1.2 to three digits and 94 % / 80 % of the systems lie in [1.0, 1.3]; the rest are the known weakness of a power
+    iteration stopped by a two-iterate 1 % test on a strongly non-normal Jacobian (T in kelvin beside mass fractions):
+    the value stalls below (min 0.49 / 0.11) or, being a quotient ||J v|| / ||v|| and not an eigenvalue, above rho
+    (max 1.38 / 1.92).  So 1.2 x sigma is NOT a bound of the spectrum for every system, status 4 or not (status-4
+    systems of 13/54: 0.57 .. 1.21) -- see DESIGN.md 4.5: the reading follows [48], and an under-staged step is caught
+    by the error control (rejection -> warm re-estimate, R16).  The asserts hold these measured facts."""
+    from paper_1309_2710_b200 import synth
+    mech = synth.make_mechanism(cfg)
+    om = oracle.OracleMech(mech)
+    states, p = synth.make_states(cfg, N)
+    ratio, flags = [], []
+    for i in range(N):
+        y0 = states[:, i].copy()
+        rho = np.abs(np.linalg.eigvals(_fd_jacobian(om, y0, p))).max()
+        sig, v, nfe, flag = oracle.spectral_radius(lambda t, y: om.rhs(y, p), 0.0, y0)
+        ratio.append(sig / rho)
+        flags.append(flag)
+    ratio, flags = np.array(ratio), np.array(flags)
+    assert 1.19 < np.median(ratio) < 1.21, np.median(ratio)
+    assert np.mean((ratio >= 1.0) & (ratio <= 1.3)) >= frac_in, np.mean((ratio >= 1.0) & (ratio <= 1.3))
+    assert ratio.min() > lo_bound and ratio.max() < 2.5, (ratio.min(), ratio.max())
+    if cfg == 2:
+        assert 2 <= np.sum(flags == 4) <= 0.12 * N                     # DESIGN.md 5: ~6 % of the 13/54 systems
+        assert ratio[flags == 4].min() > 0.4
+
+
+def test_underestimated_sigma_is_harmless_on_the_configs():
+    """The 13/54 systems whose first estimate is furthest below rho(J), and the status-4 ones: the RKC result still
+    agrees with an RKCK run at rtol 1e-11 to the accumulated local tolerance, accepted steps x (rtol |y| + atol), with
+    the same constant every other system of the config needs (measured: <= 1.4; steps are accuracy-limited, s = 2)."""
+    from paper_1309_2710_b200 import synth
+    cfg, N = 2, 96
+    mech = synth.make_mechanism(cfg)
+    om = oracle.OracleMech(mech)
+    states, p = synth.make_states(cfg, N)
+    ratio, flags = [], []
+    for i in range(N):
+        y0 = states[:, i].copy()
+        rho = np.abs(np.linalg.eigvals(_fd_jacobian(om, y0, p))).max()
+        sig, v, nfe, flag = oracle.spectral_radius(lambda t, y: om.rhs(y, p), 0.0, y0)
+        ratio.append(sig / rho)
+        flags.append(flag)
+    pick = np.unique(np.concatenate([np.argsort(ratio)[:6], np.nonzero(np.array(flags) == 4)[0]]))
+    sub = states[:, pick]
+    rtol, atol = 1e-8, 1e-12
+    y_rkc, st_rkc, stats = om.integrate(sub, p, 1e-6, rtol, atol, "rkc")
+    y_ref, st_ref, _ = om.integrate(sub, p, 1e-6, 1e-11, 1e-15, "rkck")
+    assert np.all(st_ref == 0) and np.all((st_rkc == 0) | (st_rkc == 4))
+    err = (np.abs(y_rkc - y_ref) / (rtol * np.abs(y_ref) + atol)).max(axis=0) / stats[1]
+    assert err.max() < 2.0, err
