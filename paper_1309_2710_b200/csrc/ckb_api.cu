@@ -40,6 +40,7 @@ namespace {
 struct Launch {
   int L, NV;
   bool param_tab;
+  bool big = false; /* thread-per-ODE with memory-resident stage vectors (K+1 > 16, ckb_thread.cu) */
 };
 
 /* AUTO, from the variant map measured on B200: mechanisms with K+1 <= 16 go thread-per-ODE once the batch fills
@@ -71,6 +72,11 @@ int choose(const ckb_mech *m, int variant, long long N, int method, Launch *out)
       variant = CKB_VARIANT_WARP;
   }
   int L;
+  if (variant == CKB_VARIANT_THREAD && n > 16) {
+    if (!m->tp) return CKB_EUNSUPPORTED;
+    out->L = 1; out->NV = 0; out->param_tab = false; out->big = true;
+    return m->tp->rc;
+  }
   switch (variant) {
     case CKB_VARIANT_THREAD: L = 1; break;
     case CKB_VARIANT_SUB8: L = 8; break;
@@ -90,6 +96,7 @@ int choose(const ckb_mech *m, int variant, long long N, int method, Launch *out)
 
 /* thread-per-ODE launches go to the mechanism-specialised kernels once ckb_mech_specialize() has built them */
 int dispatch_integrate(const ckb_mech *m, const Launch &l, int method, const ckb_host::IntegrateArgs &a) {
+  if (l.big) return ckb_host::thread_integrate(m, method, a);
   if (l.L == 1 && m->gen.ok) return ckb_host::gen_integrate(m, method, a);
 #define X(L_, NV_) \
   if (l.L == L_ && l.NV == NV_) return ckb_host::integrate_L##L_##_NV##NV_(m, method, a);
@@ -104,11 +111,13 @@ int dispatch_proxy(const ckb_mech *m, const Launch &l, const ckb_host::ProxyArgs
 #define X(L_, NV_) \
   if (l.L == L_ && l.NV == NV_) return ckb_host::proxy_L##L_##_NV##NV_(m, a);
   CKB_FOR_THREAD(X)
+  CKB_FOR_WARP(X)
 #undef X
   return CKB_EUNSUPPORTED;
 }
 
 int dispatch_rhs(const ckb_mech *m, const Launch &l, const ckb_host::RhsArgs &a) {
+  if (l.big) return ckb_host::thread_rhs(m, a);
   if (l.L == 1 && m->gen.ok) return ckb_host::gen_rhs(m, a);
 #define X(L_, NV_) \
   if (l.L == L_ && l.NV == NV_) return ckb_host::rhs_L##L_##_NV##NV_(m, a);
@@ -148,6 +157,13 @@ int ckb_mech_load3(const ckb_mech_desc *d, const double *nasa_high, const double
     delete m;
     return rc;
   }
+  if (m->tp) {
+    rc = ckb_host::thread_upload(*m->tp);
+    if (rc != CKB_OK) {
+      ckb_mech_free(m);
+      return rc;
+    }
+  }
   cudaError_t e = cudaMalloc((void **)&m->d_counters, CKB_COUNTER_RING * 8);
   for (int i = 0; i < CKB_NPACK && e == cudaSuccess; i++) {
     ckb_host::Packed &p = m->pk[i];
@@ -167,6 +183,7 @@ void ckb_mech_free(ckb_mech *m) {
   if (!m) return;
   for (int i = 0; i < CKB_NPACK; i++)
     if (m->pk[i].d_blob) cudaFree(m->pk[i].d_blob);
+  if (m->tp) ckb_host::thread_free(*m->tp);
   ckb_host::gen_unload(m);
   if (m->d_counters) cudaFree(m->d_counters);
   for (int i = 0; i < CKB_SCRATCH_SLOTS; i++) {
@@ -212,10 +229,12 @@ static int integrate_impl(const ckb_mech *m, double *states, const double *press
                             status, stats, stream, nullptr, cv};
   /* queue order: hottest systems first (row 0 of states = T); pointless when every system starts at once */
   if (N >= 4096) {
-    if (l.L <= 4 && method == CKB_METHOD_RKC && m->pk[0].rc == CKB_OK) {
+    const ckb_host::Packed &pk32 = m->pk[ckb_host::pack_index(32)];
+    if (l.L <= 4 && method == CKB_METHOD_RKC && (m->pk[0].rc == CKB_OK || pk32.rc == CKB_OK)) {
       /* RKC with 8 or more systems per warp: order by the cost proxy || J f / wt || (two evaluations of f per
-       * system, computed by the thread-per-ODE kernel whatever mapping integrates) */
-      const Launch l1{1, m->pk[0].dm.NV, true};
+       * system, computed by the register-resident thread-per-ODE kernel whatever mapping integrates; mechanisms
+       * beyond 16 unknowns: by the warp-per-ODE one) */
+      const Launch l1 = m->pk[0].rc == CKB_OK ? Launch{1, m->pk[0].dm.NV, true} : Launch{32, pk32.dm.NV, false};
       rc = ckb_host::queue_scratch(m, slot, N);
       if (rc) return rc;
       ckb_host::ProxyArgs pa{states, pressure, p_uniform, (long long)N, (long long)ld, 1e-3 * dt, rtol, atol,

@@ -62,6 +62,23 @@ void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<
 struct FoDesc { int n; const int32_t *reaction; const double *low3, *troe4; };
 int parse_mechanism(const ckb_mech_desc *d, Parsed &P, const FoDesc *fo = nullptr);
 int pack_for(const Parsed &P, int L, Packed &out);
+/* RKC coefficients of an s-stage step (Eq. 22-26): mu~_1, then (mu_j, nu_j, mu~_j, gamma~_j) for j = 2..s */
+void rkc_stage_coefficients(int s, double *mut1, double *stages);
+
+/* thread-per-ODE packing for mechanisms with more than 16 unknowns (ckb_thread.cu) */
+struct ThreadPack {
+  ckbt::DevThread dm{};
+  std::vector<unsigned long long> slots, aux; /* class directory + slot streams; species / sets / RKC tables */
+  unsigned long long *d_slots = nullptr, *d_aux = nullptr;
+  double *d_ws = nullptr;                     /* stage vectors of the resident grid: [CKBT_VECS][n][ws_threads] */
+  size_t ws_threads = 0, smem = 0;
+  int warps = 0, sms = 0;
+  bool param = false;                         /* the slot table travels as a kernel parameter (constant bank) */
+  int rc = CKB_EUNSUPPORTED;
+};
+int pack_thread(const Parsed &P, ThreadPack &out);
+int thread_upload(ThreadPack &tp);
+void thread_free(ThreadPack &tp);
 int load_packings(const ckb_mech_desc *d, const double *nasa_high, const double *T_mid, const FoDesc *fo, ckb_mech *m);
 #define CKB_NPACK 6
 inline int pack_index(int L) { return L == 1 ? 0 : L == 8 ? 1 : L == 16 ? 2 : L == 32 ? 3 : L == 2 ? 4 : 5; }
@@ -82,6 +99,7 @@ struct GenKernels {
 
 struct ckb_mech {
   std::shared_ptr<ckb_host::Parsed> parsed; /* kept for ckb_mech_specialize */
+  std::unique_ptr<ckb_host::ThreadPack> tp; /* K+1 > 16: thread-per-ODE with memory-resident stage vectors */
   ckb_host::GenKernels gen;
   ckb_host::Packed pk[CKB_NPACK]; /* L = 1, 8, 16, 32, 2, 4 (pack_index) */
   int K = 0, R = 0, NS = 0;
@@ -130,6 +148,7 @@ struct RhsArgs {
 
 /* the instantiation list: (lanes per system L, register slots per lane NV); a system needs K+1 <= L*NV */
 #define CKB_FOR_THREAD(X) X(1, 4) X(1, 10) X(1, 14) X(1, 16)
+#define CKB_FOR_WARP(X) X(32, 1) X(32, 2) X(32, 4) /* the warp-per-ODE subset of CKB_FOR_GROUP (cost-proxy kernels) */
 #define CKB_FOR_GROUP(X) X(2, 5) X(2, 8) X(4, 3) X(4, 4) X(8, 7) X(8, 14) X(16, 4) X(16, 7) X(32, 1) X(32, 2) X(32, 4)
 
 /* smallest instantiated NV that holds n unknowns on L lanes, or -1 */
@@ -142,6 +161,10 @@ inline int pick_nv(int L, int n) {
 #undef X
   return best;
 }
+
+/* ckb_thread.cu */
+int thread_integrate(const ckb_mech *m, int method, const IntegrateArgs &a);
+int thread_rhs(const ckb_mech *m, const RhsArgs &a);
 
 /* ckb_gen.cu */
 std::string generate_rhs(const Parsed &P);

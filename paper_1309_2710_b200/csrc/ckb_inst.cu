@@ -119,7 +119,7 @@ int CKB_CAT(rhs_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const RhsArgs &a) {
 }
 
 int CKB_CAT(proxy_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const ProxyArgs &a) {
-#if CKB_L == 1
+#if CKB_L == 1 || CKB_L == 32
   auto kern = a.cv ? ckb::cost_proxy_kernel<L, NV, Tab, 1> : ckb::cost_proxy_kernel<L, NV, Tab, 0>;
   const size_t smem = smem_bytes(m, 1, ckb::Sys<L, NV, Tab, 1>::HDOUBLES);
   int rc = prep(kern, smem);
@@ -134,7 +134,7 @@ int CKB_CAT(proxy_L, CKB_L, _NV, CKB_NV)(const ckb_mech *m, const ProxyArgs &a) 
   return CKB_OK;
 #else
   (void)m; (void)a;
-  return CKB_EUNSUPPORTED; /* the proxy order is only used by thread-per-ODE */
+  return CKB_EUNSUPPORTED; /* the proxy is computed thread-per-ODE (K+1 <= 16) or warp-per-ODE */
 #endif
 }
 

@@ -177,7 +177,7 @@ int parse_mechanism(const ckb_mech_desc *d, Parsed &P, const FoDesc *fo) {
 
 /* RKC coefficients of an s-stage step, Eq. 22-26 with R8 (w0 = 1 + (2/13)/s^2), R9
  * (a_j = 1 - b_j T_j(w0)) and R10 (b_0 = b_1 = b_2).  out: mu~_1, then (mu_j, nu_j, mu~_j, gamma~_j), j = 2..s. */
-static void rkc_coefficients(int s, double *mut1, double *stages) {
+void rkc_stage_coefficients(int s, double *mut1, double *stages) {
   std::vector<double> T(s + 1), dT(s + 1), d2T(s + 1), b(s + 1), a(s + 1);
   const double w0 = 1.0 + (2.0 / 13.0) / ((double)s * (double)s);
   T[0] = 1.0; T[1] = w0; dT[0] = 0.0; dT[1] = 1.0; d2T[0] = 0.0; d2T[1] = 0.0;
@@ -628,7 +628,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   for (int s = 2; s <= s_tab; s++) {
     double mut1;
     std::vector<double> st(4 * (size_t)(s - 1));
-    rkc_coefficients(s, &mut1, st.data());
+    rkc_stage_coefficients(s, &mut1, st.data());
     putd(m.o_rkc + (s - 2), mut1);
     const int base = m.o_rkcs + 4 * ((s - 2) * (s - 1) / 2);
     for (size_t q = 0; q < st.size(); q++) putd(base + (int)q, st[q]);
@@ -665,6 +665,11 @@ int load_packings(const ckb_mech_desc *d, const double *nasa_high, const double 
     if (pk.rc == CKB_OK && Ls[i] == 1 && pk.dm.words > CKB_PARAM_WORDS) pk.rc = CKB_EUNSUPPORTED;
     if (pk.rc != CKB_OK) pk.blob.clear();
     any = any || pk.rc == CKB_OK;
+  }
+  if (P.K + 1 > 16) { /* thread-per-ODE beyond the register-resident kernels */
+    m->tp.reset(new ThreadPack());
+    if (pack_thread(P, *m->tp) != CKB_OK) m->tp.reset();
+    any = any || m->tp;
   }
   return any ? CKB_OK : CKB_EUNSUPPORTED;
 }

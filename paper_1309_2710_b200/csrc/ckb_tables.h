@@ -94,3 +94,46 @@ __host__ __device__ __forceinline__ int region_doubles(const DevMech &m) {
 }
 
 }  // namespace ckb
+
+/* ------------------------------------------------------------------------------------------------
+ * Thread-per-ODE for mechanisms with more than 16 unknowns (ckb_thread.cuh)
+ * ---------------------------------------------------------------------------------------------- */
+namespace ckbt {
+
+/* slot tables: 64-bit words read with a warp-uniform index */
+#define CKBT_PARAM_WORDS 3840 /* 30 KB of the 32 764-byte kernel-parameter space */
+struct SlotParamTab {
+  unsigned long long w[CKBT_PARAM_WORDS];
+  __device__ __forceinline__ unsigned long long ld(int i) const { return w[i]; }
+};
+typedef ckb::GlobalTab SlotGlobalTab;
+
+/* a regular slot: 8 words (ckb_tables.h CKB_SL_*): ln A_f, beta_f, theta_f, ln A_r, beta_r, theta_r,
+ *   idx A = byte offsets (component * 256) of the reactant molecules in fields 0..2, efficiency-set index in field 3
+ *   idx B = byte offsets of the product molecules in fields 0..2
+ * Every molecule of a regular slot is a different species (reactants AND products), so Eq. 3 is -q on the reactant
+ * offsets and +q on the product offsets, read-modify-write with all reads first.
+ * An irregular slot (a species twice on one side, or on both sides): 12 words = the 8 above with the molecule counts in
+ * field 3 of idx B (nA | nB << 2 | has_tb << 4), then 4 words holding up to 8 scatter entries
+ * (int16 net coefficient << 16 | byte offset), unused entries 0. */
+#define CKBT_SLOT_WORDS 8
+#define CKBT_IRR_WORDS 12
+#define CKBT_KIND_IRREGULAR 18 /* kinds 0..17: (nA-1)*6 + (nB-1)*2 + tb */
+
+struct DevThread {
+  int K, n;
+  int ncls;      /* class directory in the slot table: [ncls][2] = (kind | count << 32, first word) */
+  int o_cls;
+  /* in the aux blob (global memory, broadcast loads): */
+  int o_sp;      /* [K][13] species table (CKB_SP_*), species order = state row order */
+  int o_sp2;     /* [K][13] high temperature range, T_mid in the CKB_SP_INVW word; 0 = one range (R30) */
+  int o_set;     /* [NTB][2]: (first word of the entries, count | fo word << 32); entries (alpha-1, byte offset) */
+  int o_rkc, o_rkcs, s_tab;
+  int NS, NTB;
+  int has_fo;
+};
+
+#define CKBT_VECS 8 /* physical stage vectors per thread in the workspace */
+#define CKBT_VB 9   /* components per batch of a pass over a stage vector (loads in flight per input vector) */
+
+}  // namespace ckbt

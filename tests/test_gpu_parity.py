@@ -98,6 +98,9 @@ CASES = [
     (4, 96, 1e-6, "warp"),
     (4, 48, 1e-5, "warp"),
     (4, 40, 1e-6, "sub8"),
+    (3, 300, 1e-6, "thread"),     # K+1 > 16: thread-per-ODE with memory-resident stage vectors
+    (4, 150, 1e-6, "thread"),
+    (4, 48, 1e-5, "thread"),
 ]
 
 
@@ -116,7 +119,7 @@ def test_parity_configs(cfg, N, dt, variant):
 
 @pytest.mark.parametrize("cfg,method,variant", [(0, "rkc", "thread"), (2, "rkck", "thread"), (0, "rkc", "warp"),
                                                 (3, "rkck", "warp"), (0, "rkc", "sub4"), (2, "rkck", "sub2"),
-                                                (0, "rkc", "gen"), (2, "rkck", "gen")])
+                                                (0, "rkc", "gen"), (2, "rkck", "gen"), (3, "rkck", "thread")])
 def test_parity_other_method(cfg, method, variant):
     """Both integrators on the mechanisms they are not the headline of (RKC on the nonstiff one, RKCK on stiff ones)."""
     mech = synth.make_mechanism(cfg)
@@ -133,6 +136,9 @@ def test_parity_other_method(cfg, method, variant):
     (2, 300, 1e-4, 1e-6, 1e-10, "gen"),       # and 1e-4 s
     (4, 24, 1e-4, 1e-6, 1e-10, "warp"),       # the ethylene-sized mechanism at 1e-4 s: tens of stages, rejections
     (4, 16, 1e-3, 1e-6, 1e-10, "sub16"),      # stage counts beyond the precomputed coefficient table
+    (3, 128, 1e-6, 1e-6, 1e-10, "thread"),
+    (4, 40, 1e-4, 1e-6, 1e-10, "thread"),     # tens of stages, rejections, sigma refreshes
+    (4, 16, 1e-3, 1e-6, 1e-10, "thread"),     # beyond the coefficient table
 ])
 def test_parity_paper_settings(cfg, N, dt, rtol, atol, variant):
     """the tolerances and global steps the paper itself used, not BASELINE.json's."""
@@ -202,8 +208,8 @@ def test_source_term_parity():
     import torch
     import oracle
     from paper_1309_2710_b200 import binding
-    for cfg, variants in ((0, ("thread", "warp", "sub8", "sub2", "sub4")), (2, ("thread", "sub16", "sub2", "sub4")), (3, ("warp", "sub8", "sub16")),
-                          (4, ("warp", "sub8"))):
+    for cfg, variants in ((0, ("thread", "warp", "sub8", "sub2", "sub4")), (2, ("thread", "sub16", "sub2", "sub4")), (3, ("warp", "sub8", "sub16", "thread")),
+                          (4, ("warp", "sub8", "thread"))):
         mech = synth.make_mechanism(cfg)
         om = oracle.OracleMech(mech)
         states, p = synth.make_states(cfg, 70)
