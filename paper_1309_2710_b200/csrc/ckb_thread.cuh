@@ -82,9 +82,17 @@ struct TSys {
   }
   /* stage-vector accesses go to L2 directly (ld/st.global.cg): they have no reuse in L1, and the few KB of L1 that the
    * shared regions leave stay with the species / coefficient tables */
+  /* a load the compiler keeps where it is written (it would otherwise sink every load of a batch down to its first use
+   * and run the batch at one memory latency per component) */
+  __device__ __forceinline__ static double ld_pinned(const double *p) {
+    double x;
+    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(x) : "l"(p) : "memory");
+    return x;
+  }
   struct VRef {
     double *p;
     __device__ __forceinline__ operator double() const { return __ldcg(p); }
+    __device__ __forceinline__ double pinned() const { return ld_pinned(p); }
     __device__ __forceinline__ void operator=(double x) const { __stcg(p, x); }
     __device__ __forceinline__ void operator*=(double x) const { __stcg(p, __ldcg(p) * x); }
   };
@@ -106,7 +114,7 @@ struct TSys {
       for (int u = 0; u < CKBT_VB; u++) {
         const int i = min(i0 + u, n - 1);
 #pragma unroll
-        for (int q = 0; q < NIN; q++) x[u][q] = V(vin[q], i);
+        for (int q = 0; q < NIN; q++) x[u][q] = V(vin[q], i).pinned();
       }
 #pragma unroll
       for (int u = 0; u < CKBT_VB; u++)
@@ -178,6 +186,9 @@ struct TSys {
         xs[2 * u + 1] = fma(-CKBT_WD(CKB_SL_THR), invT, fma(CKBT_WD(CKB_SL_BR), lnT, CKBT_WD(CKB_SL_LNAR)));
 #undef CKBT_WD
       }
+      double Mt[U];
+#pragma unroll
+      for (int u = 0; u < U; u++) Mt[u] = TB ? third_body((int)(w[u][CKB_SL_IDXA] >> 48), ctot, T, invT, lnT) : 1.0;
       ckb::ckb_exp_n<2 * U>(xs, ks, ec);
       /* Eq. 3 of the previous trip */
 #pragma unroll
@@ -195,7 +206,7 @@ struct TSys {
 #pragma unroll
       for (int u = 0; u < U; u++) {
         double q = fma(ks[2 * u], pf[u], -(ks[2 * u + 1] * pr[u])); /* Eq. 4-5, net rate of the pair */
-        if (TB) q *= third_body((int)(w[u][CKB_SL_IDXA] >> 48), ctot, T, invT, lnT);
+        if (TB) q *= Mt[u];
         qp[u] = (r + u < count) ? q : 0.0;
 #pragma unroll
         for (int x = 0; x < 3; x++) { pa[u][x] = a[u][x]; pb[u][x] = b[u][x]; }
@@ -248,11 +259,11 @@ struct TSys {
     for (int k0 = 0; k0 < K; k0 += CKBT_VB) {
       double Yb[CKBT_VB];
 #pragma unroll
-      for (int u = 0; u < CKBT_VB; u++) Yb[u] = V(vec, 1 + min(k0 + u, K - 1));
+      for (int u = 0; u < CKBT_VB; u++) Yb[u] = V(vec, 1 + min(k0 + u, K - 1)).pinned();
 #pragma unroll
       for (int u = 0; u < CKBT_VB; u++) {
-      const int k = k0 + u;
-      if (k >= K) break;
+      const int k = min(k0 + u, K - 1); /* past the end: the last species again, contributing nothing */
+      const bool live = k0 + u < K;
       const int b = m.o_sp + k * CKB_SP_WORDS;
       int bt = b;
       if (m.o_sp2) {
@@ -262,8 +273,8 @@ struct TSys {
       double cp = ad(bt + CKB_SP_CP + 4);
 #pragma unroll
       for (int q = 3; q >= 0; q--) cp = fma(cp, T, ad(bt + CKB_SP_CP + q));
-      const double v = Yb[u] * ad(b + CKB_SP_INVW); /* Y_k / W_k */
-      C((1 + k) * 256u) = v;
+      const double v = live ? Yb[u] * ad(b + CKB_SP_INVW) : 0.0; /* Y_k / W_k */
+      if (live) C((1 + k) * 256u) = v;
       s1 += v;
       s2 = fma(v, cp, s2);
       }
@@ -294,7 +305,7 @@ struct TSys {
     }
     /* Eq. 2: dY_k/dt = W_k omega_k / rho;  Eq. 6 / R29: dT/dt from sum_k (h_k/RT [- 1]) omega_k */
     double s3 = 0.0;
-#pragma unroll 2
+#pragma unroll 6
     for (int k = 0; k < K; k++) {
       const int b = m.o_sp + k * CKB_SP_WORDS;
       int bt = b;
