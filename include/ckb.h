@@ -33,6 +33,7 @@ extern "C" {
 #define CKB_ENOMEM (-2)       /* host or device allocation failed                                    */
 #define CKB_ECUDA (-3)        /* a CUDA runtime call failed; text via ckb_last_cuda_error()          */
 #define CKB_EUNSUPPORTED (-4) /* mechanism outside the packed format's limits (see ckb_mech_load)    */
+#define CKB_ECAPACITY (-5)    /* batch larger than the size reserved for the handle (ckb_mech_reserve) */
 
 #define CKB_METHOD_RKCK 0
 #define CKB_METHOD_RKC 1
@@ -87,11 +88,28 @@ typedef struct ckb_mech ckb_mech; /* opaque; owns the packed tables in device me
  * reverse reactions over the same species are fused into one slot; species-major gather lists for
  * Eq. 3; third-body efficiency sets), upload them to the current CUDA device, and return a handle in
  * *out (library-owned; release with ckb_mech_free).  Synchronous.
- * Limits (CKB_EUNSUPPORTED): K <= 254; at most 3 molecules (sum of nu) on either side of a reaction;
- * at most 65534 fused reaction slots; at most 65534 distinct third-body efficiency sets.
+ * It also allocates everything ckb_integrate will ever need for this handle: the work-queue order scratch for
+ * batches of up to CKB_DEFAULT_MAX_BATCH systems (12 bytes per system; ckb_mech_reserve changes the size) and, for
+ * mechanisms with K+1 > 16, the stage-vector workspace of the thread-per-ODE variant (64 (K+1) bytes per resident
+ * lane: 131 MB for K = 53 on a 148-SM device).
+ * Limits (CKB_EUNSUPPORTED): K <= 254; at most 3 molecules (sum of nu) on either side of a reaction; at most 65000
+ * distinct third-body efficiency sets; per mapping, the shared-memory region of a system is addressed with 16-bit
+ * byte offsets: (K+1 + sets + fused reaction slots rounded up to the lanes per system + 16) * 8 <= 65535 for the
+ * lane-distributed mappings (about 8100 fused slots), 32 times less for the register-resident thread-per-ODE mapping
+ * (K+1 <= 16); a mapping that does not fit is unavailable (CKB_EUNSUPPORTED from ckb_integrate for that variant).
  */
 int ckb_mech_load(const ckb_mech_desc *d, ckb_mech **out);
 void ckb_mech_free(ckb_mech *m);
+
+/*
+ * ckb_mech_reserve: size the handle's work-queue order scratch for batches of up to max_batch systems (the paper's
+ * "global step over all grid points"; "any scratch is sized at load time or passed by the
+ * caller").  Synchronises the device and (re)allocates; call it between steps, never concurrently with work on the
+ * handle.  ckb_integrate refuses a batch beyond the reserved size with CKB_ECAPACITY (batches below 4096 systems need
+ * no scratch).
+ */
+#define CKB_DEFAULT_MAX_BATCH (1 << 20)
+int ckb_mech_reserve(ckb_mech *m, int64_t max_batch);
 
 /*
  * ckb_mech_load2: ckb_mech_load for NASA fits with two temperature ranges ("thermodynamic properties are
@@ -161,10 +179,13 @@ const char *ckb_codegen_log(void); /* compiler log of the calling thread's last 
  *   stats    DEVICE  [4][N] int32 or NULL: f(y) evaluations, accepted steps, rejected steps, largest
  *                    RKC stage count (0 for RKCK).
  *   stream           cudaStream_t as void* (NULL = legacy default stream).
- * Asynchronous on `stream`: never synchronises, allocates nothing.  Stateless between calls.
- * N == 0 is a no-op.  Errors: CKB_EINVAL for bad arguments, CKB_EUNSUPPORTED if the variant cannot hold
- * the mechanism (thread-per-ODE and the 2- / 4-lane variants need K+1 <= 16, the others K+1 <= 4, 7 or 14 times
- * the lanes per system, see ckb_host.h),
+ * Asynchronous on `stream`: never synchronises, allocates nothing (all scratch belongs to the handle and was sized by
+ * ckb_mech_load / ckb_mech_reserve).  No state is carried from one call to the next, but calls on ONE handle
+ * share that scratch (queue order; stage vectors of the thread-per-ODE variant for K+1 > 16): they must be
+ * stream-ordered -- same stream, or ordered by events.  For concurrent calls on several streams load one handle per
+ * stream.  N == 0 is a no-op.  Errors: CKB_EINVAL for bad arguments, CKB_ECAPACITY for N beyond the reserved batch
+ * size, CKB_EUNSUPPORTED if the variant cannot hold the mechanism (the 2- / 4-lane variants need K+1 <= 16, the 8-,
+ * 16- and 32-lane ones K+1 <= 14, 7 or 4 times the lanes per system, see ckb_host.h; thread-per-ODE takes any K),
  * CKB_ECUDA if the launch failed.
  */
 int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, double p_uniform,
@@ -189,7 +210,7 @@ int ckb_integrate_host(ckb_mech *m, double *states, const double *pressure, doub
  * and the pressure follows from the ideal-gas law.  ckb_integrate_cv / ckb_integrate_host_cv / ckb_rhs_cv are
  * ckb_integrate / ckb_integrate_host / ckb_rhs with `density` (DEVICE resp. HOST [N], g/cm^3, or NULL to use
  * rho_uniform > 0) in place of the pressure; every other argument, the layouts, the mapping variants, the
- * asynchrony and the error behaviour are the same.  The same kernels run (the closure is a launch-uniform flag).
+ * asynchrony and the error behaviour are the same.  The same kernel templates run (the closure is a compile-time parameter).
  */
 int ckb_integrate_cv(const ckb_mech *m, double *states, const double *density, double rho_uniform, int64_t N,
                      int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,

@@ -14,7 +14,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libckb.so")
 
-OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ECAPACITY = 0, -1, -2, -3, -4, -5
 METHODS = {"rkck": 0, "rkc": 1}
 VARIANTS = {"auto": 0, "thread": 1, "warp": 2, "sub8": 3, "sub16": 4, "sub2": 5, "sub4": 6}
 ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
@@ -23,7 +23,8 @@ ST_OK, ST_MAXSTEPS, ST_UNDERFLOW, ST_NONFINITE, ST_SIGMA = 0, 1, 2, 3, 4
 EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "ckb_integrate_host",
            "ckb_rhs", "ckb_fp64_probe", "ckb_mech_pack_stats", "ckb_strerror", "ckb_last_cuda_error",
            "ckb_mech_specialize", "ckb_mech_precompile", "ckb_mech_codegen", "ckb_codegen_log",
-           "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv", "ckb_mech_load2", "ckb_mech_load3")
+           "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv", "ckb_mech_load2", "ckb_mech_load3",
+           "ckb_mech_reserve")
 
 
 class CkbError(RuntimeError):
@@ -70,6 +71,8 @@ def lib():
     L.ckb_mech_load3.restype = C.c_int
     L.ckb_mech_free.argtypes = [vp]
     L.ckb_mech_free.restype = None
+    L.ckb_mech_reserve.argtypes = [vp, i64]
+    L.ckb_mech_reserve.restype = C.c_int
     L.ckb_mech_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
     L.ckb_mech_info.restype = C.c_int
     integ = [vp, vp, vp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, i32, vp, vp, vp]
@@ -182,19 +185,7 @@ class Mech:
     """ckb_mech handle.  `mech` is any object that carries the arrays of ckb_mech_desc as attributes."""
 
     def __init__(self, mech):
-        keep = dict(
-            mol_weight=_f64(mech.mol_weight), nasa=_f64(mech.nasa), arr_A=_f64(mech.arr_A),
-            arr_beta=_f64(mech.arr_beta), arr_E=_f64(mech.arr_E),
-            reac_ptr=_i32(mech.reac_ptr), reac_species=_i32(mech.reac_species), reac_nu=_i32(mech.reac_nu),
-            prod_ptr=_i32(mech.prod_ptr), prod_species=_i32(mech.prod_species), prod_nu=_i32(mech.prod_nu),
-            tb_reaction=_i32(mech.tb_reaction), tb_ptr=_i32(mech.tb_ptr), tb_species=_i32(mech.tb_species),
-            tb_eff=_f64(mech.tb_eff))
-        d = _Desc()
-        d.n_species = int(keep["mol_weight"].shape[0])
-        d.n_reactions = int(keep["arr_A"].shape[0])
-        d.n_third_body = int(keep["tb_reaction"].shape[0])
-        for k, v in keep.items():
-            setattr(d, k, v.ctypes.data)
+        d, keep = _make_desc(mech)      # `keep` holds the arrays the descriptor points at until the load returns
         self._h = C.c_void_p()
         if getattr(mech, "fo_reaction", None) is not None and len(mech.fo_reaction):   # fall-off reactions
             fr, lo, tr = _i32(mech.fo_reaction), _f64(mech.fo_low), _f64(mech.fo_troe)
@@ -224,6 +215,11 @@ class Mech:
         if rc != OK:
             raise CkbError(rc, "ckb_mech_specialize: " + lib().ckb_codegen_log().decode()[-2000:])
         self.specialized = True
+        return self
+
+    def reserve(self, max_batch):
+        """ckb_mech_reserve: size the handle's queue-order scratch for batches of up to max_batch systems."""
+        _check(lib().ckb_mech_reserve(self._h, int(max_batch)), "ckb_mech_reserve")
         return self
 
     def close(self):

@@ -33,33 +33,18 @@ def instantiations():
     return out
 
 
-def systems_per_group(L: int, NV: int) -> int:
-    """Systems a group of L lanes evaluates together (template parameter M).  M = 2 shares table loads and index
-    decoding between two systems of a warp and interleaves their chains, but measured slower on B200 than M = 1
-    (129k vs 144k ODE/s on configs[3]: twice the registers, half the resident warps) -- kept as a knob."""
-    return int(os.environ.get("CKB_M32", "1")) if L == 32 else 1
-
-
-def exp_table(L: int) -> int:
-    """1 = exp through the 64-entry 2^(j/64) table in shared memory (12 FP64 instructions + one shared read instead of
-    17 FP64 instructions): pays where the FP64 pipe is the busy unit and the load/store pipe is not."""
-    env = os.environ.get("CKB_EXP_TABLE_MAXL", "0")
-    return 1 if L <= int(env) else 0
-
-
 def min_blocks(L: int, NV: int, method: str = "rkck") -> int:
     """Resident 128-thread blocks per SM that the register allocation of integrate_kernel<L, NV> must allow
     (launch bounds): 4 -> <= 128 registers, 3 -> <= 168, 2 -> <= 255.  Chosen so that no instantiation spills."""
     if L == 1:  # thread-per-ODE: k3..k5 (RKCK) / v (RKC) sit in shared scratch so that 3 blocks fit
         if method == "rkc":
             return 2
-        return int(os.environ.get("CKB_MINB_L1", "3")) if NV <= 14 else 2
+        return 3 if NV <= 14 else 2
     if L in (2, 4):  # few lanes per system: small mechanisms, short stage vectors
-        return int(os.environ.get("CKB_MINB_L24", "4")) if NV <= 5 else 3
-    doubles = NV * systems_per_group(L, NV)  # register slots per stage vector
-    if doubles <= int(os.environ.get("CKB_MINB4_MAXNV", "2")):
-        return int(os.environ.get("CKB_MINB_SMALL", "4"))
-    if doubles <= 4:
+        return 4 if NV <= 5 else 3
+    if NV <= 2:  # register slots per stage vector
+        return 4
+    if NV <= 4:
         return 3
     return 2
 
@@ -68,7 +53,7 @@ def tmem_tables(L: int, NV: int) -> int:
     """1 = the object also carries warp-per-ODE integrate kernels that read the reaction-slot table from tensor memory
     (tcgen05.ld) instead of global memory / L1: one block of 512 threads per SM then owns the SM's
     512 TMEM columns, sized by tmem_block()."""
-    return int(os.environ.get("CKB_TMEM", "1")) if (L == 32 and NV in (2, 4)) else 0
+    return 1 if (L == 32 and NV in (2, 4)) else 0
 
 
 def tmem_block(L: int, NV: int) -> int:
@@ -79,7 +64,7 @@ def tmem_block(L: int, NV: int) -> int:
 
 def block_threads(L: int, NV: int) -> int:
     """Threads per block of the table-driven kernels (CKB_BLOCK)."""
-    return int(os.environ.get("CKB_BLOCK_L32", "128")) if L == 32 else 128
+    return 128
 
 
 def _digest(extra: str) -> str:
@@ -125,9 +110,9 @@ def _run(cmd, verbose):
 
 def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
-    flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("CKB_DEFS", "").split()  # tuning knobs
+    flags = FLAGS + (["-Xptxas", "-v"] if ptxas_v else [])
     stamp = os.path.join(OBJ, "stamp")
-    digest = _digest(" ".join(flags) + os.environ.get("CKB_MINB4_MAXNV", "") + os.environ.get("CKB_MINB_SMALL", "") + os.environ.get("CKB_M32", "") + os.environ.get("CKB_US", "") + os.environ.get("CKB_MINB_L1", "") + os.environ.get("CKB_MINB_L24", "") + os.environ.get("CKB_US_L1", "") + os.environ.get("CKB_EXP_TABLE_MAXL", "") + os.environ.get("CKB_BLOCK_L32", "") + os.environ.get("CKB_TMEM", ""))
+    digest = _digest(" ".join(flags))
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     _embed_sources()
@@ -142,9 +127,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
                            f"-DCKB_MINB={max(1, min_blocks(L, NV) * 128 // bt)}", f"-DCKB_MINB_RKC={max(1, min_blocks(L, NV, 'rkc') * 128 // bt)}",
                            f"-DCKB_TMEM={tmem_tables(L, NV)}", f"-DCKB_TMEM_BLOCK={tmem_block(L, NV)}",
                            f"-DCKB_TMEM_MIN_N={148 * tmem_block(L, NV) // 32}",
-                           f"-DCKB_UNROLL_SLOTS={int(os.environ.get('CKB_US_L1', '1')) if L == 1 else int(os.environ.get('CKB_US', '1'))}",
-                           f"-DCKB_EXP_TABLE={exp_table(L)}",
-                           f"-DCKB_M={systems_per_group(L, NV)}", "-c",
+                           "-c",
                            os.path.join(CSRC, "ckb_inst.cu"), "-o", obj]))
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         list(ex.map(lambda j: _run(j[1], verbose or ptxas_v), jobs))

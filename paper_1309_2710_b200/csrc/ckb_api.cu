@@ -164,6 +164,11 @@ int ckb_mech_load3(const ckb_mech_desc *d, const double *nasa_high, const double
       return rc;
     }
   }
+  rc = ckb_mech_reserve(m, CKB_DEFAULT_MAX_BATCH);
+  if (rc != CKB_OK) {
+    ckb_mech_free(m);
+    return rc;
+  }
   cudaError_t e = cudaMalloc((void **)&m->d_counters, CKB_COUNTER_RING * 8);
   for (int i = 0; i < CKB_NPACK && e == cudaSuccess; i++) {
     ckb_host::Packed &p = m->pk[i];
@@ -177,6 +182,12 @@ int ckb_mech_load3(const ckb_mech_desc *d, const double *nasa_high, const double
   }
   *out = m;
   return CKB_OK;
+}
+
+int ckb_mech_reserve(ckb_mech *m, int64_t max_batch) {
+  if (!m || max_batch < 0) return CKB_EINVAL;
+  CK(cudaDeviceSynchronize()); /* nothing of this handle may be in flight while its scratch is replaced */
+  return ckb_host::queue_scratch(m, 0, (long long)max_batch, true);
 }
 
 void ckb_mech_free(ckb_mech *m) {
@@ -216,7 +227,7 @@ int ckb_mech_info(const ckb_mech *m, int32_t *n_species, int32_t *n_reactions, i
 static int integrate_impl(const ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
                           int64_t ld, double t, double dt, double rtol, double atol, int32_t method,
                           int32_t variant, int32_t *status, int32_t *stats, cudaStream_t stream, int slot,
-                          int64_t n_choice, int cv) {
+                          int64_t n_choice, int cv, bool grow) {
   if (!m || N < 0 || (method != CKB_METHOD_RKCK && method != CKB_METHOD_RKC)) return CKB_EINVAL;
   if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(t) || !(rtol > 0.0) || !(atol >= 0.0)) return CKB_EINVAL;
   if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
@@ -235,15 +246,15 @@ static int integrate_impl(const ckb_mech *m, double *states, const double *press
        * system, computed by the register-resident thread-per-ODE kernel whatever mapping integrates; mechanisms
        * beyond 16 unknowns: by the warp-per-ODE one) */
       const Launch l1 = m->pk[0].rc == CKB_OK ? Launch{1, m->pk[0].dm.NV, true} : Launch{32, pk32.dm.NV, false};
-      rc = ckb_host::queue_scratch(m, slot, N);
+      rc = ckb_host::queue_scratch(m, slot, N, grow);
       if (rc) return rc;
       ckb_host::ProxyArgs pa{states, pressure, p_uniform, (long long)N, (long long)ld, 1e-3 * dt, rtol, atol,
                              m->osc[slot].d_keys, stream, cv};
       rc = dispatch_proxy(m, l1, pa);
       if (rc) return rc;
-      rc = ckb_host::make_queue_order(m, slot, 1, m->osc[slot].d_keys, N, a.stream, &a.order);
+      rc = ckb_host::make_queue_order(m, slot, 1, m->osc[slot].d_keys, N, a.stream, &a.order, grow);
     } else {
-      rc = ckb_host::make_queue_order(m, slot, 0, states, N, a.stream, &a.order);
+      rc = ckb_host::make_queue_order(m, slot, 0, states, N, a.stream, &a.order, grow);
     }
     if (rc) return rc;
   }
@@ -254,14 +265,14 @@ int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, dou
                   int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
                   int32_t *status, int32_t *stats, void *stream) {
   return integrate_impl(m, states, pressure, p_uniform, N, ld, t, dt, rtol, atol, method, variant, status, stats,
-                        (cudaStream_t)stream, 0, N, 0);
+                        (cudaStream_t)stream, 0, N, 0, false);
 }
 
 int ckb_integrate_cv(const ckb_mech *m, double *states, const double *density, double rho_uniform, int64_t N,
                      int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
                      int32_t *status, int32_t *stats, void *stream) {
   return integrate_impl(m, states, density, rho_uniform, N, ld, t, dt, rtol, atol, method, variant, status, stats,
-                        (cudaStream_t)stream, 0, N, 1);
+                        (cudaStream_t)stream, 0, N, 1, false);
 }
 
 static int rhs_impl(const ckb_mech *m, const double *states, const double *pressure, double p_uniform, int64_t N,
@@ -292,7 +303,7 @@ static int integrate_host_impl(ckb_mech *m, double *states, const double *pressu
                                int32_t variant, int32_t *status, int32_t *stats, void *stream, int cv) {
   if (!m || N < 0) return CKB_EINVAL;
   if (N == 0) return integrate_impl(m, nullptr, nullptr, p_uniform, 0, 0, t, dt, rtol, atol, method, variant,
-                                    nullptr, nullptr, (cudaStream_t)stream, 0, 0, cv);
+                                    nullptr, nullptr, (cudaStream_t)stream, 0, 0, cv, true);
   if (!states || ld < N) return CKB_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
   const int n = m->K + 1;
@@ -320,12 +331,7 @@ static int integrate_host_impl(ckb_mech *m, double *states, const double *pressu
    * RKC batches are stiff problems whose kernel outlasts the copies by one to two orders of magnitude; splitting them
    * only adds a queue tail per chunk (configs[2]: 80 ms in 3 chunks against 46 ms in one), so they go through whole.
    * The device copy is dense (row stride N). */
-  static const int max_chunks = [] {
-    const char *e = std::getenv("CKB_HOST_CHUNKS"); /* tuning knob, 1..CKB_SCRATCH_SLOTS */
-    const int v = e ? std::atoi(e) : CKB_SCRATCH_SLOTS;
-    return v < 1 ? 1 : v > CKB_SCRATCH_SLOTS ? CKB_SCRATCH_SLOTS : v;
-  }();
-  const int chunks = (N >= 65536 && method == CKB_METHOD_RKCK) ? max_chunks : 1;
+  const int chunks = (N >= 65536 && method == CKB_METHOD_RKCK) ? CKB_SCRATCH_SLOTS : 1;
   if (chunks > 1 && !m->hstream[0]) {
     for (int i = 0; i < CKB_SCRATCH_SLOTS; i++) CK(cudaStreamCreateWithFlags(&m->hstream[i], cudaStreamNonBlocking));
     for (int i = 0; i <= CKB_SCRATCH_SLOTS; i++) CK(cudaEventCreateWithFlags(&m->hevent[i], cudaEventDisableTiming));
@@ -340,7 +346,7 @@ static int integrate_host_impl(ckb_mech *m, double *states, const double *pressu
     if (pressure) CK(cudaMemcpyAsync(m->ws_pressure + c0, pressure + c0, (size_t)nc * 8, cudaMemcpyHostToDevice, cs));
     int rc = integrate_impl(m, m->ws_states + c0, pressure ? m->ws_pressure + c0 : nullptr, p_uniform, nc, N, t, dt,
                             rtol, atol, method, variant, status ? m->ws_status + c0 : nullptr,
-                            stats ? m->ws_stats + 4 * c0 : nullptr, cs, c, N, cv);
+                            stats ? m->ws_stats + 4 * c0 : nullptr, cs, c, N, cv, true);
     if (rc) return rc;
     CK(cudaMemcpy2DAsync(states + c0, (size_t)ld * 8, m->ws_states + c0, (size_t)N * 8, (size_t)nc * 8, (size_t)n,
                          cudaMemcpyDeviceToHost, cs));
@@ -378,6 +384,7 @@ const char *ckb_strerror(int code) {
     case CKB_ENOMEM: return "out of memory";
     case CKB_ECUDA: return "CUDA runtime error (see ckb_last_cuda_error)";
     case CKB_EUNSUPPORTED: return "mechanism or variant outside the supported limits";
+    case CKB_ECAPACITY: return "batch larger than the size reserved for this handle (ckb_mech_reserve)";
     default: return "unknown error code";
   }
 }

@@ -933,10 +933,10 @@ struct Rkc {
 #pragma unroll
             for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0.get(sys, i), r, y.get(sys, i));
           } else {
-            const int ci = pm_it % (int)nd;
+            const int ci = pm_it % (int)nd; /* an ORIGINAL state row (0 = T, 1 + species), as in the oracle */
 #pragma unroll
             for (int i = 0; i < NV; i++)
-              if (sys.g + S::L * i == ci) w[i] = y.get(sys, i) - (w[i] - y.get(sys, i));
+              if (sys.valid(i) && (int)sys.tw(sys.m.o_perm + sys.g + S::L * i) == ci) w[i] = y.get(sys, i) - (w[i] - y.get(sys, i));
           }
           pm_it++;
           return false;
@@ -949,10 +949,10 @@ struct Rkc {
 #pragma unroll
             for (int i = 0; i < NV; i++) w[i] = fma(f[i] - f0.get(sys, i), r, y.get(sys, i));
           } else {
-            const int ci = pm_it % (int)nd;
+            const int ci = pm_it % (int)nd; /* an ORIGINAL state row (0 = T, 1 + species), as in the oracle */
 #pragma unroll
             for (int i = 0; i < NV; i++)
-              if (sys.g + S::L * i == ci) w[i] = y.get(sys, i) - (w[i] - y.get(sys, i));
+              if (sys.valid(i) && (int)sys.tw(sys.m.o_perm + sys.g + S::L * i) == ci) w[i] = y.get(sys, i) - (w[i] - y.get(sys, i));
           }
         }
 #pragma unroll

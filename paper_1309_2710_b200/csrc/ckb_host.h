@@ -111,7 +111,8 @@ struct ckb_mech {
   /* work-queue counters of the persistent kernels: a ring, one slot per launch in flight */
   unsigned long long *d_counters = nullptr;
   mutable std::atomic<unsigned> next_counter{0};
-  /* queue order scratch (ckb_order.cu), grow-only; calls on one handle must be stream-ordered */
+  /* queue order scratch (ckb_order.cu): slot 0 is sized at load / by ckb_mech_reserve and never grows inside
+   * ckb_integrate; calls on one handle must be stream-ordered (they share it) */
   struct OrderScratch { int *d_order = nullptr; unsigned *d_bins = nullptr; double *d_keys = nullptr; size_t cap = 0; };
   mutable OrderScratch osc[CKB_SCRATCH_SLOTS]; /* slot 0: ckb_integrate; slots 0..: the chunks of ckb_integrate_host */
   cudaStream_t hstream[CKB_SCRATCH_SLOTS] = {};  /* internal streams of the pipelined host entry */
@@ -132,8 +133,8 @@ struct IntegrateArgs {
 
 /* mode 0: keys are temperatures (hottest first); mode 1: keys are cost proxies (largest first, log-spaced bins) */
 int make_queue_order(const ckb_mech *m, int slot, int mode, const double *keys, long long N, cudaStream_t s,
-                     const int **order);
-int queue_scratch(const ckb_mech *m, int slot, long long N);
+                     const int **order, bool grow);
+int queue_scratch(const ckb_mech *m, int slot, long long N, bool grow);
 
 struct ProxyArgs {
   const double *states; const double *pressure; double p_uniform; long long N, ld; double h, rtol, atol;

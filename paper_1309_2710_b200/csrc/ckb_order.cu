@@ -107,9 +107,12 @@ namespace ckb_host {
 
 /* fills m's scratch with the queue order of the N systems whose temperatures are T[0..N); returns the device
  * pointer in *order (NULL: keep index order) */
-/* grow-only scratch of one slot: order[N], keys[N], bins */
-int queue_scratch(const ckb_mech *m, int slot, long long N) {
+/* scratch of one slot: order[N], keys[N], bins.  The device entry (ckb_integrate) never allocates: its slot is sized by
+ * ckb_mech_load / ckb_mech_reserve and a larger batch is refused (CKB_ECAPACITY); the host entry, which owns its
+ * workspace and synchronises anyway, grows its slots (grow = true). */
+int queue_scratch(const ckb_mech *m, int slot, long long N, bool grow) {
   ckb_mech::OrderScratch &sc = m->osc[slot];
+  if ((size_t)N > sc.cap && !grow) return CKB_ECAPACITY;
   if ((size_t)N > sc.cap) {
     if (sc.d_order) cudaFree(sc.d_order);
     if (sc.d_keys) cudaFree(sc.d_keys);
@@ -124,11 +127,11 @@ int queue_scratch(const ckb_mech *m, int slot, long long N) {
 
 /* fills the slot's scratch with the queue order of N systems by their keys; returns the device pointer in *order */
 int make_queue_order(const ckb_mech *m, int slot, int mode, const double *keys, long long N, cudaStream_t s,
-                     const int **order) {
+                     const int **order, bool grow) {
   ckb_mech::OrderScratch &sc = m->osc[slot];
   *order = nullptr;
   if (N > 2147483647LL) return CKB_OK;
-  int rc = queue_scratch(m, slot, N);
+  int rc = queue_scratch(m, slot, N, grow);
   if (rc) return rc;
   CK(cudaMemsetAsync(sc.d_bins, 0, CKB_ORDER_BINS * sizeof(unsigned), s));
   const long long per_block = CKB_ORDER_THREADS * CKB_ORDER_ITEMS;

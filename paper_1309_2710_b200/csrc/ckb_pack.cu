@@ -430,7 +430,9 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   int TBE = 0;
   for (auto &s : P.sets) TBE = std::max(TBE, (int)s.size());
   /* 16-bit region offsets, in bytes */
-  if ((long long)(n + NTB) * G * 8 > 65535 || (long long)NSR * L * G * 8 > 65535) return CKB_EUNSUPPORTED;
+  if ((long long)(n + NTB + 1) * G * 8 > 65535 ||
+      ((long long)NSR * L + (L > 1 ? CKB_ZERO_SLOTS : 0)) * G * 8 > 65535) /* idle gather entries point behind the q region */
+    return CKB_EUNSUPPORTED;
   const bool optimise = true;
 
   /* components: 0 = T, then species by decreasing gather-row length */

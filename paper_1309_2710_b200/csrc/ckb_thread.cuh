@@ -31,6 +31,9 @@ using ckb::ckb_exp;
  * pointer kept in a struct degrades to generic loads with 64-bit address arithmetic) */
 extern __shared__ double ckbt_smem[];
 
+#ifndef CKBT_LOCKSTEP
+#define CKBT_LOCKSTEP 1 /* the warps of a block enter f(y) together (one instruction stream per SM) */
+#endif
 #ifndef CKBT_U
 #define CKBT_U 3    /* reaction slots per trip of a class loop (2U exponential chains in lock step) */
 #endif
@@ -889,8 +892,12 @@ integrate_thread_kernel(const __grid_constant__ DevThread m, const __grid_consta
     /* the warps of the block enter f(y) together: one instruction stream per SM through the instruction caches (the
      * code of one trip is several times the 32 KB L1.5); a warp that has run out of systems only keeps the barrier */
     const bool warp_any = __any_sync(0xffffffffu, active);
+#if CKBT_LOCKSTEP
     if (!__syncthreads_or(warp_any)) break;
     if (!warp_any) continue;
+#else
+    if (!warp_any) break;
+#endif
     bool hold = false;
     if constexpr (METHOD == 0) { /* RKCK: stage-2 lanes sit out an evaluation that some lane needs as stage 1 (R25) */
       const bool s1 = active && integ.stage == 1;

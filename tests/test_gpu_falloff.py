@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 from paper_1309_2710_b200 import synth
-from test_gpu_parity import _compare, _oracle, _run_gpu
+from test_gpu_parity import _compare, _compare_tight, _oracle, _run_gpu
 
 pytestmark = pytest.mark.gpu
 
@@ -106,7 +106,16 @@ def test_parity_falloff(cfg, N, method, variant):
         ora2 = _oracle(mech, pert, p, 1e-6, method)
         self_flips = int((~((ora2[2] == ora[2]).all(axis=0) & (ora2[1] == ora[1]))).sum())
         flips = (2 * self_flips + 2) / N
-    rep = _compare(gpu, ora, max_flip_frac=flips)
+    if flips > 0.01:
+        # more than 1 % of the systems may flip (111/1566: the oracle flips on 7 of 64 against itself): the flip count is
+        # then no assertion at all -- instead every system of a sample must end as close to the truth (an oracle run at
+        # rtol 1e-11) as the oracle's own result does, whatever its decisions; systems with identical
+        # decisions still meet the north_star bound
+        rep = _compare(gpu, ora, max_flip_frac=1.0)
+        idx = np.arange(N) if cfg < 4 else np.arange(0, N, 5)
+        rep["against_truth"] = _compare_tight(mech, states, p, 1e-6, method, gpu, ora, idx=idx)
+    else:
+        rep = _compare(gpu, ora, max_flip_frac=flips)
     print(f"fall-off cfg{cfg} {method} {variant} N={N}: {rep}")
     assert np.isin(ora[1], (0, 4)).all()
 
@@ -129,5 +138,8 @@ def test_falloff_with_two_ranges_at_size_tensor_memory_kernel():
     m.close()
     assert np.isin(st, (0, 4)).all() and np.abs(y[1:].sum(0) - 1.0).max() < 1e-11
     pick = np.random.default_rng(5).choice(N, size=48, replace=False)
-    ora = _oracle(mech, np.ascontiguousarray(states[:, pick]), p, 1e-6, "rkc")
-    _compare((y[:, pick], st[pick], stt[:, pick]), ora, max_flip_frac=5e-2)
+    sub_states = np.ascontiguousarray(states[:, pick])
+    ora = _oracle(mech, sub_states, p, 1e-6, "rkc")
+    sub = (y[:, pick], st[pick], stt[:, pick])
+    _compare(sub, ora, max_flip_frac=1.0)            # identical decisions: north_star bound; flips: judged against the truth
+    print("against the truth:", _compare_tight(mech, sub_states, p, 1e-6, "rkc", sub, ora, idx=np.arange(0, 48, 3)))
