@@ -190,7 +190,9 @@ class GpuCase:
                "stages_max": int(st[3].max()), "status_nonzero": int((status != 0).sum()),
                "status_sigma": int((status == 4).sum())}
         if d is not None:   # Eq. 40: D = sum d_i / (32 max d_i) per 32 consecutive systems
-            out["divergence_D_mean"] = float((d.sum(1) / (32.0 * d.max(1))).mean())
+            D = d.sum(1) / (32.0 * d.max(1))
+            out["divergence_D_mean"] = float(D.mean())
+            out["divergence_D_hist10"] = [int(x) for x in np.histogram(D, bins=10, range=(0.0, 1.0))[0]]
         return out
 
     def e2e(self, K, W):
@@ -226,6 +228,15 @@ def measured_traffic(cfg, N, specialised=False):
                 if e["config"] == cfg and e["N"] == N and bool(e.get("specialised", False)) == bool(specialised):
                     return e["dram_bytes_read"] + e["dram_bytes_write"]
     return None
+
+
+def north_star_counters():
+    """branch uniformity / active lanes of the configs[3] kernels from the committed ncu captures (profiles/north_star.json)"""
+    path = os.path.join(ROOT, "profiles", "north_star.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return {"ncu": json.load(fh)}
+    return {"ncu": None}
 
 
 def roofline(case, ms, work, peak_tflops, peak_src):
@@ -301,7 +312,15 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     from paper_1309_2710_b200 import binding
-    peak_flops = binding.fp64_probe("dfma", 1 << 15)
+    # roofline denominator: sustained DFMA rate of this GPU (>= 1 s per run, SM clock sampled under that load;
+    # 3 runs of ~1.2 s after a warm-up run, the fastest counts)
+    with ClockSampler(local) as pclk:
+        t_probe = time.perf_counter()
+        peak_flops = binding.fp64_probe("dfma", 1 << 23)
+        t_probe = time.perf_counter() - t_probe
+    probe_info = {"tflops": peak_flops / 1e12, "runs": 4, "seconds_per_run": t_probe / 4.0,
+                  "sm_mhz_under_probe": pclk.summary()["sm_mhz"], "reasons": pclk.summary()["reasons"],
+                  "frac_of_nominal": peak_flops / 1e12 / FP64_NOMINAL_TFLOPS}
     exp_rate = binding.fp64_probe("exp", 1 << 12)
     # every rank integrates its own N systems (independent problems, no data-path collective): weak scaling
     case = GpuCase(args.config, N, dt, args.variant, args.ordering, local)
@@ -330,11 +349,13 @@ def run_ours(args):
         "clocks": clk.summary(),
         # our kernels per ckb_integrate call: integrate_kernel, and for N >= 4096 the queue order (hist, scan, scatter;
         # plus the cost-proxy kernel for thread-per-ODE RKC)
-        "gpu_launches": K * (1 + (3 if N >= 4096 else 0) + (1 if (N >= 24576 and spec.method == "rkc" and spec.K + 1 <= 16 and args.variant in ("auto", "thread", "sub4", "sub2")) else 0)),
+        "gpu_launches": K * (1 + (3 if N >= 4096 else 0) + (1 if (N >= 24576 and spec.method == "rkc" and spec.K + 1 <= 16 and args.variant in ("auto", "thread", "sub4", "sub2")) else 0)
+                             + (1 if (N >= 4096 and spec.method == "rkc" and spec.K + 1 > 16 and args.variant == "thread") else 0)),
         "work_per_step": work,
         "roofline": roofline(case, float(np.mean(ms)), work, peak_flops / 1e12,
-                             "measured: ckb_fp64_probe DFMA chains on this GPU (MEASURED_PEAKS.json has no FP64 figure)"),
+                             "measured: ckb_fp64_probe, sustained DFMA chains on this GPU, >= 1 s per run (MEASURED_PEAKS.json has no FP64 figure)"),
         "exp_per_s": {"achieved": 2.0 * case.m.n_slots * work["rhs_calls"] / (np.mean(ms) * 1e-3), "peak_measured": exp_rate},
+        "fp64_probe": probe_info,
         "ms_min_max": [float(min(ms)), float(max(ms))],
     }
     if not args.no_extra:  # every rank at the same time (they share the host's PCIe complex), max over ranks
@@ -355,62 +376,84 @@ def run_ours(args):
         r1, n1, _, t1 = oracle_time(args.config, N, dt, budget_s=6.0, nthreads=1)
         out["cpu_baseline"]["single_core"] = {"value": r1, "sample_n": n1, "seconds": t1}
         extra = {}
-        others = [c for c in (2, 3, 4) if c != args.config] + ([1] if args.config != 1 else [])
-        for c in others:
-            s2, N2, dt2 = workload(c)
-            for var in (("auto",) if c != 3 else ("warp", "sub16")):
-                try:
-                    cs = GpuCase(c, N2, dt2, var)
-                    wk = cs.work()
-                    m2 = cs.timed_steps(3, 3)
-                    extra[f"cfg{c}_{s2.method}_{var}_N{N2}"] = {
-                        "odes_per_s": N2 / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)), "work": wk,
-                        "roofline": roofline(cs, float(np.mean(m2)), wk, peak_flops / 1e12, "measured DFMA probe")}
-                    cs.close()
-                    del cs
-                except Exception as ex:  # pragma: no cover
-                    extra[f"cfg{c}_{var}"] = {"error": str(ex)}
-        # constant-volume closure (ckb_integrate_cv) on the headline workload and on configs[3]
-        for c in (1, 3):
+
+        def measure(key, c, N2, dt2, var, K2=3, W2=3, cpu=False, **kw):
+            """one more workload: ODEs/s, work counters, roofline; optionally the oracle on a bounded sample of it"""
             try:
-                s2, N2, dt2 = workload(c)
-                cs = GpuCase(c, N2, dt2, "auto", cv=True)
+                s2 = synth.CONFIGS[c]
+                cs = GpuCase(c, N2, dt2, var, **kw)
                 wk = cs.work()
-                m2 = cs.timed_steps(3, 3)
-                extra[f"cv_cfg{c}_{s2.method}_auto_N{N2}"] = {
-                    "odes_per_s": N2 / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)), "work": wk,
-                    "roofline": roofline(cs, float(np.mean(m2)), wk, peak_flops / 1e12, "measured DFMA probe")}
-                cs.close()
-                del cs
-            except Exception as ex:  # pragma: no cover
-                extra[f"cv_cfg{c}"] = {"error": str(ex)}
-        # two-range thermodynamics + fall-off reactions (ckb_mech_load3) on the same workloads
-        for c in (1, 3):
-            try:
-                s2, N2, dt2 = workload(c)
-                if c == 3:
-                    N2 //= 4   # the fall-off variant of 53/634 needs 7x the f evaluations per system: a quarter batch
-                cs = GpuCase(c, N2, dt2, "auto", f1=True)
-                wk = cs.work()
-                m2 = cs.timed_steps(3, 3)
+                m2 = cs.timed_steps(K2, W2)
                 rf = roofline(cs, float(np.mean(m2)), wk, peak_flops / 1e12, "measured DFMA probe")
-                rf["traffic"] = None
-                extra[f"f1_cfg{c}_{s2.method}_auto_N{N2}"] = {
-                    "odes_per_s": N2 / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)), "work": wk, "roofline": rf,
-                    "n_falloff": int(len(cs.mech.fo_reaction))}
+                if kw.get("f1"):
+                    rf["traffic"] = None
+                e = {"odes_per_s": N2 / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)), "N": N2, "dt": dt2,
+                     "method": s2.method, "variant": var, "work": wk, "roofline": rf}
+                if kw.get("f1"):
+                    e["n_falloff"] = int(len(cs.mech.fo_reaction))
                 cs.close()
                 del cs
+                if cpu:   # SURVEY D9: the oracle on all cores and on one core, bounded sample of the same workload
+                    r, n_used, cores, t = oracle_time(c, N2, dt2, budget_s=5.0)
+                    r1, n1, _, t1 = oracle_time(c, N2, dt2, budget_s=3.0, nthreads=1)
+                    e["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                         "sample": f"first {n_used} of {N2} systems, {t:.1f} s",
+                                         "single_core": {"value": r1, "sample_n": n1, "seconds": t1}}
+                extra[key] = e
             except Exception as ex:  # pragma: no cover
-                extra[f"f1_cfg{c}"] = {"error": str(ex)}
+                extra[key] = {"error": str(ex)[:300]}
+
+        # BASELINE.json configs[2..4] at their full sizes; configs[3] with the warp-per-ODE AND the thread-per-ODE variant
+        # (B:configs[3]); configs[4] at both global steps (B:configs[4])
+        if args.config != 2:
+            measure(f"cfg2_rkc_auto_N{HEADLINE_N[2]}", 2, HEADLINE_N[2], 1e-6, "auto", cpu=True)
+        if args.config != 3:
+            measure(f"cfg3_rkc_warp_N{HEADLINE_N[3]}", 3, HEADLINE_N[3], 1e-6, "warp", cpu=True)
+            measure(f"cfg3_rkc_thread_N{HEADLINE_N[3]}", 3, HEADLINE_N[3], 1e-6, "thread")
+        if args.config != 4:
+            measure(f"cfg4_rkc_auto_N{HEADLINE_N[4]}_dt1e-6", 4, HEADLINE_N[4], 1e-6, "auto", cpu=True)
+            measure(f"cfg4_rkc_auto_N{HEADLINE_N[4] // 4}_dt1e-5", 4, HEADLINE_N[4] // 4, 1e-5, "auto", K2=2, W2=1, cpu=True)
+        if args.config != 1:
+            measure(f"cfg1_rkck_auto_N{HEADLINE_N[1]}", 1, HEADLINE_N[1], 1e-6, "auto", cpu=True)
+        # constant-volume closure (SURVEY 8(f)-f3) and two-range thermo + fall-off (8(f)-f1) on the 53-species class
+        measure(f"cv_cfg3_rkc_auto_N{HEADLINE_N[3] // 4}", 3, HEADLINE_N[3] // 4, 1e-6, "auto", K2=2, W2=1, cv=True)
+        measure(f"f1_cfg3_rkc_auto_N{HEADLINE_N[3] // 8}", 3, HEADLINE_N[3] // 8, 1e-6, "auto", K2=2, W2=1, f1=True)
         # the paper's "similar neighbours" experiment (P:247, P:269): the same systems sorted by T
         try:
             cs = GpuCase(args.config, N, dt, args.variant, "similar")
             m2 = cs.timed_steps(3, 3)
+            wk = cs.work()
             extra["headline_similar_ordering"] = {"odes_per_s": N / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2)),
-                                                  "divergence_D_mean": cs.work().get("divergence_D_mean")}
+                                                  "divergence_D_mean": wk.get("divergence_D_mean"),
+                                                  "divergence_D_hist10": wk.get("divergence_D_hist10")}
             cs.close()
         except Exception as ex:  # pragma: no cover
             extra["headline_similar_ordering"] = {"error": str(ex)}
+        # ODEs/s versus N for the other configs (BASELINE.json metric; a few sizes of each N_list)
+        for c, sizes in ((2, (2 ** 10, 2 ** 14, 2 ** 16)), (3, (2 ** 10, 2 ** 13, 2 ** 15)), (4, (2 ** 13, 2 ** 14))):
+            if c == args.config:
+                continue
+            sw = {}
+            for n2 in sizes:
+                try:
+                    cs = GpuCase(c, n2, 1e-6, "auto")
+                    m2 = cs.timed_steps(2, 3)
+                    sw[str(n2)] = {"odes_per_s": n2 / (np.mean(m2) * 1e-3), "ms": float(np.mean(m2))}
+                    cs.close()
+                    del cs
+                except Exception as ex:  # pragma: no cover
+                    sw[str(n2)] = {"error": str(ex)[:200]}
+            extra[f"sweep_cfg{c}_auto"] = sw
+        # the figure BASELINE.json's north_star target is stated on: configs[3] (53/634, RKC) at N = 2^17
+        ns = [extra.get(k) for k in (f"cfg3_rkc_warp_N{HEADLINE_N[3]}", f"cfg3_rkc_thread_N{HEADLINE_N[3]}")]
+        ns = [e for e in ns if e and "roofline" in e]
+        if ns:
+            best = max(ns, key=lambda e: e["odes_per_s"])
+            out["north_star"] = {"config": 3, "N": HEADLINE_N[3], "method": "rkc", "variant": best["variant"],
+                                 "odes_per_s": best["odes_per_s"], "frac": best["roofline"]["frac"],
+                                 "frac_of_nominal": best["roofline"]["frac_of_nominal"], "target_frac": 0.40,
+                                 "by_variant": {e["variant"]: {"odes_per_s": e["odes_per_s"], "frac": e["roofline"]["frac"]} for e in ns},
+                                 **north_star_counters()}
         out["configs"] = extra
     if (args.sweep or not args.no_extra) and rank == 0 and world == 1:  # ODEs/s versus N (BASELINE.json metric)
         sw = {}

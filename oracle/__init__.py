@@ -87,6 +87,12 @@ def lib():
         L.ora_rkc_step.restype = None
         L.ora_spectral_radius.argtypes = [RHS_FN, C.c_void_p, C.c_int, C.c_double, dp, dp, C.c_int, ip, ip]
         L.ora_spectral_radius.restype = C.c_double
+        L.ora_fit_reverse.argtypes = [dp, dp, dp]
+        L.ora_fit_reverse.restype = None
+        L.ora_equilibrium_constant.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.ora_equilibrium_constant.restype = C.c_double
+        L.ora_reverse_parameters.argtypes = [C.c_void_p, C.c_int, dp, dp]
+        L.ora_reverse_parameters.restype = None
         L.ora_num_threads.argtypes = []
         L.ora_num_threads.restype = C.c_int
         _lib = L
@@ -164,6 +170,16 @@ class OracleMech:
         y = _f64(y)
         out = np.empty_like(y)
         (lib().ora_rhs_cv if cv else lib().ora_rhs)(self._h, _dp(y), float(p), _dp(out))
+        return out
+
+    def equilibrium_constant(self, j, T):
+        """K_c of reaction j at T (Chemkin form, reading R32)."""
+        return lib().ora_equilibrium_constant(self._h, int(j), float(T))
+
+    def reverse_parameters(self, j, T3):
+        """Appendix A: (A_r, beta_r, E_r [cal/mol]) of the reverse of reaction j from k_f / K_c at the three temperatures."""
+        T3, out = _f64(T3), np.zeros(3)
+        lib().ora_reverse_parameters(self._h, int(j), _dp(T3), _dp(out))
         return out
 
     def integrate(self, states, p, dt, rtol, atol, method, t=0.0, nthreads=0, pressure=None, cv=False):
@@ -270,6 +286,13 @@ def spectral_radius(fn, t, y, v=None):
     s = lib().ora_spectral_radius(wrap_rhs(fn, n), None, n, float(t), _dp(y), _dp(vv), int(have_v),
                                   C.byref(nfe), C.byref(flag))
     return s, vv, nfe.value, flag.value
+
+
+def fit_reverse(T3, kr3):
+    """Eq. A.10-A.12: (A_r, beta_r, T_ar) through three (T, k_r) points."""
+    T3, kr3, out = _f64(T3), _f64(kr3), np.zeros(3)
+    lib().ora_fit_reverse(_dp(T3), _dp(kr3), _dp(out))
+    return out
 
 
 def num_threads():

@@ -800,6 +800,62 @@ int ora_integrate_cv(const ora_mech *m, double *states, const double *density, d
   return integrate_closure(m, states, density, rho_uniform, N, ld, t, dt, rtol, atol, method, status, stats, nthreads, 1);
 }
 
+/* ================================================================================================
+ * Appendix A: reversible -> irreversible conversion.  SURVEY 8(f)-f2.
+ * ============================================================================================== */
+
+/* Eq. A.10-A.12: the reverse Arrhenius parameters (A_r, beta_r, T_ar = E_r / R) through the three points
+ * (T_i, k_ri), with x_i = ln T_i and a_i = ln k_ri.  out[0] = A_r, out[1] = beta_r, out[2] = T_ar (kelvin). */
+void ora_fit_reverse(const double *T, const double *kr, double *out) {
+  const double T1 = T[0], T2 = T[1], T3 = T[2];
+  const double x1 = log(T1), x2 = log(T2), x3 = log(T3);
+  const double a1 = log(kr[0]), a2 = log(kr[1]), a3 = log(kr[2]);
+  const double den = x1 * T1 * (T3 - T2) + x2 * T2 * (T1 - T3) + x3 * T3 * (T2 - T1);
+  const double beta = (a1 * T1 * (T3 - T2) + a2 * T2 * (T1 - T3) + a3 * T3 * (T2 - T1)) / den;            /* A.10 */
+  const double Tar = T1 * T2 * T3 * (a1 * (x2 - x3) + a2 * (x3 - x1) + a3 * (x1 - x2)) / den;              /* A.11 */
+  const double lnA = (a1 * T1 * (x2 * T2 - x3 * T3) + a2 * T2 * (x3 * T3 - x1 * T1) + a3 * T3 * (x1 * T1 - x2 * T2)) / den; /* A.12 */
+  out[0] = exp(lnA);
+  out[1] = beta;
+  out[2] = Tar;
+}
+
+/* The equilibrium constant in concentration units of reaction j of a loaded mechanism at temperature T (reading R32:
+ * the paper takes "the equilibrium constants" as known, P:84 / P:461; the Chemkin form is used):
+ *     K_p = exp( sum_k nu_k (s_k/R - h_k/(R T)) ),   K_c = K_p (P_atm / (Ru T))^(sum_k nu_k),   nu = nu'' - nu',
+ *     s_k/R = a1 ln T + a2 T + a3 T^2/2 + a4 T^3/3 + a5 T^4/4 + a7,   h_k/(RT) = a1 + a2 T/2 + .. + a5 T^4/5 + a6/T,
+ * P_atm = 1.01325e6 dyn/cm^2; the NASA range of each species is picked by R30 when the mechanism has two. */
+double ora_equilibrium_constant(const ora_mech *m, int j, double T) {
+  double dG = 0.0;   /* sum_k nu_k (s_k/R - h_k/RT) */
+  int dnu = 0;
+  for (int side = 0; side < 2; side++) {
+    const int32_t *ptr = side ? m->prod_ptr : m->reac_ptr, *sp = side ? m->prod_sp : m->reac_sp,
+                  *nu = side ? m->prod_nu : m->reac_nu;
+    const int sign = side ? 1 : -1;
+    for (int e = ptr[j]; e < ptr[j + 1]; e++) {
+      const int k = sp[e];
+      const double *a = m->nasa + 7 * (size_t)k;
+      if (m->T_mid && T > m->T_mid[k]) a = m->nasa_hi + 7 * (size_t)k;
+      const double sR = a[0] * log(T) + a[1] * T + a[2] * T * T / 2.0 + a[3] * T * T * T / 3.0 + a[4] * T * T * T * T / 4.0 + a[6];
+      const double hRT = a[0] + a[1] * T / 2.0 + a[2] * T * T / 3.0 + a[3] * T * T * T / 4.0 + a[4] * T * T * T * T / 5.0 + a[5] / T;
+      dG += sign * nu[e] * (sR - hRT);
+      dnu += sign * nu[e];
+    }
+  }
+  return exp(dG) * pow(1.01325e6 / (ORA_RU * T), (double)dnu);
+}
+
+/* Appendix A for reaction j: k_r = k_f / K_c at the three temperatures, then Eq. A.10-A.12.
+ * out[0] = A_r, out[1] = beta_r, out[2] = E_r in cal/mol (= T_ar R_c). */
+void ora_reverse_parameters(const ora_mech *m, int j, const double *T3, double *out) {
+  double kr[3];
+  for (int i = 0; i < 3; i++) {
+    const double kf = m->A[j] * pow(T3[i], m->beta[j]) * exp(-m->E[j] / (ORA_RC * T3[i]));
+    kr[i] = kf / ora_equilibrium_constant(m, j, T3[i]);
+  }
+  ora_fit_reverse(T3, kr, out);
+  out[2] *= ORA_RC;
+}
+
 int ora_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();
