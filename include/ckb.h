@@ -168,6 +168,33 @@ int ckb_mech_codegen(const ckb_mech_desc *d, char *buf, int64_t cap, int64_t *ne
 const char *ckb_codegen_log(void); /* compiler log of the calling thread's last specialize / precompile */
 
 /*
+ * Chemkin-format reader and the paper's reversible -> irreversible converter (Appendix A).
+ * Host-side preprocessing, no device work.
+ *   mech_text    HOST  NUL-terminated text of a mechanism file: ELEMENTS, SPECIES, [THERMO], REACTIONS blocks
+ *   thermo_text  HOST  NUL-terminated text of a thermodynamic database (THERMO block), or NULL if mech_text has one
+ *   fit_T3       HOST  [3] the three distinct temperatures (K) of Appendix A, or NULL for 1000, 1500, 2000 K (the paper
+ *                      does not say which it used: DESIGN.md reading R33)
+ * Every reversible reaction ("=" / "<=>") becomes two irreversible ones: the reverse one takes its REV parameters if
+ * given, else (A_r, beta_r, E_r) from Eq. A.10-A.12 through k_r = k_f / K_c at the three temperatures, K_c in the Chemkin
+ * form from the NASA fits incl. a7 (reading R32).  A reversible fall-off reaction gets a reverse fall-off reaction with
+ * both limits fitted that way (P_r and F are the same for both directions).  Units are converted to mol-cm-s-K and
+ * cal/mol.  Supported syntax and what is refused: see csrc/ckb_chemkin.cu.
+ * ckb_chemkin_desc fills `d` and the ckb_mech_load3 arguments with pointers into the object (valid until
+ * ckb_chemkin_free; the low temperature range is d->nasa, the high one *nasa_high, R30).
+ * Errors: CKB_EINVAL (syntax, unknown species, unbalanced reaction, missing thermo), CKB_EUNSUPPORTED (a construct
+ * outside the list above), CKB_ENOMEM; ckb_chemkin_error() returns the calling thread's last message.
+ */
+typedef struct ckb_chemkin ckb_chemkin;
+int ckb_chemkin_parse(const char *mech_text, const char *thermo_text, const double *fit_T3, ckb_chemkin **out);
+void ckb_chemkin_free(ckb_chemkin *ck);
+int ckb_chemkin_desc(const ckb_chemkin *ck, ckb_mech_desc *d, const double **nasa_high, const double **T_mid,
+                     int32_t *n_falloff, const int32_t **fo_reaction, const double **fo_low, const double **fo_troe);
+const char *ckb_chemkin_species(const ckb_chemkin *ck, int32_t k);          /* name of species k, or NULL */
+/* which reaction of the file the irreversible reaction j came from (0-based), and whether it is a generated reverse */
+int ckb_chemkin_reaction_origin(const ckb_chemkin *ck, int32_t j, int32_t *input_reaction, int32_t *is_reverse);
+const char *ckb_chemkin_error(void);
+
+/*
  * ckb_integrate: advance every system i in [0, N) from t to t+dt, in place.
  *   states   DEVICE  SoA, row-major [(K+1)][ld]: row 0 = T (K), rows 1..K = mass fractions Y_k;
  *                    element (c, i) at states[c*ld + i]; ld >= N.  Caller-owned (e.g. a torch tensor).

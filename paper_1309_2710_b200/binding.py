@@ -24,7 +24,8 @@ EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "
            "ckb_rhs", "ckb_fp64_probe", "ckb_mech_pack_stats", "ckb_strerror", "ckb_last_cuda_error",
            "ckb_mech_specialize", "ckb_mech_precompile", "ckb_mech_codegen", "ckb_codegen_log",
            "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv", "ckb_mech_load2", "ckb_mech_load3",
-           "ckb_mech_reserve")
+           "ckb_mech_reserve", "ckb_chemkin_parse", "ckb_chemkin_free", "ckb_chemkin_desc", "ckb_chemkin_species",
+           "ckb_chemkin_reaction_origin", "ckb_chemkin_error")
 
 
 class CkbError(RuntimeError):
@@ -73,6 +74,19 @@ def lib():
     L.ckb_mech_free.restype = None
     L.ckb_mech_reserve.argtypes = [vp, i64]
     L.ckb_mech_reserve.restype = C.c_int
+    L.ckb_chemkin_parse.argtypes = [C.c_char_p, C.c_char_p, vp, C.POINTER(vp)]
+    L.ckb_chemkin_parse.restype = C.c_int
+    L.ckb_chemkin_free.argtypes = [vp]
+    L.ckb_chemkin_free.restype = None
+    L.ckb_chemkin_desc.argtypes = [vp, C.POINTER(_Desc), C.POINTER(vp), C.POINTER(vp), C.POINTER(i32), C.POINTER(vp),
+                                   C.POINTER(vp), C.POINTER(vp)]
+    L.ckb_chemkin_desc.restype = C.c_int
+    L.ckb_chemkin_species.argtypes = [vp, i32]
+    L.ckb_chemkin_species.restype = C.c_char_p
+    L.ckb_chemkin_reaction_origin.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32)]
+    L.ckb_chemkin_reaction_origin.restype = C.c_int
+    L.ckb_chemkin_error.argtypes = []
+    L.ckb_chemkin_error.restype = C.c_char_p
     L.ckb_mech_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
     L.ckb_mech_info.restype = C.c_int
     integ = [vp, vp, vp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, i32, vp, vp, vp]
@@ -179,6 +193,64 @@ def precompile(mech, arch="sm_100a") -> None:
     rc = lib().ckb_mech_precompile(C.byref(d), arch.encode())
     if rc != OK:
         raise CkbError(rc, "ckb_mech_precompile: " + lib().ckb_codegen_log().decode()[-2000:])
+
+
+class ChemkinMechanism:
+    """The arrays of ckb_mech_desc / ckb_mech_load3 as numpy attributes (copies), as ckb_chemkin_parse produced them."""
+
+
+def chemkin_parse(mech_text, thermo_text=None, fit_T=None) -> ChemkinMechanism:
+    """ckb_chemkin_parse + ckb_chemkin_desc (host only): read a Chemkin-format mechanism and convert every reversible
+    reaction into two irreversible ones (Appendix A).  The result can be given to mech_load()."""
+    L = lib()
+    h = C.c_void_p()
+    T3 = None if fit_T is None else _f64(fit_T)
+    rc = L.ckb_chemkin_parse(mech_text.encode(), None if thermo_text is None else thermo_text.encode(),
+                             None if T3 is None else C.c_void_p(T3.ctypes.data), C.byref(h))
+    if rc != OK:
+        raise CkbError(rc, "ckb_chemkin_parse: " + L.ckb_chemkin_error().decode())
+    try:
+        d = _Desc()
+        hi, tm, fr, lo, tr, nfo = C.c_void_p(), C.c_void_p(), C.c_void_p(), C.c_void_p(), C.c_void_p(), C.c_int32()
+        _check(L.ckb_chemkin_desc(h, C.byref(d), C.byref(hi), C.byref(tm), C.byref(nfo), C.byref(fr), C.byref(lo), C.byref(tr)),
+               "ckb_chemkin_desc")
+        K, R, R3, nf = d.n_species, d.n_reactions, d.n_third_body, nfo.value
+
+        def arr(ptr, n, ct, dt):
+            if n == 0 or not ptr:
+                return np.zeros(0, dtype=dt)
+            return np.ctypeslib.as_array(C.cast(ptr, C.POINTER(ct)), shape=(n,)).astype(dt, copy=True)
+
+        m = ChemkinMechanism()
+        m.name = "chemkin"
+        m.n_species, m.n_reactions = K, R
+        m.mol_weight = arr(d.mol_weight, K, C.c_double, np.float64)
+        m.nasa = arr(d.nasa, 7 * K, C.c_double, np.float64).reshape(K, 7)
+        m.nasa_high = arr(hi.value, 7 * K, C.c_double, np.float64).reshape(K, 7)
+        m.T_mid = arr(tm.value, K, C.c_double, np.float64)
+        m.arr_A, m.arr_beta, m.arr_E = (arr(p_, R, C.c_double, np.float64) for p_ in (d.arr_A, d.arr_beta, d.arr_E))
+        m.reac_ptr = arr(d.reac_ptr, R + 1, C.c_int32, np.int32)
+        m.prod_ptr = arr(d.prod_ptr, R + 1, C.c_int32, np.int32)
+        m.reac_species = arr(d.reac_species, int(m.reac_ptr[-1]), C.c_int32, np.int32)
+        m.reac_nu = arr(d.reac_nu, int(m.reac_ptr[-1]), C.c_int32, np.int32)
+        m.prod_species = arr(d.prod_species, int(m.prod_ptr[-1]), C.c_int32, np.int32)
+        m.prod_nu = arr(d.prod_nu, int(m.prod_ptr[-1]), C.c_int32, np.int32)
+        m.tb_reaction = arr(d.tb_reaction, R3, C.c_int32, np.int32)
+        m.tb_ptr = arr(d.tb_ptr, R3 + 1, C.c_int32, np.int32)
+        m.tb_species = arr(d.tb_species, int(m.tb_ptr[-1]), C.c_int32, np.int32)
+        m.tb_eff = arr(d.tb_eff, int(m.tb_ptr[-1]), C.c_double, np.float64)
+        m.fo_reaction = arr(fr.value, nf, C.c_int32, np.int32)
+        m.fo_low = arr(lo.value, 3 * nf, C.c_double, np.float64).reshape(nf, 3)
+        m.fo_troe = arr(tr.value, 4 * nf, C.c_double, np.float64).reshape(nf, 4)
+        m.species_names = [L.ckb_chemkin_species(h, k).decode() for k in range(K)]
+        org, rev = C.c_int32(), C.c_int32()
+        m.origin, m.is_reverse = np.zeros(R, dtype=np.int32), np.zeros(R, dtype=np.int32)
+        for j in range(R):
+            _check(L.ckb_chemkin_reaction_origin(h, j, C.byref(org), C.byref(rev)), "ckb_chemkin_reaction_origin")
+            m.origin[j], m.is_reverse[j] = org.value, rev.value
+        return m
+    finally:
+        L.ckb_chemkin_free(h)
 
 
 class Mech:

@@ -117,7 +117,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
         return LIB
     _embed_sources()
     jobs = []
-    for src in ("ckb_api.cu", "ckb_pack.cu", "ckb_order.cu", "ckb_probe.cu", "ckb_gen.cu", "ckb_thread.cu"):
+    for src in ("ckb_api.cu", "ckb_pack.cu", "ckb_order.cu", "ckb_probe.cu", "ckb_gen.cu", "ckb_thread.cu", "ckb_chemkin.cu"):
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
         jobs.append((obj, [NVCC, *flags, "-c", os.path.join(CSRC, src), "-o", obj]))
     for (L, NV) in instantiations():
