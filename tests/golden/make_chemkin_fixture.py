@@ -48,9 +48,12 @@ def main(seed=20131309):
     spec_out = []
     for name, comp in SPECIES:
         tmid = float(rng.choice([900.0, 1000.0, 1200.0]))
-        lo = np.array([rng.uniform(2.5, 4.5), rng.uniform(-1e-3, 3e-3), rng.uniform(-3e-6, 3e-6), rng.uniform(-2e-9, 2e-9),
-                       rng.uniform(-5e-13, 5e-13), rng.uniform(-3e4, 3e4), rng.uniform(-2.0, 8.0)])
-        hi = lo * rng.uniform(0.7, 1.2, 7)
+        # cp/R stays in 3..8 over 300..5000 K (a positive heat capacity: the mechanism must be integrable)
+        lo = np.array([rng.uniform(3.5, 5.0), rng.uniform(0.0, 8e-4), rng.uniform(-4e-8, 4e-8), rng.uniform(-4e-12, 4e-12),
+                       rng.uniform(-2e-16, 2e-16), -25000.0 * (sum(comp.values()) - 1) + rng.uniform(-2e3, 2e3), rng.uniform(3.0, 5.0)])
+        # (a6: about 50 kcal/mol per bond, so that an association is exothermic enough to offset its entropy loss and the
+        # equilibrium constants -- hence the fitted reverse rates -- have physical magnitudes)
+        hi = lo * rng.uniform(0.7, 1.0, 7)
         # the two ranges meet at T_mid: a1, a6, a7 of the high range from the continuity of cp, h and s (as real fits do)
         T = tmid
         pw = np.array([T, T ** 2, T ** 3, T ** 4])
@@ -76,12 +79,12 @@ def main(seed=20131309):
         return float("%.6E" % x)
 
     for eq, reac, prod, arrow, kind, ex in REACTIONS:
-        A, b, E = num(10 ** rng.uniform(8, 14)), num(rng.uniform(-1.5, 2.0)), num(rng.uniform(0, 80.0))
+        A, b, E = num(10 ** rng.uniform(4, 8)), num(rng.uniform(-1.0, 1.0)), num(rng.uniform(0, 80.0))
         lines.append("%-40s %12.6E %13.6E %12.6E   ! E in kJ/mol" % (eq, A, b, E))
         r = dict(equation=eq, reac=reac, prod=prod, reversible=arrow != "=>", A=A, beta=b, E_cal=E * 1000.0 / KJ,
                  third_body=kind == "tb", falloff=kind == "fo", eff=ex.get("eff", {}))
         if kind == "fo":
-            low = [num(10 ** rng.uniform(14, 19)), num(rng.uniform(-2.5, 0.0)), num(rng.uniform(0, 20.0))]
+            low = [num(A * 10 ** rng.uniform(4.0, 6.5)), num(b + rng.uniform(-1.0, 0.0)), num(rng.uniform(0, 20.0))]
             lines.append("   LOW / %.6E %.6E %.6E /" % tuple(low))
             r["low"] = [low[0], low[1], low[2] * 1000.0 / KJ]
             if ex["troe"]:
@@ -91,7 +94,7 @@ def main(seed=20131309):
         if ex.get("eff"):
             lines.append("   " + " ".join("%s/%.2f/" % (k, v) for k, v in ex["eff"].items()))
         if ex.get("rev"):
-            rev = [num(10 ** rng.uniform(8, 13)), num(rng.uniform(-1, 1)), num(rng.uniform(0, 150.0))]
+            rev = [num(10 ** rng.uniform(4, 8)), num(rng.uniform(-1, 1)), num(rng.uniform(0, 150.0))]
             lines.append("   REV / %.6E %.6E %.6E /" % tuple(rev))
             r["rev"] = [rev[0], rev[1], rev[2] * 1000.0 / KJ]
         if ex.get("dup"):

@@ -131,11 +131,17 @@ def test_units_and_separate_thermo_file():
         assert np.allclose(other.arr_A, base.arr_A, rtol=1e-7) and np.allclose(other.fo_low, base.fo_low, rtol=1e-7)
 
 
+def _without_last_low(text):
+    lines = text.splitlines()
+    last = max(i for i, l in enumerate(lines) if l.strip().startswith("LOW"))
+    return "\n".join(lines[:last] + lines[last + 1:]) + "\n"
+
+
 def test_syntax_errors_are_reported():
     cases = [
         (INP.replace("H+O2=O+OH ", "H+O2=O+XYZ "), binding.EINVAL, "unknown species"),
         (INP.replace("2OH=O+H2O", "2OH=O+H2O2"), binding.EINVAL, "not balanced"),
-        ("\n".join(l for l in INP.splitlines() if not l.startswith("   LOW / 9.050485E+15")) + "\n", binding.EINVAL, "without LOW"),
+        (_without_last_low(INP), binding.EINVAL, "without LOW"),
         (INP.replace("   N2/1.40/", "   SRI / 0.5 100. 200. /"), binding.EUNSUPPORTED, "SRI"),
         (INP.replace("H+H+M=H2+M", "H+H+M=H2"), binding.EINVAL, "third body"),
         (INP.replace("HO2  H2O2  N2  AR  NO  N", "HO2  H2O2  N2  AR  NO  N  HE"), binding.EINVAL, "no thermodynamic data"),
@@ -155,7 +161,9 @@ def test_parsed_mechanism_runs_on_the_gpu_and_matches_the_oracle():
     om = oracle.OracleMech(m)
     rng = np.random.default_rng(1)
     N, K = 96, m.n_species
-    states = np.ascontiguousarray(np.vstack([rng.uniform(1000, 2200, N)[None, :], rng.dirichlet(np.ones(K), size=N).T]))
+    # 900-1500 K, dt = 1e-6 s: sigma up to ~1e9 1/s, RKC with 2-3 stages, RKCK with a few rejections per system; the oracle
+    # perturbed by one ulp takes the same decisions on all 96 systems there (hotter states reach s > 100: DESIGN.md 4.6)
+    states = np.ascontiguousarray(np.vstack([rng.uniform(900, 1500, N)[None, :], rng.dirichlet(np.ones(K), size=N).T]))
     p = 1.01325e6
     ref = np.stack([om.rhs(states[:, i].copy(), p) for i in range(N)], axis=1)
     h = binding.mech_load(m)
@@ -165,4 +173,4 @@ def test_parsed_mechanism_runs_on_the_gpu_and_matches_the_oracle():
         assert (np.abs(out - ref) <= 1e-11 * scale + 1e-13 * np.abs(ref)).all(), v
     h.close()
     for method, variant in (("rkck", "thread"), ("rkc", "warp"), ("rkc", "gen")):
-        _compare(_run_gpu(m, states, p, 1e-7, method, variant=variant), _oracle(m, states, p, 1e-7, method), max_flip_frac=0.03)
+        _compare(_run_gpu(m, states, p, 1e-6, method, variant=variant), _oracle(m, states, p, 1e-6, method), max_flip_frac=0.03)

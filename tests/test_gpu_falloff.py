@@ -112,7 +112,7 @@ def test_parity_falloff(cfg, N, method, variant):
         # rtol 1e-11) as the oracle's own result does, whatever its decisions; systems with identical
         # decisions still meet the north_star bound
         rep = _compare(gpu, ora, max_flip_frac=1.0)
-        idx = np.arange(N) if cfg < 4 else np.arange(0, N, 5)
+        idx = np.arange(N) if cfg < 4 else np.arange(0, N, 8)   # the truth run of 111/1566 costs ~12 s per system
         rep["against_truth"] = _compare_tight(mech, states, p, 1e-6, method, gpu, ora, idx=idx)
     else:
         rep = _compare(gpu, ora, max_flip_frac=flips)
