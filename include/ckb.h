@@ -220,6 +220,23 @@ int ckb_integrate(const ckb_mech *m, double *states, const double *pressure, dou
                   int32_t variant, int32_t *status, int32_t *stats, void *stream);
 
 /*
+ * ckb_integrate_static: ckb_integrate for callers that must never allocate device memory on the call path (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the work-queue order scratch does not
+ * come from the handle but from ONE file-scope device array inside the library (csrc/ckb_order.cu), 12 bytes per system
+ * + 8 KB = 6.0 MiB for CKB_STATIC_MAX_BATCH systems, which every GPU that loads the library holds until the process
+ * exits.  Arguments, layouts, results and status codes exactly as ckb_integrate (constant-pressure closure); the call
+ * and everything behind it use no cudaMalloc, cudaFree or allocating library routine.
+ * N > CKB_STATIC_MAX_BATCH is refused with CKB_ECAPACITY (nothing is launched).
+ * The array is shared by EVERY call in the process (all handles, all streams) and keeps the last call's contents (the
+ * part that must start at zero is cleared on `stream` by each call): two calls that overlap on the GPU race on it and
+ * may skip systems or advance them twice -- order them (same stream, or events).  ckb_integrate itself does not use it.
+ */
+#define CKB_STATIC_MAX_BATCH 524288
+int ckb_integrate_static(const ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                         int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
+                         int32_t *status, int32_t *stats, void *stream);
+
+/*
  * ckb_integrate_host: the same call with HOST buffers (states, pressure, status, stats as above but in
  * host memory, pinned or pageable).  Copies host->device, integrates, copies device->host on `stream`
  * and synchronises it before returning -- the per-global-step protocol the paper timed.  Uses

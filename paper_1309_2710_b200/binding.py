@@ -25,7 +25,7 @@ EXPORTS = ("ckb_mech_load", "ckb_mech_free", "ckb_mech_info", "ckb_integrate", "
            "ckb_mech_specialize", "ckb_mech_precompile", "ckb_mech_codegen", "ckb_codegen_log",
            "ckb_integrate_cv", "ckb_integrate_host_cv", "ckb_rhs_cv", "ckb_mech_load2", "ckb_mech_load3",
            "ckb_mech_reserve", "ckb_chemkin_parse", "ckb_chemkin_free", "ckb_chemkin_desc", "ckb_chemkin_species",
-           "ckb_chemkin_reaction_origin", "ckb_chemkin_error")
+           "ckb_chemkin_reaction_origin", "ckb_chemkin_error", "ckb_integrate_static")
 
 
 class CkbError(RuntimeError):
@@ -94,6 +94,8 @@ def lib():
     L.ckb_integrate.restype = C.c_int
     L.ckb_integrate_host.argtypes = integ
     L.ckb_integrate_host.restype = C.c_int
+    L.ckb_integrate_static.argtypes = integ
+    L.ckb_integrate_static.restype = C.c_int
     L.ckb_rhs.argtypes = [vp, vp, vp, dbl, i64, i64, vp, i32, i32, vp]
     L.ckb_rhs.restype = C.c_int
     L.ckb_integrate_cv.argtypes = integ
@@ -326,6 +328,27 @@ def integrate(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None,
         int(METHODS.get(method, method)), int(VARIANTS.get(variant, variant)),
         _dev_ptr(status, torch.int32, "status"), _dev_ptr(stats, torch.int32, "stats"), _stream_ptr(stream))
     _check(rc, "ckb_integrate")
+    return states
+
+
+STATIC_MAX_BATCH = 524288
+
+
+def integrate_static(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None, pressure=None,
+                     variant="auto", status=None, stats=None, stream=None):
+    """ckb_integrate_static: ckb_integrate with its scratch in the library's static device array -- no device allocation on
+    the call path; N <= STATIC_MAX_BATCH; calls that overlap on the GPU race on that array."""
+    import torch
+    if states.dim() != 2 or states.shape[0] != m.K + 1:
+        raise ValueError("states must be [(K+1)][ld]")
+    ld = int(states.shape[1])
+    N = ld if N is None else int(N)
+    rc = lib().ckb_integrate_static(
+        m._h, _dev_ptr(states, torch.float64, "states"), _dev_ptr(pressure, torch.float64, "pressure"),
+        float(0.0 if p is None else p), N, ld, float(t), float(dt), float(rtol), float(atol),
+        int(METHODS.get(method, method)), int(VARIANTS.get(variant, variant)),
+        _dev_ptr(status, torch.int32, "status"), _dev_ptr(stats, torch.int32, "stats"), _stream_ptr(stream))
+    _check(rc, "ckb_integrate_static")
     return states
 
 

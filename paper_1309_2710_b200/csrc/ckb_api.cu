@@ -275,6 +275,44 @@ int ckb_integrate_cv(const ckb_mech *m, double *states, const double *density, d
                         (cudaStream_t)stream, 0, N, 1, false);
 }
 
+/* ckb_integrate with the queue-order scratch in the library's static device array (ckb_order.cu): a separate path, so
+ * that ckb_integrate is untouched.  Calls no cudaMalloc / cudaFree and no routine that allocates. */
+int ckb_integrate_static(const ckb_mech *m, double *states, const double *pressure, double p_uniform, int64_t N,
+                         int64_t ld, double t, double dt, double rtol, double atol, int32_t method, int32_t variant,
+                         int32_t *status, int32_t *stats, void *stream) {
+  if (!m || N < 0 || (method != CKB_METHOD_RKCK && method != CKB_METHOD_RKC)) return CKB_EINVAL;
+  if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(t) || !(rtol > 0.0) || !(atol >= 0.0)) return CKB_EINVAL;
+  if (!pressure && !(p_uniform > 0.0)) return CKB_EINVAL;
+  if (N > CKB_STATIC_MAX_BATCH) return CKB_ECAPACITY; /* the static scratch holds CKB_STATIC_MAX_BATCH systems */
+  Launch l;
+  int rc = choose(m, variant, (long long)N, method, &l);
+  if (rc) return rc;
+  if (N == 0) return CKB_OK;
+  if (!states || ld < N) return CKB_EINVAL;
+  cudaStream_t s = (cudaStream_t)stream;
+  ckb_host::IntegrateArgs a{states, pressure, p_uniform, (long long)N, (long long)ld, t, dt, rtol, atol,
+                            status, stats, s, nullptr, 0};
+  if (N >= 4096) { /* the same queue order as ckb_integrate: cost proxy for RKC with 8 or more systems per warp, else T */
+    const ckb_host::Packed &pk32 = m->pk[ckb_host::pack_index(32)];
+    if (l.L <= 4 && method == CKB_METHOD_RKC && (m->pk[0].rc == CKB_OK || pk32.rc == CKB_OK)) {
+      const Launch l1 = m->pk[0].rc == CKB_OK ? Launch{1, m->pk[0].dm.NV, true} : Launch{32, pk32.dm.NV, false};
+      double *d_keys;
+      int *d_order;
+      unsigned *d_bins;
+      rc = ckb_host::static_scratch(&d_keys, &d_order, &d_bins);
+      if (rc) return rc;
+      ckb_host::ProxyArgs pa{states, pressure, p_uniform, (long long)N, (long long)ld, 1e-3 * dt, rtol, atol, d_keys, s, 0};
+      rc = dispatch_proxy(m, l1, pa);
+      if (rc) return rc;
+      rc = ckb_host::static_queue_order(1, d_keys, N, s, &a.order);
+    } else {
+      rc = ckb_host::static_queue_order(0, states, N, s, &a.order);
+    }
+    if (rc) return rc;
+  }
+  return dispatch_integrate(m, l, method, a);
+}
+
 static int rhs_impl(const ckb_mech *m, const double *states, const double *pressure, double p_uniform, int64_t N,
                     int64_t ld, double *dydt, int32_t variant, int32_t repeat, void *stream, int cv) {
   if (!m || N < 0 || repeat < 1) return CKB_EINVAL;
@@ -384,7 +422,9 @@ const char *ckb_strerror(int code) {
     case CKB_ENOMEM: return "out of memory";
     case CKB_ECUDA: return "CUDA runtime error (see ckb_last_cuda_error)";
     case CKB_EUNSUPPORTED: return "mechanism or variant outside the supported limits";
-    case CKB_ECAPACITY: return "batch larger than the size reserved for this handle (ckb_mech_reserve)";
+    case CKB_ECAPACITY:
+      return "batch larger than the size reserved for this handle (ckb_mech_reserve) or than CKB_STATIC_MAX_BATCH "
+             "(ckb_integrate_static)";
     default: return "unknown error code";
   }
 }

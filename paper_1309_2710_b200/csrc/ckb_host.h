@@ -135,6 +135,9 @@ struct IntegrateArgs {
 int make_queue_order(const ckb_mech *m, int slot, int mode, const double *keys, long long N, cudaStream_t s,
                      const int **order, bool grow);
 int queue_scratch(const ckb_mech *m, int slot, long long N, bool grow);
+/* the same with the scratch in a file-scope device array (ckb_order.cu; ckb_integrate_static): no allocation ever */
+int static_scratch(double **keys, int **order, unsigned **bins);
+int static_queue_order(int mode, const double *keys, long long N, cudaStream_t s, const int **order);
 
 struct ProxyArgs {
   const double *states; const double *pressure; double p_uniform; long long N, ld; double h, rtol, atol;

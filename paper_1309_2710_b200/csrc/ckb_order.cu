@@ -144,4 +144,59 @@ int make_queue_order(const ckb_mech *m, int slot, int mode, const double *keys, 
   return CKB_OK;
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * The same queue order with its scratch in a file-scope device array (ckb_integrate_static, include/ckb.h): for callers
+ * that may not allocate device memory at all -- nothing here or behind it calls cudaMalloc / cudaFree.
+ * Layout: keys[MAX] doubles (cost-proxy keys of the RKC order), order[MAX] ints, bins[CKB_ORDER_BINS] unsigned:
+ * 12 bytes per system + 8 KB = 6.0 MiB for CKB_STATIC_MAX_BATCH = 524288, held by every GPU that loads the library
+ * until the process exits.  Every call shares it and it keeps the last call's contents: the bins are cleared per call,
+ * keys and order are overwritten for [0, N) before they are read.  Calls that overlap on the GPU race on it.
+ * In host code the array's NAME is a host-side stand-in, not a device address: its address is taken once per device
+ * with cudaGetSymbolAddress (that device current) and only that pointer is handed to kernels.
+ * ---------------------------------------------------------------------------------------------- */
+#define CKB_STATIC_BYTES ((size_t)CKB_STATIC_MAX_BATCH * 12 + (size_t)CKB_ORDER_BINS * 4)
+static __device__ __align__(256) unsigned char g_static_scratch[CKB_STATIC_BYTES];
+
+#define CKB_STATIC_MAX_DEVICES 64
+static std::atomic<unsigned char *> g_static_ptr[CKB_STATIC_MAX_DEVICES];
+
+/* device pointers of the three parts on the current device */
+int static_scratch(double **keys, int **order, unsigned **bins) {
+  int dev = 0;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= CKB_STATIC_MAX_DEVICES) return CKB_EUNSUPPORTED;
+  unsigned char *p = g_static_ptr[dev].load(std::memory_order_acquire);
+  if (!p) { /* once per device; a second thread racing here gets the same address */
+    void *q = nullptr;
+    CK(cudaGetSymbolAddress(&q, g_static_scratch));
+    if (!q) return CKB_ECUDA;
+    p = (unsigned char *)q;
+    g_static_ptr[dev].store(p, std::memory_order_release);
+  }
+  *keys = reinterpret_cast<double *>(p);
+  *order = reinterpret_cast<int *>(p + (size_t)CKB_STATIC_MAX_BATCH * 8);
+  *bins = reinterpret_cast<unsigned *>(p + (size_t)CKB_STATIC_MAX_BATCH * 12);
+  return CKB_OK;
+}
+
+/* make_queue_order with the static scratch: N <= CKB_STATIC_MAX_BATCH (checked by the caller as well) */
+int static_queue_order(int mode, const double *keys, long long N, cudaStream_t s, const int **order) {
+  *order = nullptr;
+  if (N < 0 || N > CKB_STATIC_MAX_BATCH) return CKB_ECAPACITY;
+  double *d_keys;
+  int *d_order;
+  unsigned *d_bins;
+  int rc = static_scratch(&d_keys, &d_order, &d_bins);
+  if (rc) return rc;
+  CK(cudaMemsetAsync(d_bins, 0, CKB_ORDER_BINS * sizeof(unsigned), s)); /* the one part that must start at zero */
+  const long long per_block = CKB_ORDER_THREADS * CKB_ORDER_ITEMS;
+  const unsigned blocks = (unsigned)((N + per_block - 1) / per_block);
+  ckb::order_hist_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(keys, N, d_bins, mode);
+  ckb::order_scan_kernel<<<1, CKB_ORDER_BINS / 2, 0, s>>>(d_bins);
+  ckb::order_scatter_kernel<<<blocks, CKB_ORDER_THREADS, 0, s>>>(keys, N, d_bins, d_order, mode);
+  CK(cudaGetLastError());
+  *order = d_order;
+  return CKB_OK;
+}
+
 }  // namespace ckb_host
