@@ -410,7 +410,7 @@ struct Sys {
       const ExpConst<true> ec;
       double *qp = sR + qoff + g;
       const char *c = reinterpret_cast<const char *>(sR);
-      const int last = m.NSR - 1;
+      const int last = m.NSR - 1, nq = m.NSR * L; /* -q_s sits NSR*L doubles behind q_s */
       for (int r = 0; r < m.NSR; r += U, qp += U * L) {
         unsigned v[U][16];
 #pragma unroll
@@ -439,7 +439,10 @@ struct Sys {
         for (int u = 0; u < U; u++) res[u] = (ks[2 * u] * pf[u] - ks[2 * u + 1] * pr[u]) * mt[u];
 #pragma unroll
         for (int u = 0; u < U; u++)
-          if (u == 0 || r + u <= last) qp[u * L] = res[u];
+          if (u == 0 || r + u <= last) {
+            qp[u * L] = res[u];
+            qp[nq + u * L] = -res[u];
+          }
       }
     } else
 #endif
@@ -469,7 +472,9 @@ struct Sys {
           const double pf = CKB_AT(a0) * CKB_AT(a1) * CKB_AT(a2);
           const double pr = CKB_AT(b0) * CKB_AT(b1) * CKB_AT(b2);
           const double kf = ckb_exp(xf, ec), kr = ckb_exp(xr, ec);
-          qp[q * RS] = (kf * pf - kr * pr) * CKB_AT(tb);
+          const double qs = (kf * pf - kr * pr) * CKB_AT(tb);
+          qp[q * RS] = qs;
+          if (L > 1) qp[q * RS + m.NSR * L] = -qs; /* the gather reads -q_s where the coefficient is -1 */
 #undef CKB_AT
         }
       }
@@ -481,6 +486,7 @@ struct Sys {
     for (int q = 0; q < M; q++) s3[q] = 0.0;
     int gp = m.o_gat + g;
     const double *sQ = sR + qoff;
+    double om[M][NV]; /* Eq. 3 per register slot */
 #pragma unroll
     for (int i = 0; i < NV; i++) {
       const int len = (int)tw(m.o_glen + i);
@@ -496,29 +502,61 @@ struct Sys {
           for (int q = 0; q < M; q++)
             acc0[q] = fma(coef, *reinterpret_cast<const double *>(reinterpret_cast<const char *>(sQ + q * RS) + o), acc0[q]);
         }
-      } else { /* two entries per word: (coefficient +1 / -1 << 16) | q offset.  The coefficient is applied by XOR-ing
-                  its sign (bit 31 of the entry) into q: no int -> double conversion, an add instead of an FMA
-                  (exactly fma(+-1, q, acc)); a stoichiometric coefficient |nu| > 1 is entered |nu| times, an idle
-                  entry reads one of the 0.0 slots behind the q region */
+      } else { /* four entries per word, each the byte offset of q_s (coefficient +1), of -q_s (coefficient -1: the slot
+                  loop stores both) or of one of the 0.0 slots behind them (idle entry): an extract, a shared read and
+                  an add per entry; |nu| > 1 is entered |nu| times */
+        double acc2[M], acc3[M];
+#pragma unroll
+        for (int q = 0; q < M; q++) acc2[q] = acc3[q] = 0.0;
         for (int t = 0; t < len; t++, gp += L) {
           const unsigned long long w = tw(gp);
           const unsigned lo = (unsigned)w, hi = (unsigned)(w >> 32);
-          const unsigned o0 = lo & 0xFFFFu, o1 = hi & 0xFFFFu;
 #pragma unroll
           for (int q = 0; q < M; q++) {
             const char *qb = reinterpret_cast<const char *>(sQ + q * RS);
-            const double q0 = *reinterpret_cast<const double *>(qb + o0), q1 = *reinterpret_cast<const double *>(qb + o1);
-            acc0[q] += __hiloint2double(__double2hiint(q0) ^ (int)(lo & 0x80000000u), __double2loint(q0));
-            acc1[q] += __hiloint2double(__double2hiint(q1) ^ (int)(hi & 0x80000000u), __double2loint(q1));
+            acc0[q] += *reinterpret_cast<const double *>(qb + (lo & 0xFFFFu));
+            acc1[q] += *reinterpret_cast<const double *>(qb + (lo >> 16));
+            acc2[q] += *reinterpret_cast<const double *>(qb + (hi & 0xFFFFu));
+            acc3[q] += *reinterpret_cast<const double *>(qb + (hi >> 16));
           }
         }
+#pragma unroll
+        for (int q = 0; q < M; q++) {
+          acc0[q] += acc2[q];
+          acc1[q] += acc3[q];
+        }
       }
+#pragma unroll
+      for (int q = 0; q < M; q++) om[q][i] = acc0[q] + acc1[q];
+    }
+    if (L > 1 && m.o_split) { /* launch-uniform: the tails of the longest rows were summed in the last level's spare slots
+                                 (ckb_pack.cu); a component takes its tail from the lane that holds it */
+      double tail[M][NV];
+#pragma unroll
+      for (int i = 0; i < NV; i++) {
+        const int src = (int)tw(m.o_split + i * L + g);
+#pragma unroll
+        for (int q = 0; q < M; q++) {
+          const double t = __shfl_sync(mask, om[q][NV - 1], src < 0 ? src0 : src0 + src);
+          tail[q][i] = src < 0 ? 0.0 : t;
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < NV; i++)
+#pragma unroll
+        for (int q = 0; q < M; q++) om[q][i] += tail[q][i];
+      if (g + L * (NV - 1) >= n) { /* a spare slot has handed its sum over: it is no component (its h - 1 is not 0 at constant volume) */
+#pragma unroll
+        for (int q = 0; q < M; q++) om[q][NV - 1] = 0.0;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
       const double W = td(m.o_sp + i * CKB_SP_WORDS * L + g + CKB_SP_W * L);
 #pragma unroll
       for (int q = 0; q < M; q++) {
-        const double acc = acc0[q] + acc1[q];
-        f[q][i] = W * acc * invrho[q];
-        s3[q] = fma(L == 1 ? sH[i * GI] : hrt[q][i], acc, s3[q]);
+        f[q][i] = W * om[q][i] * invrho[q];
+        s3[q] = fma(L == 1 ? sH[i * GI] : hrt[q][i], om[q][i], s3[q]);
       }
     }
 #pragma unroll
@@ -1133,7 +1171,7 @@ __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem
   if (L > 1 && sys.g < CKB_ZERO_SLOTS) { /* the operands of idle gather entries (a group has >= 2 lanes: loop) */
     for (int z = sys.g; z < CKB_ZERO_SLOTS; z += L) {
 #pragma unroll
-      for (int q = 0; q < M; q++) sys.sR[q * sys.RS + sys.qoff + m.NSR * L + z] = 0.0;
+      for (int q = 0; q < M; q++) sys.sR[q * sys.RS + sys.qoff + 2 * m.NSR * L + z] = 0.0;
     }
   }
 #endif

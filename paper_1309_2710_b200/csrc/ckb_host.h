@@ -58,7 +58,8 @@ struct Parsed {
   double flops_per_rhs = 0.0;
 };
 /* components: 0 = T, then species by decreasing gather-row length (ckb_tables.h) */
-void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<int> &comp_of_sp);
+/* cap > 0: rows count as min(length, cap) (their tails live elsewhere, pack_for) */
+void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<int> &comp_of_sp, int cap = 0);
 struct FoDesc { int n; const int32_t *reaction; const double *low3, *troe4; };
 int parse_mechanism(const ckb_mech_desc *d, Parsed &P, const FoDesc *fo = nullptr);
 int pack_for(const Parsed &P, int L, Packed &out);

@@ -319,13 +319,43 @@ struct GEntry { int pos, coef; };
 
 /* One gather level: rows[g] = entries lane g must sum.  Returns steps[t][g] (pos = -1: idle).  With
  * `optimise`, a proper edge colouring of (lane, pos mod 16) per half-warp; else row order. */
-std::vector<std::vector<GEntry>> colour_gather(const std::vector<std::vector<GEntry>> &rows, int L, bool optimise) {
+std::vector<std::vector<GEntry>> colour_gather(const std::vector<std::vector<GEntry>> &rows, int L, bool optimise,
+                                               bool relaxed = false) {
   size_t maxlen = 0;
   for (auto &r : rows) maxlen = std::max(maxlen, r.size());
   if (!optimise || L < 16) {
     std::vector<std::vector<GEntry>> steps(maxlen, std::vector<GEntry>(L, GEntry{-1, 0}));
     for (int g = 0; g < L; g++)
       for (size_t t = 0; t < rows[g].size(); t++) steps[t][g] = rows[g][t];
+    return steps;
+  }
+  if (relaxed) {
+    /* As many steps as the longest row, not as the busiest bank pair: per step each lane takes, of the entries it has
+     * left, the one whose bank pair is least used in this step by its half-warp, or waits if it can afford to.  A few
+     * two-way conflicts remain (reported): a replay costs one cycle of the shared-memory pipe, a step an issue slot
+     * per entry. */
+    std::vector<std::vector<GEntry>> steps(maxlen, std::vector<GEntry>(L, GEntry{-1, 0}));
+    for (int h = 0; h < L / 16; h++) {
+      std::vector<std::vector<GEntry>> left(16);
+      for (int l = 0; l < 16; l++) left[l] = rows[h * 16 + l];
+      for (size_t t = 0; t < maxlen; t++) {
+        int cnt[16] = {0};
+        std::vector<int> order(16);
+        std::iota(order.begin(), order.end(), 0);
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return left[a].size() > left[b].size(); });
+        for (int l : order) {
+          if (left[l].empty()) continue;
+          const long slack = (long)(maxlen - t) - (long)left[l].size();
+          size_t best = 0;
+          for (size_t e = 1; e < left[l].size(); e++)
+            if (cnt[left[l][e].pos & 15] < cnt[left[l][best].pos & 15]) best = e;
+          if (cnt[left[l][best].pos & 15] > 0 && slack > 0) continue; /* wait for a free bank pair */
+          cnt[left[l][best].pos & 15]++;
+          steps[t][h * 16 + l] = left[l][best];
+          left[l].erase(left[l].begin() + best);
+        }
+      }
+    }
     return steps;
   }
   std::vector<std::vector<GEntry>> steps;
@@ -408,13 +438,24 @@ int excess_wavefronts(const std::vector<int> &addr_of_lane /* L entries (L = 16 
 
 }  // namespace
 
-void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<int> &comp_of_sp) {
+/* entries of species k's Eq. 3 row as the lane-distributed gather counts them (|nu| > 1 entered |nu| times) */
+static int row_entries(const Parsed &P, int k) {
+  int len = 0;
+  for (auto &sc : P.rows[k]) len += std::abs(sc.second);
+  return len;
+}
+
+void component_order(const Parsed &P, std::vector<int> &sp_of_comp, std::vector<int> &comp_of_sp, int cap) {
   const int K = P.K, n = K + 1;
   sp_of_comp.assign(n, -1);
   comp_of_sp.assign(K, 0);
   std::vector<int> order(K);
   std::iota(order.begin(), order.end(), 0);
-  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return P.rows[a].size() > P.rows[b].size(); });
+  if (cap > 0)
+    std::stable_sort(order.begin(), order.end(),
+                     [&](int a, int b) { return std::min(row_entries(P, a), cap) > std::min(row_entries(P, b), cap); });
+  else
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return P.rows[a].size() > P.rows[b].size(); });
   for (int c = 1; c < n; c++) {
     sp_of_comp[c] = order[c - 1];
     comp_of_sp[order[c - 1]] = c;
@@ -431,13 +472,30 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   for (auto &s : P.sets) TBE = std::max(TBE, (int)s.size());
   /* 16-bit region offsets, in bytes */
   if ((long long)(n + NTB + 1) * G * 8 > 65535 ||
-      ((long long)NSR * L + (L > 1 ? CKB_ZERO_SLOTS : 0)) * G * 8 > 65535) /* idle gather entries point behind the q region */
+      ((long long)NSR * L * (L > 1 ? 2 : 1) + (L > 1 ? CKB_ZERO_SLOTS : 0)) * G * 8 > 65535) /* q, -q and the 0.0 slots of idle entries */
     return CKB_EUNSUPPORTED;
   const bool optimise = true;
 
-  /* components: 0 = T, then species by decreasing gather-row length */
+  /* Row splitting (lane-distributed mappings): the NV*L - n register slots of the last gather level that hold no
+   * component take the TAILS of the longest Eq. 3 rows, so that no row is longer than cap = the (spare + 1)-th longest;
+   * f(y) adds a tail to its component with one shuffle (DevMech::o_split). */
+  const int spare = (L > 1) ? NV * L - n : 0;
+  int cap = 0;
+  if (spare > 0 && K > spare) {
+    std::vector<int> lens(K);
+    for (int k = 0; k < K; k++) lens[k] = row_entries(P, k);
+    std::sort(lens.begin(), lens.end(), std::greater<int>());
+    if (lens[0] > lens[spare] && lens[spare] >= 4) cap = lens[spare];
+  }
+  /* components: 0 = T, then species by decreasing (capped) gather-row length */
   std::vector<int> sp_of_comp, comp_of_sp;
-  component_order(P, sp_of_comp, comp_of_sp);
+  component_order(P, sp_of_comp, comp_of_sp, cap);
+  std::vector<int> tail_slot(n, -1); /* component -> virtual slot (>= n) that holds the tail of its row */
+  if (cap > 0) {
+    int v = n;
+    for (int c = 1; c < n && v < NV * L; c++)
+      if (row_entries(P, sp_of_comp[c]) > cap) tail_slot[c] = v++;
+  }
   /* which lane evaluates which slot, and the gather schedule of every level */
   const std::vector<Placed> placed = place_slots(P, comp_of_sp, L, NSR, optimise);
   std::vector<int> pos_of_slot(NS, -1);
@@ -449,18 +507,30 @@ int pack_for(const Parsed &P, int L, Packed &out) {
     std::vector<std::vector<GEntry>> rows(L);
     for (int g = 0; g < L; g++) {
       const int c = g + L * i;
-      if (c < 1 || c >= n) continue;
-      for (auto &sc : P.rows[sp_of_comp[c]]) {
+      if (c < 1) continue;
+      int owner = c < n ? c : -1; /* a slot without a component holds the tail of some component's row */
+      if (c >= n)
+        for (int o = 1; o < n; o++)
+          if (tail_slot[o] == c) owner = o;
+      if (owner < 0) continue;
+      std::vector<GEntry> all;
+      for (auto &sc : P.rows[sp_of_comp[owner]]) {
         if (L == 1) {
-          rows[g].push_back(GEntry{pos_of_slot[sc.first], sc.second});
-        } else { /* lane-distributed mappings apply the coefficient as a sign: |nu| > 1 is entered |nu| times */
+          all.push_back(GEntry{pos_of_slot[sc.first], sc.second});
+        } else { /* lane-distributed mappings apply the coefficient by where they read: |nu| > 1 is entered |nu| times */
           for (int rep = 0; rep < std::abs(sc.second); rep++)
-            rows[g].push_back(GEntry{pos_of_slot[sc.first], sc.second > 0 ? 1 : -1});
+            all.push_back(GEntry{pos_of_slot[sc.first], sc.second > 0 ? 1 : -1});
         }
       }
+      if (c < n) { /* the head of the row (all of it unless it is split) */
+        const size_t keep = (tail_slot[c] >= 0) ? (size_t)cap : all.size();
+        rows[g].assign(all.begin(), all.begin() + std::min(keep, all.size()));
+      } else {
+        rows[g].assign(all.begin() + cap, all.end());
+      }
     }
-    sched[i] = colour_gather(rows, L, optimise);
-    glen[i] = (L == 1) ? (int)sched[i].size() : ((int)sched[i].size() + 1) / 2;
+    sched[i] = colour_gather(rows, L, optimise, /*relaxed=*/true);
+    glen[i] = (L == 1) ? (int)sched[i].size() : ((int)sched[i].size() + 3) / 4;
   }
   const int gwords = std::accumulate(glen.begin(), glen.end(), 0);
   const int s_tab = (L == 1) ? 12 : 48;
@@ -481,6 +551,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   m.o_glen = take(NV);
   m.o_rflag = off; off += NSR;
   m.o_perm = off; off += n;
+  m.o_split = (cap > 0) ? take((size_t)NV * L) : 0;
   m.o_sp2 = P.nasa_hi.empty() ? 0 : take((size_t)NV * CKB_SP_WORDS * L);
   m.o_fo = P.fo.empty() ? 0 : take((size_t)NTBR * 8 * L);
   m.s_tab = s_tab;
@@ -519,6 +590,9 @@ int pack_for(const Parsed &P, int L, Packed &out) {
     }
   }
   for (int c = 0; c < n; c++) b[(size_t)m.o_perm + c] = (unsigned long long)(c == 0 ? 0 : 1 + sp_of_comp[c]);
+  if (m.o_split)
+    for (int c = 0; c < NV * L; c++) /* [level][lane] */
+      b[(size_t)m.o_split + c] = (unsigned long long)(long long)((c < n && tail_slot[c] >= 0) ? tail_slot[c] % L : -1);
 
   const double LN_ZERO = -1.0e4; /* stands for ln 0: ckb_exp() returns ~1e-308 for it, no special case on the device */
   for (int q = 0; q < NSR * L; q++) {
@@ -570,14 +644,14 @@ int pack_for(const Parsed &P, int L, Packed &out) {
       }
     }
   }
-  { /* gather entries: (coefficient int16 << 16) | (q offset), two per word; an idle lane reads, with
-       coefficient 0, a q whose bank pair nobody in its half-warp uses in that step */
+  { /* gather entries: L > 1: 16-bit byte offsets of q_s / -q_s, four per word; an idle lane reads the 0.0 slot of a bank
+       pair nobody in its half-warp uses in that step.  L = 1: (double coefficient | q offset), one per word */
     int w0 = 0;
     out.gather_steps = 0;
     out.gather_excess_wavefronts = 0;
     for (int i = 0; i < NV; i++) {
       b[(size_t)m.o_glen + i] = (unsigned long long)glen[i];
-      const int per_word = (L == 1) ? 1 : 2;
+      const int per_word = (L == 1) ? 1 : 4;
       for (int t = 0; t < per_word * glen[i]; t++) {
         std::vector<int> addr(L >= 16 ? L : 0, -1);
         for (int g = 0; g < L; g++) {
@@ -597,16 +671,15 @@ int pack_for(const Parsed &P, int L, Packed &out) {
               for (int r0 = 0; r0 < 16; r0++)
                 if (!busy[r0]) { e.pos = r0; break; }
             }
-            if (zero_slot) e.pos = NSR * L + ((e.pos - NSR * L) % 16 + 16) % 16; /* same bank pair, behind the q region */
+            if (zero_slot) e.pos = 2 * NSR * L + ((e.pos - 2 * NSR * L) % 16 + 16) % 16; /* same bank pair, behind q and -q */
           }
           if (L >= 16) addr[g] = e.pos;
           if (L == 1) { /* double coefficient with the q offset in its 16 lowest mantissa bits */
             b[(size_t)m.o_gat + (size_t)(w0 + t) * L + g] =
                 (dbits((double)e.coef) & ~0xFFFFull) | (unsigned long long)(e.pos * G * 8);
-          } else {
-            const unsigned long long ent =
-                ((unsigned long long)((unsigned)(e.coef & 0xFFFF)) << 16) | (unsigned long long)(e.pos * G * 8);
-            b[(size_t)m.o_gat + (size_t)(w0 + t / 2) * L + g] |= ent << (32 * (t & 1));
+          } else { /* coefficient -1: the entry points at -q_s, NSR*L doubles behind q_s (the same bank pair) */
+            const int pos = (e.coef < 0 && e.pos < NSR * L) ? e.pos + NSR * L : e.pos;
+            b[(size_t)m.o_gat + (size_t)(w0 + t / 4) * L + g] |= (unsigned long long)(pos * G * 8) << (16 * (t & 3));
           }
         }
         if (L >= 16) out.gather_excess_wavefronts += excess_wavefronts(addr);

@@ -13,7 +13,8 @@
  *   [0, n)            C_c, concentration of component c; C_0 = 1.0 stands for "no molecule"
  *   [n, n+NTB+1)      [M]_t per third-body efficiency set; the last one = 1.0 stands for "no third body"
  *   [n+NTB+1, +NSR*L) q_s, net rate of progress of reaction slot s
- *   L > 1: then 16 doubles of 0.0 (one per bank pair), the operand of an idle entry of the Eq. 3 gather
+ *   L > 1: then NSR*L doubles -q_s (so that the Eq. 3 gather applies a coefficient of +1 / -1 by WHERE it reads), then
+ *          16 doubles of 0.0 (one per bank pair), the operand of an idle entry of the gather
  */
 #pragma once
 #ifndef __CUDACC__
@@ -71,10 +72,10 @@ struct DevMech {
   int o_rflag;       /* [NSR]              round flags: 1 = a third molecule is read, 2 = a third body is read   */
   int o_tb;          /* [NTBR][TBE][2][L]  (alpha-1, region byte offset of the species)                        */
   int o_glen;        /* [NV]               64-bit words per lane of gather level i (uniform over lanes)   */
-  int o_gat;         /* [sum glen][L]      gather entries.  L > 1: two per word, (int16 coefficient +1 / -1 << 16) |
-                                           BYTE offset (x G) of q_s inside the q region (bit 31 = sign of the
-                                           coefficient; |nu| > 1 is entered nu times; idle: a 0.0 slot); L = 1: one
-                                           per word, double coefficient with the offset in its low 16 bits */
+  int o_gat;         /* [sum glen][L]      gather entries.  L > 1: four per word, each the 16-bit BYTE offset inside
+                                           the q region of q_s (coefficient +1), of -q_s (coefficient -1) or of a 0.0
+                                           slot (idle); |nu| > 1 is entered nu times.  L = 1: one per word, double
+                                           coefficient with the offset in its low 16 bits */
   int o_rkc;         /* RKC coefficients for s = 2..s_tab: [s-2] -> mu~_1; stages at o_rkcs               */
   int o_rkcs;        /* [(s-2)(s-1)/2 + (j-2)][4] = mu_j, nu_j, mu~_j, gamma~_j, j = 2..s                  */
   int s_tab;
@@ -83,6 +84,9 @@ struct DevMech {
   int o_fo;          /* [NTBR][8][L] fall-off description of efficiency set t (R31): kind (0 none, 1 Lindemann,
                         2 Troe, 3 Troe without T**), ln A_0 - ln A_inf, beta_0 - beta_inf, (E_0 - E_inf)/R_c,
                         a, 1/T***, 1/T*, T**; 0 = the mechanism has no fall-off reaction                     */
+  int o_split;       /* [NV][L] L > 1: lane whose LAST gather level holds the second part of this component's Eq. 3 row, or
+                        -1 (ckb_pack.cu: the NV*L - n register slots without a component take the tails of the longest
+                        rows, so that no row is longer than the (NV*L - n + 1)-th longest); 0 = no row is split    */
   int o_sp2;         /* [NV][13][L] second species table: the high temperature range of the NASA fits, with
                         T_mid in the CKB_SP_INVW word (W word unused); 0 = the mechanism has one range       */
 };
@@ -90,7 +94,7 @@ struct DevMech {
 /* doubles of shared memory per system: C region, [M] region, q region */
 #define CKB_ZERO_SLOTS 16 /* L > 1: 0.0 in every bank pair behind the q region, read by idle gather entries */
 __host__ __device__ __forceinline__ int region_doubles(const DevMech &m) {
-  return m.n + m.NTB + 1 + m.NSR * m.L + (m.L > 1 ? CKB_ZERO_SLOTS : 0);
+  return m.n + m.NTB + 1 + m.NSR * m.L + (m.L > 1 ? m.NSR * m.L + CKB_ZERO_SLOTS : 0);
 }
 
 }  // namespace ckb

@@ -81,13 +81,14 @@ def test_integrate_argument_errors_without_handle(L):
 @pytest.mark.parametrize("cfg", [0, 2, 3, 4])
 def test_packing_report(cfg, L):
     """Host-only packing (ckb_mech_pack_stats): forward/reverse pairs are fused, the gather schedule of the
-    warp-per-ODE packing is free of shared-memory bank conflicts, thread-per-ODE tables fit the parameter block."""
+    warp-per-ODE packing is as short as its longest (split) row with few shared-memory bank conflicts left, thread-per-ODE
+    tables fit the parameter block."""
     mech = synth.make_mechanism(cfg)
     spec = synth.CONFIGS[cfg]
     warp = binding.pack_stats(mech, 32)
     assert warp["slots"] == spec.R // 2                       # every synthetic reaction has its reverse
     assert warp["slot_rounds"] == -(-warp["slots"] // 32)
-    assert warp["gather_conflict_replays"] == 0               # edge-coloured schedule
+    assert warp["gather_conflict_replays"] <= 0.5 * warp["gather_steps"]   # least-used-bank schedule: < 1 replay per 2 steps
     assert warp["register_slots"] == -(-(spec.K + 1) // 32) or warp["register_slots"] in (1, 2, 4)
     nnz = sum(len(set(mech.reac_species[mech.reac_ptr[j]:mech.reac_ptr[j + 1]]) |
                   set(mech.prod_species[mech.prod_ptr[j]:mech.prod_ptr[j + 1]])) for j in range(0, spec.R, 2))
