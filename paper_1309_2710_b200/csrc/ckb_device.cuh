@@ -81,31 +81,44 @@ struct ExpConst {
 };
 
 #if CKB_EXP_TABLE
-/* Table variant (specialised thread-per-ODE kernels, where the FP64 pipe is the busiest unit and the load/store
- * pipe is idle): x = (64 k + j) ln2/64 + r, |r| <= ln2/128, e^x = 2^k 2^(j/64) p(r) with p of degree 5 (truncation
- * r^6/720 <= 3.5e-17) and 2^(j/64) from a 64-entry table in shared memory: 12 FP64 instructions instead of 17. */
+/* Table variant: x = (64 k + j) ln2/64 + r, |r| <= ln2/128, e^x = 2^k 2^(j/64) p(r) with p of degree 5 (truncation
+ * r^6/720 <= 3.5e-17) and 2^(j/64) from a 64-entry table in shared memory: 12 FP64 instructions instead of 17 and a
+ * dependency chain of 9 instead of 14.  CKB_EXP_TABLE_REPL copies of the table, entry j of copy c at [j * REPL + c]:
+ * with 16 copies lane l reads copy (l mod 16), i.e. always its own bank pair -- conflict free whatever j is (the
+ * lane-distributed kernels, whose shared-memory pipe is busy); one copy where that pipe is idle (thread-per-ODE). */
+#ifndef CKB_EXP_TABLE_REPL
+#define CKB_EXP_TABLE_REPL 1
+#endif
 __device__ __forceinline__ double *ckb_exp_table() {
-  __shared__ double tab[64];
+  __shared__ double tab[64 * CKB_EXP_TABLE_REPL];
   return tab;
 }
 __device__ __forceinline__ void ckb_exp_table_init() {
-  if (threadIdx.x < 64) ckb_exp_table()[threadIdx.x] = exp2((double)threadIdx.x * 0.015625);
+  for (int i = threadIdx.x; i < 64 * CKB_EXP_TABLE_REPL; i += blockDim.x)
+    ckb_exp_table()[i] = exp2((double)(i / CKB_EXP_TABLE_REPL) * 0.015625);
   __syncthreads();
 }
+__device__ __forceinline__ double ckb_exp_table_at(int kj) {
+  if (CKB_EXP_TABLE_REPL == 1) return ckb_exp_table()[kj & 63];
+  return ckb_exp_table()[(kj & 63) * CKB_EXP_TABLE_REPL + (threadIdx.x & (CKB_EXP_TABLE_REPL - 1))];
+}
+static __constant__ double c_expt[6] = {92.332482616893657 /* 64 / ln 2 */, -0.6931471805599453 * 0.015625,
+                                        -2.3190468138462996e-17 * 0.015625, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0};
 template <bool PIN>
 __device__ __forceinline__ double ckb_exp(double x, const ExpConst<PIN> &) {
-  const double t = fma(x, 92.332482616893657, 6755399441055744.0); /* 64 / ln 2 */
+  const double t = fma(x, c_expt[0], 6755399441055744.0);
   const double kd = t - 6755399441055744.0;
-  double r = fma(kd, -0.6931471805599453 * 0.015625, x);
-  r = fma(kd, -2.3190468138462996e-17 * 0.015625, r);
-  double p = 1.0 / 120.0;
-  p = fma(p, r, 1.0 / 24.0);
-  p = fma(p, r, 1.0 / 6.0);
+  double r = fma(kd, c_expt[1], x);
+  r = fma(kd, c_expt[2], r);
+  const int kj = __double2loint(t);
+  const double tv = ckb_exp_table_at(kj);
+  double p = c_expt[3];
+  p = fma(p, r, c_expt[4]);
+  p = fma(p, r, c_expt[5]);
   p = fma(p, r, 0.5);
   p = fma(p, r, 1.0);
   p = fma(p, r, 1.0);
-  const int kj = __double2loint(t);
-  p *= ckb_exp_table()[kj & 63];
+  p *= tv;
   int k = kj >> 6;
   k = max(-1022, min(1022, k));
   return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
@@ -131,6 +144,39 @@ __device__ __forceinline__ double ckb_exp(double x, const ExpConst<PIN> &c) {
 /* N exponentials advanced in lock step (same arithmetic per chain as ckb_exp, non-table form): the N dependency
  * chains are emitted interleaved, step by step, so that a warp has N DFMAs in flight instead of one (the compiler
  * keeps the emission order; left to itself it runs the chains one after the other). */
+#if CKB_EXP_TABLE
+template <int N, bool PIN>
+__device__ __forceinline__ void ckb_exp_n(const double (&x)[N], double (&out)[N], const ExpConst<PIN> &) {
+  double t[N], r[N], p[N], tv[N];
+  double a0 = c_expt[0], a1 = c_expt[1], a2 = c_expt[2];
+  if (PIN) asm volatile("" : "+d"(a0), "+d"(a1), "+d"(a2));
+#pragma unroll
+  for (int u = 0; u < N; u++) t[u] = fma(x[u], a0, 6755399441055744.0);
+#pragma unroll
+  for (int u = 0; u < N; u++) tv[u] = ckb_exp_table_at(__double2loint(t[u]));
+#pragma unroll
+  for (int u = 0; u < N; u++) r[u] = fma(t[u] - 6755399441055744.0, a1, x[u]);
+#pragma unroll
+  for (int u = 0; u < N; u++) r[u] = fma(t[u] - 6755399441055744.0, a2, r[u]);
+#pragma unroll
+  for (int u = 0; u < N; u++) p[u] = fma(c_expt[3], r[u], c_expt[4]);
+#pragma unroll
+  for (int u = 0; u < N; u++) p[u] = fma(p[u], r[u], c_expt[5]);
+#pragma unroll
+  for (int u = 0; u < N; u++) p[u] = fma(p[u], r[u], 0.5);
+#pragma unroll
+  for (int u = 0; u < N; u++) p[u] = fma(p[u], r[u], 1.0);
+#pragma unroll
+  for (int u = 0; u < N; u++) p[u] = fma(p[u], r[u], 1.0);
+#pragma unroll
+  for (int u = 0; u < N; u++) {
+    p[u] *= tv[u];
+    int k = __double2loint(t[u]) >> 6;
+    k = max(-1022, min(1022, k));
+    out[u] = __hiloint2double(__double2hiint(p[u]) + (k << 20), __double2loint(p[u]));
+  }
+}
+#else
 template <int N, bool PIN>
 __device__ __forceinline__ void ckb_exp_n(const double (&x)[N], double (&out)[N], const ExpConst<PIN> &c) {
   double t[N], r[N], p[N];
@@ -158,6 +204,7 @@ __device__ __forceinline__ void ckb_exp_n(const double (&x)[N], double (&out)[N]
     out[u] = __hiloint2double(__double2hiint(p[u]) + (k << 20), __double2loint(p[u]));
   }
 }
+#endif
 
 #ifndef CKB_TMEM
 #define CKB_TMEM 0 /* warp-per-ODE integrate kernels: 1 = the reaction-slot table is read from tensor memory */
@@ -833,7 +880,7 @@ struct Rkc {
   XVec<S, 2, XSF> wjm2;
   XVec<S, 0, XS> v;
   double t, h, t1, Dt, rtol, atol, nd;
-  double sigma, err_old, h_old;
+  double sigma, err_old, h_old;                   /* err_old: CUBE ROOT of the previous accepted step's error norm */
   double pm_d, pm_sigma;                          /* power method: displacement size, last estimate */
   int state, j, s, s_max, pm_it, cbase;           /* cbase: this step's rows of the coefficient table */
   int nfe, nacc, nrej, smax_used, attempts, since_sigma, status, flag;
@@ -912,7 +959,11 @@ struct Rkc {
 
   /* Eq. 39 (R12), coefficients for j = 1, 2 (Eq. 22-26, R8-R10), first stage Eq. 19; true = failed */
   __device__ __forceinline__ bool take_step(const S &sys) {
-    s = 1 + (int)floor(sqrt(fma(1.54 * h, sigma, 1.0)));
+    {
+      const double x39 = fma(1.54 * h, sigma, 1.0);
+      /* x < 4 (and NaN: the cast of NaN is 0): floor(sqrt(x)) <= 1, so s = 2 without the square root */
+      s = (x39 >= 4.0) ? 1 + (int)floor(sqrt(x39)) : 2;
+    }
     if (s < 2) s = 2;
     if (s > s_max) {
       s = s_max;
@@ -1065,9 +1116,10 @@ struct Rkc {
     if (err <= 1.0) {
       nacc++;
       double fac;
+      double e3 = 0.0;
       if (err > 0.0) {
-        const double e3 = cbrt(err);
-        if (have_prev) fac = 0.8 * (cbrt(err_old) / e3) * (h / h_old) * (1.0 / e3); /* Eq. 34, R13 */
+        e3 = cbrt(err);
+        if (have_prev) fac = 0.8 * (err_old / e3) * (h / h_old) * (1.0 / e3); /* Eq. 34, R13; err_old = cbrt of that error */
         else fac = 0.8 / e3;
       } else fac = 10.0; /* R26 */
       fac = fmin(10.0, fmax(0.1, fac)); /* Eq. 33 */
@@ -1076,7 +1128,7 @@ struct Rkc {
         y.set(sys, i, w[i]);
         f0.set(sys, i, f[i]);
       }
-      err_old = err;
+      err_old = e3; /* the cube root is what Eq. 34 needs next time (cbrt(0) = 0 as well) */
       h_old = h;
       have_prev = true;
       sigma_fresh = false;
@@ -1228,46 +1280,37 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
     tm_fence_sync_fence();
   }
 #endif
-  /* queue positions: every group starts with M of its own, then pulls from the counter */
-  const long long n_static = (long long)gridDim.x * (BLOCK / 32) * G * M;
-  const long long grp_id = ((long long)blockIdx.x * (BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L;
-  typename IntegratorOf<S, METHOD>::type integ[M];
-  long long qi[M], ode[M];
-  bool need_load[M], active[M];
-  double f[M][NV];
+  /* queue positions: every group starts with one of its own, then pulls from the counter.  One system per group (M = 1):
+   * the loop state is kept in scalars -- as arrays indexed by the system of the group it stayed in local memory (flags,
+   * counters and a pointer were re-read from the stack on every evaluation of f(y): ~5 % of the stall samples). */
+  static_assert(M == 1, "integrate_kernel handles one system per group");
+  const long long n_static = (long long)gridDim.x * (BLOCK / 32) * G;
+  typename IntegratorOf<S, METHOD>::type integ;
+  long long qi = ((long long)blockIdx.x * (BLOCK / 32) + (threadIdx.x >> 5)) * G + (threadIdx.x & 31) / L, ode = 0;
+  bool need_load = true, active = true;
+  double f[1][NV];
+  sys.set_pressure(0, 1.0);
 #pragma unroll
-  for (int q = 0; q < M; q++) {
-    qi[q] = grp_id * M + q;
-    ode[q] = 0;
-    need_load[q] = true;
-    active[q] = true;
-    sys.set_pressure(q, 1.0);
-#pragma unroll
-    for (int i = 0; i < NV; i++) integ[q].w[i] = 1.0; /* finite argument for a slot that never gets a system */
-  }
+  for (int i = 0; i < NV; i++) integ.w[i] = 1.0; /* finite argument for a group that never gets a system */
   bool held_last = false;
   while (true) {
-    bool any = false;
+    if (need_load && active) {
+      if (qi >= N) {
+        active = false; /* queue exhausted: this group idles (its f(y) input stays at the last finite state) */
+      } else {
+        ode = order ? (long long)order[qi] : qi; /* queue position -> system */
+        sys.set_pressure(0, pressure ? pressure[ode] : p_uniform);
+        double y0[NV];
 #pragma unroll
-    for (int q = 0; q < M; q++) {
-      if (need_load[q] && active[q]) {
-        if (qi[q] >= N) {
-          active[q] = false; /* queue exhausted: this slot idles (its f(y) input stays at the last finite state) */
-        } else {
-          ode[q] = order ? (long long)order[qi[q]] : qi[q]; /* queue position -> system */
-          sys.set_pressure(q, pressure ? pressure[ode[q]] : p_uniform);
-          double y0[NV];
-#pragma unroll
-          for (int i = 0; i < NV; i++) {
-            const int c = sys.g + L * i;
-            y0[i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode[q]] : 0.0;
-          }
-          integ[q].start(sys, y0, t0, t0 + dt, rtol, atol, m.n);
-          need_load[q] = false;
+        for (int i = 0; i < NV; i++) {
+          const int c = sys.g + L * i;
+          y0[i] = (c < m.n) ? states[(size_t)sys.tw(m.o_perm + c) * ld + ode] : 0.0;
         }
+        integ.start(sys, y0, t0, t0 + dt, rtol, atol, m.n);
+        need_load = false;
       }
-      any = any || active[q];
     }
+    bool any = active;
 #if CKB_BLOCK_LOCKSTEP
     /* the warps of a block enter f(y) together (one instruction stream per block through the instruction caches:
      * the generated straight-line f(y) is larger than the 32 KB L1.5 I-cache) and leave the loop together */
@@ -1285,10 +1328,10 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
      * stage 2 (k1 rescaled, R25).  When some lane needs stage 1, the stage-2 lanes sit that evaluation out (their
      * argument is evaluated again next time: same values, not counted). */
     bool hold = false;
-    if constexpr (METHOD == 0 && L < 32 && M == 1 && CKB_RKCK_ALIGN != 0) {
-      const bool s1 = active[0] && integ[0].stage == 1;
+    if constexpr (METHOD == 0 && L < 32 && CKB_RKCK_ALIGN != 0) {
+      const bool s1 = active && integ.stage == 1;
       const bool any1 = __any_sync(0xffffffffu, s1); /* every lane votes */
-      hold = active[0] && !s1 && any1;
+      hold = active && !s1 && any1;
     }
     /* RKC with several systems per warp: a step with s stages is s - 1 stage evaluations (S_STAGE) and the evaluation of the error
      * estimate (S_FINAL); with lane refill and the occasional power-method excursion the lanes of a warp drift
@@ -1296,38 +1339,35 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
      * evaluation out when that lines it up with the majority: S_FINAL lanes wait for lanes that are in their last
      * stage, last-stage lanes wait for S_FINAL lanes (which start their next step's stages afterwards).  Never
      * twice in a row, so no lane starves. */
-    if constexpr (METHOD == 1 && L < 32 && M == 1 && CKB_RKC_ALIGN != 0) {
-      const int ph = active[0] ? integ[0].phase() : 0;
+    if constexpr (METHOD == 1 && L < 32 && CKB_RKC_ALIGN != 0) {
+      const int ph = active ? integ.phase() : 0;
       const int n_last = __popc(__ballot_sync(0xffffffffu, ph == 2)), n_final = __popc(__ballot_sync(0xffffffffu, ph == 3));
       hold = !held_last && ((ph == 3 && n_last > 0 && n_last >= n_final) || (ph == 2 && n_final > n_last));
       held_last = hold;
     }
-    /* an idle slot (queue exhausted) keeps evaluating its last argument: harmless, never stored */
-    sys.rhs([&](int q, int i) -> double { return integ[q].w[i]; }, f);
+    /* an idle group (queue exhausted) keeps evaluating its last argument: harmless, never stored */
+    sys.rhs([&](int, int i) -> double { return integ.w[i]; }, f);
+    if (active && !hold && integ.advance(sys, f[0])) {
+      int st[4];
+      integ.result(st);
 #pragma unroll
-    for (int q = 0; q < M; q++) {
-      if (active[q] && !hold && integ[q].advance(sys, f[q])) {
-        int st[4];
-        integ[q].result(st);
-#pragma unroll
-        for (int i = 0; i < NV; i++) {
-          const int c = sys.g + L * i;
-          if (c < m.n) states[(size_t)sys.tw(m.o_perm + c) * ld + ode[q]] = integ[q].y_at(sys, i);
-        }
-        if (sys.g == 0) {
-          if (status) status[ode[q]] = integ[q].status;
-          if (stats) {
-#pragma unroll
-            for (int k = 0; k < 4; k++) stats[(size_t)k * N + ode[q]] = st[k];
-          }
-        }
-        /* next system: lane refill (L = 1) / group refill */
-        unsigned long long nx = 0;
-        if (sys.g == 0) nx = atomicAdd(counter, 1ull);
-        if (L > 1) nx = __shfl_sync(sys.mask, nx, sys.src0);
-        qi[q] = n_static + (long long)nx;
-        need_load[q] = true;
+      for (int i = 0; i < NV; i++) {
+        const int c = sys.g + L * i;
+        if (c < m.n) states[(size_t)sys.tw(m.o_perm + c) * ld + ode] = integ.y_at(sys, i);
       }
+      if (sys.g == 0) {
+        if (status) status[ode] = integ.status;
+        if (stats) {
+#pragma unroll
+          for (int k = 0; k < 4; k++) stats[(size_t)k * N + ode] = st[k];
+        }
+      }
+      /* next system: lane refill (L = 1) / group refill */
+      unsigned long long nx = 0;
+      if (sys.g == 0) nx = atomicAdd(counter, 1ull);
+      if (L > 1) nx = __shfl_sync(sys.mask, nx, sys.src0);
+      qi = n_static + (long long)nx;
+      need_load = true;
     }
   }
 #if CKB_TMEM
