@@ -57,6 +57,8 @@ def parse():
     ap.add_argument("--no-specialize", action="store_true",
                     help="keep the table-driven thread-per-ODE kernels (no runtime-generated mechanism code)")
     ap.add_argument("--no-extra", action="store_true", help="skip the other configs, e2e and cpu_baseline")
+    ap.add_argument("--f1", action="store_true", help="the config's mechanism with two-range thermo and fall-off reactions (SURVEY 8(f)-f1)")
+    ap.add_argument("--cv", action="store_true", help="constant-volume closure (SURVEY 8(f)-f3)")
     ap.add_argument("--sweep", action="store_true", help="also sweep N over the config's N_list")
     args = ap.parse_args()
     RTOL, ATOL = args.rtol, args.atol   # every leg (ours, e2e, oracle) uses the same tolerances
@@ -323,7 +325,7 @@ def run_ours(args):
                   "frac_of_nominal": peak_flops / 1e12 / FP64_NOMINAL_TFLOPS}
     exp_rate = binding.fp64_probe("exp", 1 << 12)
     # every rank integrates its own N systems (independent problems, no data-path collective): weak scaling
-    case = GpuCase(args.config, N, dt, args.variant, args.ordering, local)
+    case = GpuCase(args.config, N, dt, args.variant, args.ordering, local, cv=args.cv, f1=args.f1)
     work = case.work()
     barrier()
     with ClockSampler(local) as clk:
@@ -342,7 +344,7 @@ def run_ours(args):
         "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config}]: {spec.name} species/reactions, {spec.method.upper()}, "
                                f"N={N} per GPU, dt={dt:g} s, rtol={RTOL:g}, atol={ATOL:g}",
-                   "N_per_gpu": N, "variant": args.variant, "ordering": args.ordering,
+                   "N_per_gpu": N, "variant": args.variant, "ordering": args.ordering, "f1": args.f1, "cv": args.cv,
                    "specialised": case.specialized, **({"specialise_error": case.specialize_error} if case.specialize_error else {}),
                    "l2": "flushed between timed steps (256 MiB write, untimed)",
                    "restart": "every step restarts from the same initial states (device copy, untimed)"},

@@ -1,5 +1,7 @@
-"""The N > 1 path of bench.py on CPU: two gloo ranks shard independent systems (no data-path collective);
-the only exchange is the barrier and the max-over-ranks of the per-rank time."""
+"""The N > 1 protocol of bench.py on CPU: two gloo ranks shard independent systems (no data-path collective); the only
+exchange is the barrier and the max-over-ranks of the per-rank time.  What integrates here is the ORACLE
+(there is no GPU on the CPU box and the product has no CPU path): the test covers the sharding, the barrier and the
+reduction of the timing, not the CUDA kernels -- those have no inter-rank step at all ("replicas only")."""
 import os
 import socket
 import subprocess
