@@ -104,8 +104,8 @@ void ckb_mech_free(ckb_mech *m);
 /*
  * ckb_mech_reserve: size the handle's work-queue order scratch for batches of up to max_batch systems (the paper's
  * "global step over all grid points"; "any scratch is sized at load time or passed by the
- * caller").  Synchronises the device and (re)allocates; call it between steps, never concurrently with work on the
- * handle.  ckb_integrate refuses a batch beyond the reserved size with CKB_ECAPACITY (batches below 4096 systems need
+ * caller").  Grow-only (a smaller max_batch than what is reserved changes nothing).  Synchronises the device and
+ * (re)allocates; call it between steps, never concurrently with work on the handle.  ckb_integrate refuses a batch beyond the reserved size with CKB_ECAPACITY (batches below 4096 systems need
  * no scratch).
  */
 #define CKB_DEFAULT_MAX_BATCH (1 << 20)

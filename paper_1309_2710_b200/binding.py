@@ -332,6 +332,7 @@ def integrate(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None,
 
 
 STATIC_MAX_BATCH = 524288
+DEFAULT_MAX_BATCH = 1 << 20   # CKB_DEFAULT_MAX_BATCH: what ckb_mech_load reserves for ckb_integrate
 
 
 def integrate_static(m: Mech, states, dt, rtol, atol, method, *, N=None, t=0.0, p=None, pressure=None,

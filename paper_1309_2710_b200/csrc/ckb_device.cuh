@@ -526,7 +526,7 @@ struct Sys {
           const double kf = ckb_exp(xf, ec), kr = ckb_exp(xr, ec);
           const double qs = (kf * pf - kr * pr) * CKB_AT(tb);
           qp[q * RS] = qs;
-          if (L > 1) qp[q * RS + m.NSR * L] = -qs; /* the gather reads -q_s where the coefficient is -1 */
+          if (L == CKB_NEGQ_L) qp[q * RS + m.NSR * L] = -qs; /* the gather reads -q_s where the coefficient is -1 */
 #undef CKB_AT
         }
       }
@@ -553,6 +553,20 @@ struct Sys {
 #pragma unroll
           for (int q = 0; q < M; q++)
             acc0[q] = fma(coef, *reinterpret_cast<const double *>(reinterpret_cast<const char *>(sQ + q * RS) + o), acc0[q]);
+        }
+      } else if (L < CKB_NEGQ_L) { /* two entries per word: (sign of the coefficient in bit 31) | q offset; the sign is
+                  XOR-ed into q (exactly fma(+-1, q, acc)); |nu| > 1 is entered |nu| times, an idle entry reads a 0.0 slot */
+        for (int t = 0; t < len; t++, gp += L) {
+          const unsigned long long w = tw(gp);
+          const unsigned lo = (unsigned)w, hi = (unsigned)(w >> 32);
+          const unsigned o0 = lo & 0xFFFFu, o1 = hi & 0xFFFFu;
+#pragma unroll
+          for (int q = 0; q < M; q++) {
+            const char *qb = reinterpret_cast<const char *>(sQ + q * RS);
+            const double q0 = *reinterpret_cast<const double *>(qb + o0), q1 = *reinterpret_cast<const double *>(qb + o1);
+            acc0[q] += __hiloint2double(__double2hiint(q0) ^ (int)(lo & 0x80000000u), __double2loint(q0));
+            acc1[q] += __hiloint2double(__double2hiint(q1) ^ (int)(hi & 0x80000000u), __double2loint(q1));
+          }
         }
       } else { /* four entries per word, each the byte offset of q_s (coefficient +1), of -q_s (coefficient -1: the slot
                   loop stores both) or of one of the 0.0 slots behind them (idle entry): an extract, a shared read and
@@ -1229,7 +1243,7 @@ __device__ __forceinline__ void sys_setup(S &sys, const DevMech &m, double *smem
   if (L > 1 && sys.g < CKB_ZERO_SLOTS) { /* the operands of idle gather entries (a group has >= 2 lanes: loop) */
     for (int z = sys.g; z < CKB_ZERO_SLOTS; z += L) {
 #pragma unroll
-      for (int q = 0; q < M; q++) sys.sR[q * sys.RS + sys.qoff + 2 * m.NSR * L + z] = 0.0;
+      for (int q = 0; q < M; q++) sys.sR[q * sys.RS + sys.qoff + (L == CKB_NEGQ_L ? 2 : 1) * m.NSR * L + z] = 0.0;
     }
   }
 #endif

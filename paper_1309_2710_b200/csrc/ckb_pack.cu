@@ -472,7 +472,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   for (auto &s : P.sets) TBE = std::max(TBE, (int)s.size());
   /* 16-bit region offsets, in bytes */
   if ((long long)(n + NTB + 1) * G * 8 > 65535 ||
-      ((long long)NSR * L * (L > 1 ? 2 : 1) + (L > 1 ? CKB_ZERO_SLOTS : 0)) * G * 8 > 65535) /* q, -q and the 0.0 slots of idle entries */
+      ((long long)NSR * L * (L == CKB_NEGQ_L ? 2 : 1) + (L > 1 ? CKB_ZERO_SLOTS : 0)) * G * 8 > 65535) /* q, -q and the 0.0 slots of idle entries */
     return CKB_EUNSUPPORTED;
   const bool optimise = true;
 
@@ -501,6 +501,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
   std::vector<int> pos_of_slot(NS, -1);
   for (int q = 0; q < NSR * L; q++)
     if (placed[q].slot >= 0) pos_of_slot[placed[q].slot] = q;
+  const int per_word_L = (L == 1) ? 1 : (L == CKB_NEGQ_L) ? 4 : 2; /* gather entries per 64-bit table word */
   std::vector<std::vector<std::vector<GEntry>>> sched(NV);
   std::vector<int> glen(NV, 0); /* 64-bit words per lane: two entries per word */
   for (int i = 0; i < NV; i++) {
@@ -530,9 +531,10 @@ int pack_for(const Parsed &P, int L, Packed &out) {
       }
     }
     sched[i] = colour_gather(rows, L, optimise, /*relaxed=*/true);
-    glen[i] = (L == 1) ? (int)sched[i].size() : ((int)sched[i].size() + 3) / 4;
+    glen[i] = (L == 1) ? (int)sched[i].size() : ((int)sched[i].size() + per_word_L - 1) / per_word_L;
   }
   const int gwords = std::accumulate(glen.begin(), glen.end(), 0);
+  const int qcopies = (L == CKB_NEGQ_L) ? 2 : 1;
   const int s_tab = (L == 1) ? 12 : 48;
 
   ckb::DevMech &m = out.dm;
@@ -651,7 +653,7 @@ int pack_for(const Parsed &P, int L, Packed &out) {
     out.gather_excess_wavefronts = 0;
     for (int i = 0; i < NV; i++) {
       b[(size_t)m.o_glen + i] = (unsigned long long)glen[i];
-      const int per_word = (L == 1) ? 1 : 4;
+      const int per_word = per_word_L;
       for (int t = 0; t < per_word * glen[i]; t++) {
         std::vector<int> addr(L >= 16 ? L : 0, -1);
         for (int g = 0; g < L; g++) {
@@ -671,15 +673,18 @@ int pack_for(const Parsed &P, int L, Packed &out) {
               for (int r0 = 0; r0 < 16; r0++)
                 if (!busy[r0]) { e.pos = r0; break; }
             }
-            if (zero_slot) e.pos = 2 * NSR * L + ((e.pos - 2 * NSR * L) % 16 + 16) % 16; /* same bank pair, behind q and -q */
+            if (zero_slot) e.pos = qcopies * NSR * L + ((e.pos - qcopies * NSR * L) % 16 + 16) % 16; /* same bank pair, behind q (and -q) */
           }
           if (L >= 16) addr[g] = e.pos;
           if (L == 1) { /* double coefficient with the q offset in its 16 lowest mantissa bits */
             b[(size_t)m.o_gat + (size_t)(w0 + t) * L + g] =
                 (dbits((double)e.coef) & ~0xFFFFull) | (unsigned long long)(e.pos * G * 8);
-          } else { /* coefficient -1: the entry points at -q_s, NSR*L doubles behind q_s (the same bank pair) */
+          } else if (L == CKB_NEGQ_L) { /* coefficient -1: the entry points at -q_s, NSR*L doubles behind q_s (the same bank pair) */
             const int pos = (e.coef < 0 && e.pos < NSR * L) ? e.pos + NSR * L : e.pos;
             b[(size_t)m.o_gat + (size_t)(w0 + t / 4) * L + g] |= (unsigned long long)(pos * G * 8) << (16 * (t & 3));
+          } else { /* (sign of the coefficient in bit 31) | offset, two per word */
+            const unsigned long long ent = ((e.coef < 0 && e.pos < NSR * L) ? 0x80000000ull : 0ull) | (unsigned long long)(e.pos * G * 8);
+            b[(size_t)m.o_gat + (size_t)(w0 + t / 2) * L + g] |= ent << (32 * (t & 1));
           }
         }
         if (L >= 16) out.gather_excess_wavefronts += excess_wavefronts(addr);

@@ -13,8 +13,8 @@
  *   [0, n)            C_c, concentration of component c; C_0 = 1.0 stands for "no molecule"
  *   [n, n+NTB+1)      [M]_t per third-body efficiency set; the last one = 1.0 stands for "no third body"
  *   [n+NTB+1, +NSR*L) q_s, net rate of progress of reaction slot s
- *   L > 1: then NSR*L doubles -q_s (so that the Eq. 3 gather applies a coefficient of +1 / -1 by WHERE it reads), then
- *          16 doubles of 0.0 (one per bank pair), the operand of an idle entry of the gather
+ *   L = 32: then NSR*L doubles -q_s (so that the Eq. 3 gather applies a coefficient of +1 / -1 by WHERE it reads)
+ *   L > 1: then 16 doubles of 0.0 (one per bank pair), the operand of an idle entry of the gather
  */
 #pragma once
 #ifndef __CUDACC__
@@ -72,9 +72,11 @@ struct DevMech {
   int o_rflag;       /* [NSR]              round flags: 1 = a third molecule is read, 2 = a third body is read   */
   int o_tb;          /* [NTBR][TBE][2][L]  (alpha-1, region byte offset of the species)                        */
   int o_glen;        /* [NV]               64-bit words per lane of gather level i (uniform over lanes)   */
-  int o_gat;         /* [sum glen][L]      gather entries.  L > 1: four per word, each the 16-bit BYTE offset inside
+  int o_gat;         /* [sum glen][L]      gather entries.  L = 32: four per word, each the 16-bit BYTE offset inside
                                            the q region of q_s (coefficient +1), of -q_s (coefficient -1) or of a 0.0
-                                           slot (idle); |nu| > 1 is entered nu times.  L = 1: one per word, double
+                                           slot (idle).  1 < L < 32 (shared memory is what limits those mappings: no
+                                           -q copies): two per word, (sign of the coefficient in bit 31) | BYTE offset
+                                           of q_s.  |nu| > 1 is entered nu times.  L = 1: one per word, double
                                            coefficient with the offset in its low 16 bits */
   int o_rkc;         /* RKC coefficients for s = 2..s_tab: [s-2] -> mu~_1; stages at o_rkcs               */
   int o_rkcs;        /* [(s-2)(s-1)/2 + (j-2)][4] = mu_j, nu_j, mu~_j, gamma~_j, j = 2..s                  */
@@ -93,8 +95,9 @@ struct DevMech {
 
 /* doubles of shared memory per system: C region, [M] region, q region */
 #define CKB_ZERO_SLOTS 16 /* L > 1: 0.0 in every bank pair behind the q region, read by idle gather entries */
+#define CKB_NEGQ_L 32     /* the mapping whose slot loop stores -q_s beside q_s (warp-per-ODE) */
 __host__ __device__ __forceinline__ int region_doubles(const DevMech &m) {
-  return m.n + m.NTB + 1 + m.NSR * m.L + (m.L > 1 ? m.NSR * m.L + CKB_ZERO_SLOTS : 0);
+  return m.n + m.NTB + 1 + m.NSR * m.L + (m.L == CKB_NEGQ_L ? m.NSR * m.L : 0) + (m.L > 1 ? CKB_ZERO_SLOTS : 0);
 }
 
 }  // namespace ckb

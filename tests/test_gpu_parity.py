@@ -374,6 +374,35 @@ def test_mid_size_auto_sampled(cfg, N, n_sample):
     print(f"mid size cfg{cfg} N={N}: {rep}")
 
 
+def test_reserved_batch_size_is_enforced_without_allocation():
+    """ckb_integrate allocates nothing: its queue-order scratch is sized by ckb_mech_load / ckb_mech_reserve, and a batch
+    beyond the reserved size is refused (CKB_ECAPACITY) with the states untouched; after reserving more it runs."""
+    import torch
+    from paper_1309_2710_b200 import binding
+    mech = synth.make_mechanism(1)
+    N = binding.DEFAULT_MAX_BATCH + 1                        # one more than ckb_mech_load reserves
+    base, p = synth.make_states(1, 4096)
+    states = np.ascontiguousarray(np.tile(base, (1, N // 4096 + 1))[:, :N])
+    m = binding.mech_load(mech)
+    dev = torch.from_numpy(states).cuda()
+    with pytest.raises(binding.CkbError) as e:
+        binding.integrate(m, dev, 1e-6, RTOL, ATOL, "rkck", p=p, variant="thread")
+    assert e.value.code == binding.ECAPACITY
+    torch.cuda.synchronize()
+    assert torch.equal(dev, torch.from_numpy(states).cuda())   # nothing was launched
+    m.reserve(N)
+    status = torch.full((N,), -7, dtype=torch.int32, device="cuda")
+    stats = torch.full((4, N), -7, dtype=torch.int32, device="cuda")
+    before = torch.cuda.memory_allocated()
+    binding.integrate(m, dev, 1e-6, RTOL, ATOL, "rkck", p=p, variant="thread", status=status, stats=stats)
+    torch.cuda.synchronize()
+    assert torch.cuda.memory_allocated() == before           # (torch's own allocator: the call made no tensor either)
+    m.close()
+    pick = np.arange(0, N, 30)
+    ora = _oracle(mech, np.ascontiguousarray(states[:, pick]), p, 1e-6, "rkck")
+    _compare((dev.cpu().numpy()[:, pick], status.cpu().numpy()[pick], stats.cpu().numpy()[:, pick]), ora)
+
+
 def test_empty_and_single():
     import torch
     from paper_1309_2710_b200 import binding
