@@ -287,7 +287,7 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": 1e3 * N / value, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config}]: {spec.name} species/reactions, {spec.method.upper()}, "
-                               f"N={N}, dt={dt:g} s, rtol={RTOL:g}, atol={ATOL:g}", "N": N, "sample_n": n_used},
+                               f"N={N} per GPU, dt={dt:g} s, rtol={RTOL:g}, atol={ATOL:g}", "N_per_gpu": N, "sample_n": n_used},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
