@@ -128,6 +128,28 @@ int parse_mechanism(const ckb_mech_desc *d, Parsed &P, const FoDesc *fo) {
     }
   }
   if (P.sets.size() > 65000) return CKB_EUNSUPPORTED;
+  if (!P.fo.empty()) {
+    /* Efficiency sets in the order Troe, Lindemann, ordinary: the lane-distributed kernels evaluate the blending factors
+     * set round by set round, each lane its own set -- grouped like this the fall-off sets fill whole rounds with lanes
+     * that all do the same work, and the rounds of ordinary sets skip the pass (53/634 with 51 fall-off reactions: 2 busy
+     * rounds instead of 4 half-idle ones). */
+    P.fo.resize(P.sets.size());
+    std::vector<int> order(P.sets.size()), new_id(P.sets.size());
+    std::iota(order.begin(), order.end(), 0);
+    auto rank = [&](int t) { return P.fo[t].kind >= 2 ? 0 : P.fo[t].kind == 1 ? 1 : 2; };
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rank(a) < rank(b); });
+    std::vector<std::vector<std::pair<int, double>>> sets2(P.sets.size());
+    std::vector<Parsed::Fo> fo2(P.sets.size());
+    for (size_t q = 0; q < order.size(); q++) {
+      new_id[order[q]] = (int)q;
+      sets2[q] = P.sets[order[q]];
+      fo2[q] = P.fo[order[q]];
+    }
+    P.sets.swap(sets2);
+    P.fo.swap(fo2);
+    for (int j = 0; j < R; j++)
+      if (rx[j].tbset >= 0) rx[j].tbset = new_id[rx[j].tbset];
+  }
 
   /* fuse forward / reverse reactions over the same species (and the same third body) into one slot */
   typedef std::pair<std::pair<std::vector<int>, std::vector<int>>, int> Key;
