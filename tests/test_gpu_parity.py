@@ -403,6 +403,38 @@ def test_reserved_batch_size_is_enforced_without_allocation():
     _compare((dev.cpu().numpy()[:, pick], status.cpu().numpy()[pick], stats.cpu().numpy()[:, pick]), ora)
 
 
+def test_concurrent_calls_on_two_streams_with_one_handle_each():
+    """include/ckb.h: calls on one handle share its scratch and must be stream-ordered; for concurrent calls load one
+    handle per stream.  Two handles, two streams, launched back to back without synchronisation in between: each result
+    equals the one the same call gives alone."""
+    import torch
+    from paper_1309_2710_b200 import binding
+    mech = synth.make_mechanism(1)
+    N = 60000
+    states, p = synth.make_states(1, 2 * N)
+    halves = [np.ascontiguousarray(states[:, :N]), np.ascontiguousarray(states[:, N:])]
+    handles = [binding.mech_load(mech), binding.mech_load(mech)]
+    alone = []
+    for h, st in zip(handles, halves):
+        dev = torch.from_numpy(st).cuda()
+        binding.integrate(h, dev, 1e-6, RTOL, ATOL, "rkck", p=p, variant="thread")
+        torch.cuda.synchronize()
+        alone.append(dev.cpu().numpy())
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    devs = [torch.from_numpy(st).cuda() for st in halves]
+    torch.cuda.synchronize()
+    for rep in range(3):                                   # several rounds: the launches really overlap
+        for h, dev, st, s in zip(handles, devs, halves, streams):
+            with torch.cuda.stream(s):
+                dev.copy_(torch.from_numpy(st), non_blocking=False)
+                binding.integrate(h, dev, 1e-6, RTOL, ATOL, "rkck", p=p, variant="thread", stream=s)
+    torch.cuda.synchronize()
+    for dev, ref in zip(devs, alone):
+        assert np.array_equal(dev.cpu().numpy(), ref)
+    for h in handles:
+        h.close()
+
+
 def test_empty_and_single():
     import torch
     from paper_1309_2710_b200 import binding
