@@ -30,11 +30,16 @@
  *                              incl. the orientation of Eq. 34's memory term and the [0.1, 10] clamp; Eq. 36-38 by
  *                              hand; Eq. 39 truncated with dt sigma inside the stability interval; the 25-step /
  *                              after-rejection refresh of sigma.
+ *   ora_fit_reverse / ora_equilibrium_constant / ora_reverse_parameters (Appendix A, tests/test_oracle_convert.py):
+ *                              exact round trip of three points of a known Arrhenius law, numpy's 3 x 3 linear solve,
+ *                              closed-form reverse parameters on species with a1, a6, a7 only (dnu = 0 and 1), the
+ *                              equilibrium ratio reached by the integrated forward / fitted-reverse pair.
  *   PARITY UNPINNED (builder's reading, nothing in the paper or the mathematics fixes them; the traces pin that the
  *   code does what the reading says, not that the reading is the only possible one):
  *   R4 (RKCK first trial step), R5 (end-of-interval clipping), R6/R7 (failure codes), R10 (b_1 = b_2 for
  *   nonlinear f), R13 (controller memory dropped after a rejection), R14/R15 (initial-step weights and cap),
- *   R16 (sigma refreshed after a rejection only when stale), R17/R18 (power-method details and its 1.2 safety factor).
+ *   R16 (sigma refreshed after a rejection only when stale), R17/R18 (power-method details and its 1.2 safety factor),
+ *   R32 (the equilibrium constant in the Chemkin form), R33 (the three fitting temperatures).
  */
 #include <math.h>
 #include <stdint.h>
