@@ -1332,9 +1332,12 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
     }
     bool any = active;
 #if CKB_BLOCK_LOCKSTEP
-    /* the warps of a block enter f(y) together (one instruction stream per block through the instruction caches:
-     * the generated straight-line f(y) is larger than the 32 KB L1.5 I-cache) and leave the loop together */
-    {
+    /* RKC: the warps of a block enter f(y) together (one instruction stream per block through the instruction caches:
+     * the generated straight-line f(y) is larger than the 32 KB L1.5 I-cache) and leave the loop together.  RKCK runs
+     * its warps independently: with the lanes of a warp stage-aligned its advance() is a few vector updates, and the
+     * barrier cost more than the shared instruction stream saved (configs[1]: 9.32e8 -> 1.03e9 ODE/s without it; lock
+     * step in 2, 3, 4, 6 groups of warps was measured in between; RKC loses 16 % with two groups already). */
+    if constexpr (METHOD == 1) {
       const bool mine = any;
       any = __syncthreads_or(any);
       /* a warp that has run out of systems only keeps the barrier: the stragglers of the block get its issue slots */
