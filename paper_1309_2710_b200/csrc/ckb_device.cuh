@@ -32,6 +32,9 @@ namespace ckb {
 #ifndef CKB_XS_RKC_F0
 #define CKB_XS_RKC_F0 0 /* thread-per-ODE RKC: 1 = f0 and w_{j-2} live in the shared scratch too */
 #endif
+#ifndef CKB_RKC_BLOCK_ALIGN
+#define CKB_RKC_BLOCK_ALIGN 1 /* ... and, in a lock-step block, over the warps of the block */
+#endif
 #ifndef CKB_BLOCK_LOCKSTEP
 #define CKB_BLOCK_LOCKSTEP 0
 #endif
@@ -1313,6 +1316,11 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
 #pragma unroll
   for (int i = 0; i < NV; i++) integ.w[i] = 1.0; /* finite argument for a group that never gets a system */
   bool held_last = false;
+  constexpr bool BALIGN = CKB_BLOCK_LOCKSTEP != 0 && METHOD == 1 && L < 32 && CKB_RKC_ALIGN != 0 && CKB_RKC_BLOCK_ALIGN != 0;
+#if CKB_BLOCK_LOCKSTEP
+  __shared__ unsigned ls_ph[64];
+  unsigned ls_iter = 0;
+#endif
   while (true) {
     if (need_load && active) {
       if (qi >= N) {
@@ -1331,6 +1339,7 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
       }
     }
     bool any = active;
+    int b_last = 0, b_final = 0;
 #if CKB_BLOCK_LOCKSTEP
     /* RKC: the warps of a block enter f(y) together (one instruction stream per block through the instruction caches:
      * the generated straight-line f(y) is larger than the 32 KB L1.5 I-cache) and leave the loop together.  RKCK runs
@@ -1339,7 +1348,19 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
      * step in 2, 3, 4, 6 groups of warps was measured in between; RKC loses 16 % with two groups already). */
     if constexpr (METHOD == 1) {
       const bool mine = any;
+      if constexpr (BALIGN) { /* this warp's lanes in their last stage / at the error estimate, for the block-wide vote below */
+        const int ph = active ? integ.phase() : 0;
+        const unsigned w_last = __popc(__ballot_sync(0xffffffffu, ph == 2)), w_final = __popc(__ballot_sync(0xffffffffu, ph == 3));
+        if ((threadIdx.x & 31) == 0) ls_ph[(ls_iter & 1) * 32 + (threadIdx.x >> 5)] = w_last | (w_final << 16);
+      }
       any = __syncthreads_or(any);
+      if constexpr (BALIGN) {
+        const int lane = threadIdx.x & 31;
+        const unsigned v = __reduce_add_sync(0xffffffffu, lane < BLOCK / 32 ? ls_ph[(ls_iter & 1) * 32 + lane] : 0u);
+        b_last = (int)(v & 0xFFFFu);
+        b_final = (int)(v >> 16);
+        ls_iter++; /* double buffer: a warp writes its next counts while a slower one may still read these */
+      }
       /* a warp that has run out of systems only keeps the barrier: the stragglers of the block get its issue slots */
       if (any && !__any_sync(0xffffffffu, mine)) continue;
     }
@@ -1364,7 +1385,10 @@ integrate_kernel(const __grid_constant__ DevMech m, const __grid_constant__ TAB 
      * twice in a row, so no lane starves. */
     if constexpr (METHOD == 1 && L < 32 && CKB_RKC_ALIGN != 0) {
       const int ph = active ? integ.phase() : 0;
-      const int n_last = __popc(__ballot_sync(0xffffffffu, ph == 2)), n_final = __popc(__ballot_sync(0xffffffffu, ph == 3));
+      /* block lock step: the vote is taken over the block, so that its warps reach the error estimate -- the long path of
+       * advance(), which every warp waits for at the barrier -- on the same evaluations */
+      const int n_last = BALIGN ? b_last : __popc(__ballot_sync(0xffffffffu, ph == 2));
+      const int n_final = BALIGN ? b_final : __popc(__ballot_sync(0xffffffffu, ph == 3));
       hold = !held_last && ((ph == 3 && n_last > 0 && n_last >= n_final) || (ph == 2 && n_final > n_last));
       held_last = hold;
     }
