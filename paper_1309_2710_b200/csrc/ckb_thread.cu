@@ -165,7 +165,7 @@ int thread_upload(ThreadPack &tp) {
   CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   CK(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
   const size_t per_warp = (size_t)2 * tp.dm.n * 32 * sizeof(double);
-  int warps = (int)((size_t)smem_max / per_warp);
+  int warps = (int)(((size_t)smem_max - 256) / per_warp); /* 256 B: the static words of the block-wide stage vote */
   if (warps > CKBT_MAX_BLOCK / 32) warps = CKBT_MAX_BLOCK / 32;
   if (warps < 1) return CKB_EUNSUPPORTED;
   tp.warps = warps;

@@ -874,6 +874,10 @@ integrate_thread_kernel(const __grid_constant__ DevThread m, const __grid_consta
   typename MemIntegratorOf<S, METHOD>::type integ;
   long long qi = (long long)blockIdx.x * blockDim.x + threadIdx.x, ode = 0;
   bool need_load = true, active = true, held_last = false;
+#if CKBT_LOCKSTEP
+  __shared__ unsigned ls_ph[64];
+  unsigned ls_iter = 0;
+#endif
   sys.set_pressure(1.0);
   integ.iw = 0;
   for (int i = 0; i < n; i++) sys.V(0, i) = 1.0; /* finite argument for a lane that never gets a system */
@@ -893,7 +897,20 @@ integrate_thread_kernel(const __grid_constant__ DevThread m, const __grid_consta
      * code of one trip is several times the 32 KB L1.5); a warp that has run out of systems only keeps the barrier */
     const bool warp_any = __any_sync(0xffffffffu, active);
 #if CKBT_LOCKSTEP
+    int b_last = 0, b_final = 0;
+    if constexpr (METHOD == 1) { /* this warp's lanes in their last stage / at the error estimate, for the block-wide vote */
+      const int ph = active ? integ.phase() : 0;
+      const unsigned w_last = __popc(__ballot_sync(0xffffffffu, ph == 2)), w_final = __popc(__ballot_sync(0xffffffffu, ph == 3));
+      if ((threadIdx.x & 31) == 0) ls_ph[(ls_iter & 1) * 32 + (threadIdx.x >> 5)] = w_last | (w_final << 16);
+    }
     if (!__syncthreads_or(warp_any)) break;
+    if constexpr (METHOD == 1) {
+      const int lane = threadIdx.x & 31;
+      const unsigned v = __reduce_add_sync(0xffffffffu, lane < (int)(blockDim.x >> 5) ? ls_ph[(ls_iter & 1) * 32 + lane] : 0u);
+      b_last = (int)(v & 0xFFFFu);
+      b_final = (int)(v >> 16);
+      ls_iter++; /* double buffer: a warp writes its next counts while a slower one may still read these */
+    }
     if (!warp_any) continue;
 #else
     if (!warp_any) break;
@@ -905,7 +922,11 @@ integrate_thread_kernel(const __grid_constant__ DevThread m, const __grid_consta
       hold = active && !s1 && any1;
     } else { /* RKC: last-stage and error-estimate evaluations line up (never held twice in a row) */
       const int ph = active ? integ.phase() : 0;
+#if CKBT_LOCKSTEP /* the vote is taken over the block: its warps reach the error estimate, the long path of advance(), together */
+      const int n_last = b_last, n_final = b_final;
+#else
       const int n_last = __popc(__ballot_sync(0xffffffffu, ph == 2)), n_final = __popc(__ballot_sync(0xffffffffu, ph == 3));
+#endif
       hold = !held_last && ((ph == 3 && n_last > 0 && n_last >= n_final) || (ph == 2 && n_final > n_last));
       held_last = hold;
     }
